@@ -1,0 +1,367 @@
+// oracle/lbm_oracle.cpp
+//
+// TEST INFRASTRUCTURE — NOT THE PRODUCT.  This is the plain, slow, CPU oracle of
+// the lattice-Boltzmann hot path of IMEXLBM (arXiv 2201.11330).  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// build, load or call it.  It shares no code, header, table or constant with the
+// CUDA path under paper_2201_11330_b200/csrc/ and includes nothing from it.
+//
+// It follows the paper step by step, un-fused, in the paper's own order
+// (section 3.1): Collision -> BoundaryCondition -> Propagation ->
+// PostProcessing, on the paper's two arrays `f` and `fb` (Table 3)
+// in the paper's array-of-structures indexing f(id*nq+iq).
+// "P:n" below = /root/reference/PAPER.md line n.  "D:Rk" = reading Rk in DESIGN.md
+// (points where the paper is silent and BASELINE.json fixes the behaviour).
+//
+// Pin status (tests/test_oracle_pins.py, run with -m "not gpu"):
+//   lattice tables ............ pinned: Eq. 3-4 as printed (tests/golden), isotropy identities
+//   equilibrium Eq. 2 / Eq. 5 . pinned: moment identities, fixed point, P:375 constants
+//   collision + propagation ... pinned: conservation, Taylor-Green decay rate, shear-wave decay
+//   halfway bounce-back ....... pinned: Poiseuille parabola + BGK slip constant (closed form)
+//   moving wall (Ladd) ........ pinned: planar Couette exact linear profile, cavity mass
+//   Guo forcing ............... pinned: momentum gain F*N per step, Poiseuille
+//   indexing .................. pinned: independent brute-force gather on 4^3 (long double)
+//   D3Q27 ..................... pinned only through the same invariants and closed forms;
+//                               no D3Q27-specific printed value exists in the paper.
+//
+// Floating point: IEEE double throughout ("double precision"); compile with
+// -ffp-contract=off so that no FMA contraction happens.  Reductions for the
+// diagnostics are accumulated in long double.
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+struct Lattice {
+  int Q = 0;
+  int e[27][3];
+  double t[27];
+};
+
+// Velocity set and weights.  P:49-53: the paper prints only D2Q9 (Eq. 3-4); its
+// columns run lexicographically over (e_x, e_y), each component -1 -> 0 -> +1, e_x
+// outermost, which gives the stated property opposite(alpha) = m-1-alpha.
+// D:R4: the 3-D sets extend the same rule to (e_x, e_y, e_z); D3Q19 is that list
+// without the 8 corner vectors.  Weights by squared speed (Qian et al., refs [11],
+// [12] cited at P:43).  Q = 9 is the printed D2Q9 itself (e_z = 0).
+bool make_lattice(int Q, Lattice& L) {
+  if (Q != 9 && Q != 19 && Q != 27) return false;
+  L.Q = Q;
+  int q = 0;
+  for (int ex = -1; ex <= 1; ++ex)
+    for (int ey = -1; ey <= 1; ++ey)
+      for (int ez = -1; ez <= 1; ++ez) {
+        const int s = ex * ex + ey * ey + ez * ez;
+        if (Q == 9 && ez != 0) continue;
+        if (Q == 19 && s == 3) continue;
+        double w = 0.0;
+        if (Q == 9) w = (s == 0) ? 4.0 / 9.0 : (s == 1) ? 1.0 / 9.0 : 1.0 / 36.0;
+        if (Q == 19) w = (s == 0) ? 1.0 / 3.0 : (s == 1) ? 1.0 / 18.0 : 1.0 / 36.0;
+        if (Q == 27)
+          w = (s == 0) ? 8.0 / 27.0 : (s == 1) ? 2.0 / 27.0 : (s == 2) ? 1.0 / 54.0 : 1.0 / 216.0;
+        L.e[q][0] = ex;
+        L.e[q][1] = ey;
+        L.e[q][2] = ez;
+        L.t[q] = w;
+        ++q;
+      }
+  return q == Q;
+}
+
+enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };              // Eq. 2 | Eq. 5
+enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2 };
+
+struct Oracle {
+  int nx, ny, nz;
+  int64_t N;
+  Lattice L;
+  int eq;            // EQ_STANDARD or EQ_INCOMP
+  double omega;      // P:61-63 Eq. 6: 1/(tau/dt + 1/2); D:R1: API tau = tau_paper/dt + 1/2
+  double rho0;       // constant density of the incompressible model, 1
+  int face_kind[6];  // x-, x+, y-, y+, z-, z+
+  double face_u[6][3];
+  double F[3];       // uniform body force density (D:R7, Guo forcing; not in the paper)
+  std::vector<double> f;      // P:208 `f`:  pre-collision populations, AoS f[id*Q+iq]
+  std::vector<double> fb;     // P:208 `fb`: "backup" = post-collision populations
+  std::vector<double> rho_w;  // density seen by the collision sweep, kept for the wall term (D:R6)
+  int64_t steps_done = 0;
+
+  int64_t cell(int x, int y, int z) const { return (int64_t)x + (int64_t)nx * ((int64_t)y + (int64_t)ny * z); }
+};
+
+// Eq. 2 with c_s^2 = 1/3  (P:375-376 prints the constants 3, 4.5, 1.5):
+//   feq = t rho [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]
+// Eq. 5 (code form P:375): feq = t [ p/c_s^2 + rho0 (3 e.u + 4.5 (e.u)^2 - 1.5 u.u) ],
+//   where `rho` below stands for p/c_s^2 = sum_alpha f_alpha (Eq. 8).
+inline double feq_value(const Oracle& o, int iq, double rho, const double u[3]) {
+  double edu = 0.0, udu = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    edu += o.L.e[iq][d] * u[d];
+    udu += u[d] * u[d];
+  }
+  if (o.eq == EQ_STANDARD) return o.L.t[iq] * rho * (1.0 + 3.0 * edu + 4.5 * edu * edu - 1.5 * udu);
+  return o.L.t[iq] * (rho + o.rho0 * (3.0 * edu + 4.5 * edu * edu - 1.5 * udu));
+}
+
+// Moments, Eq. 8-9:  rho = sum f (= p/c_s^2),  u = (1/rho) sum e f.
+// D:R5: under Eq. 5 the divisor is the constant rho0 (the code multiplies the velocity
+// terms by rho0).  D:R7: with a body force the velocity carries the half-force
+// shift, u = (sum e f + F/2)/rho (Guo et al.).
+inline void moments_of(const Oracle& o, const double* fc, double& rho, double u[3]) {
+  rho = 0.0;
+  double m[3] = {0.0, 0.0, 0.0};
+  for (int iq = 0; iq < o.L.Q; ++iq) {
+    rho += fc[iq];
+    for (int d = 0; d < 3; ++d) m[d] += o.L.e[iq][d] * fc[iq];
+  }
+  const double div = (o.eq == EQ_STANDARD) ? rho : o.rho0;
+  for (int d = 0; d < 3; ++d) u[d] = (m[d] + 0.5 * o.F[d]) / div;
+}
+
+// InitPDF: f(x, 0) = feq(rho0(x), u0(x)).
+void init_pdf(Oracle& o, const double* rho, const double* u /* SoA u[c*N+i] */) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < o.N; ++i) {
+    const double r = rho ? rho[i] : 1.0;
+    double uu[3] = {0.0, 0.0, 0.0};
+    if (u)
+      for (int d = 0; d < 3; ++d) uu[d] = u[(int64_t)d * o.N + i];
+    for (int iq = 0; iq < o.L.Q; ++iq) o.f[i * o.L.Q + iq] = feq_value(o, iq, r, uu);
+  }
+  o.steps_done = 0;
+}
+
+// Sweep 1 — Collision (Eq. 6; listing P:357-382):  f -> fb.
+//   fb = f - omega (f - feq)                                       [Eq. 6]
+//      + (1 - omega/2) t [3 (e - u) + 9 (e.u) e] . F              [D:R7, only when F != 0]
+void collision(Oracle& o) {
+  const int Q = o.L.Q;
+  const bool forced = (o.F[0] != 0.0 || o.F[1] != 0.0 || o.F[2] != 0.0);
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < o.N; ++i) {
+    const double* fc = &o.f[i * Q];
+    double rho, u[3];
+    moments_of(o, fc, rho, u);
+    o.rho_w[i] = (o.eq == EQ_STANDARD) ? rho : o.rho0;
+    for (int iq = 0; iq < Q; ++iq) {
+      const double feq = feq_value(o, iq, rho, u);
+      double out = fc[iq] - o.omega * (fc[iq] - feq);
+      if (forced) {
+        double edu = 0.0;
+        for (int d = 0; d < 3; ++d) edu += o.L.e[iq][d] * u[d];
+        double s = 0.0;
+        for (int d = 0; d < 3; ++d) s += (3.0 * (o.L.e[iq][d] - u[d]) + 9.0 * edu * o.L.e[iq][d]) * o.F[d];
+        out += (1.0 - 0.5 * o.omega) * o.L.t[iq] * s;
+      }
+      o.fb[i * Q + iq] = out;
+    }
+  }
+}
+
+// Sweep 2 — BoundaryCondition, pre-propagation.  On a single domain there
+// is no halo to exchange (P:395-397 is the MPI part); the wall links are resolved in
+// the propagation sweep below from fb of the same cell, which is the equivalent
+// pre-propagation form of Eq. 10 for a wall half-way between nodes (D:R3).
+void boundary_condition(Oracle&) {}
+
+// Sweep 3 — Propagation (Eq. 7):  f_alpha(x, t) = fb_alpha(x - e_alpha, t - 1).
+// If x - e_alpha leaves the box through a non-periodic face the link is a wall link:
+//   f_alpha(x) = fb_opp(alpha)(x)                                  [Eq. 10; opp = Q-1-alpha, P:49]
+//              + 6 t_alpha rho_w (e_alpha . u_w)                   [D:R6, Ladd; u_w = 0 on resting walls]
+// D:R6 tie-break: when the upstream node lies beyond several non-periodic faces, a MOVING
+// face takes precedence over BOUNCE faces; among several MOVING faces the highest face
+// index (z+ > z- > y+ > y- > x+ > x-) is used.
+void propagation(Oracle& o) {
+  const int Q = o.L.Q;
+  const int n[3] = {o.nx, o.ny, o.nz};
+#pragma omp parallel for schedule(static)
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x) {
+        const int c[3] = {x, y, z};
+        const int64_t i = o.cell(x, y, z);
+        for (int iq = 0; iq < Q; ++iq) {
+          int s[3];
+          bool outside = false;
+          int moving_face = -1;
+          for (int d = 0; d < 3; ++d) {
+            s[d] = c[d] - o.L.e[iq][d];
+            if (s[d] < 0 || s[d] >= n[d]) {
+              const int face = 2 * d + (s[d] < 0 ? 0 : 1);
+              if (o.face_kind[face] == FACE_PERIODIC) {
+                s[d] = ((s[d] % n[d]) + n[d]) % n[d];
+              } else {
+                outside = true;
+                if (o.face_kind[face] == FACE_MOVING && face > moving_face) moving_face = face;
+              }
+            }
+          }
+          if (!outside) {
+            o.f[i * Q + iq] = o.fb[o.cell(s[0], s[1], s[2]) * Q + iq];
+          } else {
+            double v = o.fb[i * Q + (Q - 1 - iq)];
+            if (moving_face >= 0) {
+              double eduw = 0.0;
+              for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * o.face_u[moving_face][d];
+              v += 6.0 * o.L.t[iq] * o.rho_w[i] * eduw;
+            }
+            o.f[i * Q + iq] = v;
+          }
+        }
+      }
+}
+
+// Sweep 4 — PostProcessing (Eq. 8-9) and Monitor, on
+// demand.  diagnostics[8] = { sum rho, sum rho u_x, sum rho u_y, sum rho u_z,
+// 1/2 sum rho |u|^2, max |u|, min rho, number of cells with a non-finite rho or u }.
+// Under Eq. 5 "rho u" and "rho |u|^2" use rho0 (D:R5).  D:R13: 3-component magnitude,
+// all cells (the listing's 2-D magnitude and idn=1 start are typos of the extraction).
+void post_processing(const Oracle& o, double* rho_out, double* u_out, double* diag) {
+  long double s_rho = 0, s_m[3] = {0, 0, 0}, s_e = 0;
+  double umax = 0.0, rmin = INFINITY;
+  int64_t bad = 0;
+  for (int64_t i = 0; i < o.N; ++i) {
+    double rho, u[3];
+    moments_of(o, &o.f[i * o.L.Q], rho, u);
+    if (rho_out) rho_out[i] = rho;
+    if (u_out)
+      for (int d = 0; d < 3; ++d) u_out[(int64_t)d * o.N + i] = u[d];
+    if (!diag) continue;
+    const double usq = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    if (!std::isfinite(rho) || !std::isfinite(usq)) {
+      ++bad;
+      continue;
+    }
+    const double rw = (o.eq == EQ_STANDARD) ? rho : o.rho0;
+    s_rho += rho;
+    for (int d = 0; d < 3; ++d) s_m[d] += (long double)rw * u[d];
+    s_e += 0.5L * rw * usq;
+    umax = std::fmax(umax, std::sqrt(usq));
+    rmin = std::fmin(rmin, rho);
+  }
+  if (diag) {
+    diag[0] = (double)s_rho;
+    diag[1] = (double)s_m[0];
+    diag[2] = (double)s_m[1];
+    diag[3] = (double)s_m[2];
+    diag[4] = (double)s_e;
+    diag[5] = umax;
+    diag[6] = rmin;
+    diag[7] = (double)bad;
+  }
+}
+
+}  // namespace
+
+// ---- tiny C ABI so that tests can drive the oracle through ctypes ------------------
+// All pointers are HOST pointers.  Field layouts at this interface are the canonical
+// ones of include/lbm.h (rho[i], u[c*N+i], f[alpha*N+i], i = x + nx*(y + ny*z)); the
+// AoS <-> SoA transposition happens here and nowhere else.
+extern "C" {
+
+void* orc_create(int nx, int ny, int nz, int Q, int eq, double tau, const int* face_kind,
+                 const double* face_u /*6x3 or NULL*/, const double* force /*3 or NULL*/) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(tau > 0.5)) return nullptr;
+  Oracle* o = new Oracle();
+  if (!make_lattice(Q, o->L)) {
+    delete o;
+    return nullptr;
+  }
+  o->nx = nx;
+  o->ny = ny;
+  o->nz = nz;
+  o->N = (int64_t)nx * ny * nz;
+  o->eq = eq;
+  o->omega = 1.0 / tau;  // D:R1
+  o->rho0 = 1.0;
+  for (int k = 0; k < 6; ++k) {
+    o->face_kind[k] = face_kind ? face_kind[k] : FACE_PERIODIC;
+    for (int d = 0; d < 3; ++d) o->face_u[k][d] = face_u ? face_u[3 * k + d] : 0.0;
+  }
+  for (int d = 0; d < 3; ++d) o->F[d] = force ? force[d] : 0.0;
+  o->f.assign((size_t)o->N * Q, 0.0);
+  o->fb.assign((size_t)o->N * Q, 0.0);
+  o->rho_w.assign((size_t)o->N, 1.0);
+  return o;
+}
+
+void orc_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+// Lattice tables in the oracle's order: e_out[3*Q] (e[iq*3+d], the paper's e(iq*dim+ind),
+// P:373) and t_out[Q].
+int orc_lattice(int Q, int* e_out, double* t_out) {
+  Lattice L;
+  if (!make_lattice(Q, L)) return -1;
+  for (int q = 0; q < Q; ++q) {
+    for (int d = 0; d < 3; ++d) e_out[3 * q + d] = L.e[q][d];
+    t_out[q] = L.t[q];
+  }
+  return 0;
+}
+
+// Single-cell equilibrium for table-level tests: feq_out[Q].
+int orc_feq(int Q, int eq, double rho, const double* u, double* feq_out) {
+  Oracle o;
+  if (!make_lattice(Q, o.L)) return -1;
+  o.eq = eq;
+  o.rho0 = 1.0;
+  for (int q = 0; q < Q; ++q) feq_out[q] = feq_value(o, q, rho, u);
+  return 0;
+}
+
+void orc_init_equilibrium(void* h, const double* rho, const double* u) { init_pdf(*static_cast<Oracle*>(h), rho, u); }
+
+void orc_collision(void* h) { collision(*static_cast<Oracle*>(h)); }
+void orc_boundary_condition(void* h) { boundary_condition(*static_cast<Oracle*>(h)); }
+void orc_propagation(void* h) { propagation(*static_cast<Oracle*>(h)); }
+
+// The time loop of P:112-114.
+void orc_step(void* h, int nsteps) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int s = 0; s < nsteps; ++s) {
+    collision(o);
+    boundary_condition(o);
+    propagation(o);
+    ++o.steps_done;
+  }
+}
+
+void orc_moments(void* h, double* rho, double* u, double* diag) { post_processing(*static_cast<Oracle*>(h), rho, u, diag); }
+
+static void export_soa(const Oracle& o, const std::vector<double>& a, double* out) {
+  for (int iq = 0; iq < o.L.Q; ++iq)
+    for (int64_t i = 0; i < o.N; ++i) out[(int64_t)iq * o.N + i] = a[i * o.L.Q + iq];
+}
+
+void orc_get_f(void* h, double* out) { export_soa(*static_cast<Oracle*>(h), static_cast<Oracle*>(h)->f, out); }
+void orc_get_fb(void* h, double* out) { export_soa(*static_cast<Oracle*>(h), static_cast<Oracle*>(h)->fb, out); }
+
+void orc_set_f(void* h, const double* in) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int iq = 0; iq < o.L.Q; ++iq)
+    for (int64_t i = 0; i < o.N; ++i) o.f[i * o.L.Q + iq] = in[(int64_t)iq * o.N + i];
+}
+
+// Populations of selected cells only: out[k*Q + iq] for cell index cells[k].
+void orc_get_f_cells(void* h, const int64_t* cells, int64_t ncells, double* out) {
+  const Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t k = 0; k < ncells; ++k)
+    for (int iq = 0; iq < o.L.Q; ++iq) out[k * o.L.Q + iq] = o.f[cells[k] * o.L.Q + iq];
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

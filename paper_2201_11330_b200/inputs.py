@@ -1,0 +1,158 @@
+"""Seeded synthetic inputs for the BASELINE.json configs (numpy only).
+
+This module holds NO lattice-Boltzmann arithmetic: it only produces the macroscopic
+initial fields (rho, u) and the boundary description that are handed, unchanged, to both
+the CUDA library and the CPU oracle.  It imports neither of them.
+
+Recipe:
+  * Taylor-Green vortex on a 2*pi box with x_i = 2*pi*i/n:
+        u = u0 * ( sin x cos y cos z, -cos x sin y cos z, 0 )
+  * density noise rho = 1 + a*(2r - 1), r in [0,1) from a counter-based hash of
+    (seed, global cell index) so that any sub-box can be generated point-wise.
+Layouts: rho[i], u[c*N + i], i = x + nx*(y + ny*z).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SEED_BASE = 0x22011330
+
+FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING = 0, 1, 2
+EQ_STANDARD, EQ_INCOMP = 0, 1
+
+_M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
+
+
+def hash_uniform(seed: int, index: np.ndarray) -> np.ndarray:
+    """Counter-based uniform r in [0,1): splitmix64 finaliser of (seed, index), top 53 bits."""
+    with np.errstate(over="ignore"):
+        z = index.astype(np.uint64) + np.uint64(seed & 0xFFFFFFFFFFFFFFFF) * np.uint64(0x9E3779B97F4A7C15)
+        z = (z + np.uint64(0x9E3779B97F4A7C15)) & _M64
+        z = ((z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)) & _M64
+        z = ((z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)) & _M64
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+def _axes(n, lo, hi, wrap):
+    """Global integer coordinates lo..hi-1 of one axis, wrapped into [0, n) if asked."""
+    g = np.arange(lo, hi, dtype=np.int64)
+    return np.mod(g, n) if wrap else g
+
+
+def taylor_green(nx, ny, nz, u0, noise=0.0, seed=0, box=None):
+    """rho[N], u[3,N] of the 3-D Taylor-Green vortex (+ seeded density noise).
+
+    `box` = ((x0,x1),(y0,y1),(z0,z1)) evaluates the SAME global field on a sub-box whose
+    coordinates are wrapped periodically into the global grid (for sampled parity checks).
+    """
+    if box is None:
+        box = ((0, nx), (0, ny), (0, nz))
+    gx = _axes(nx, *box[0], True)
+    gy = _axes(ny, *box[1], True)
+    gz = _axes(nz, *box[2], True)
+    X = 2.0 * np.pi * gx / nx
+    Y = 2.0 * np.pi * gy / ny
+    Z = 2.0 * np.pi * gz / nz
+    sx, cx = np.sin(X)[None, None, :], np.cos(X)[None, None, :]
+    sy, cy = np.sin(Y)[None, :, None], np.cos(Y)[None, :, None]
+    cz = np.cos(Z)[:, None, None]
+    n = gx.size * gy.size * gz.size
+    u = np.zeros((3, n))
+    u[0] = (u0 * sx * cy * cz).reshape(-1)
+    u[1] = (-u0 * cx * sy * cz).reshape(-1)
+    rho = density_noise(nx, ny, nz, noise, seed, box)
+    return rho, u
+
+
+def taylor_green_2d(nx, ny, nz, u0):
+    """z-invariant 2-D Taylor-Green vortex with its exact pressure field.
+
+    u = u0 (sin x cos y, -cos x sin y, 0),  rho = 1 + 3 (u0^2/4)(cos 2x + cos 2y)
+    (p = rho/3): an exact Navier-Stokes solution decaying as exp(-2 nu k^2 t) per velocity
+    component, |k|^2 = 2 (2 pi/n)^2 (SURVEY.md section 8c pins).
+    """
+    X = 2.0 * np.pi * np.arange(nx) / nx
+    Y = 2.0 * np.pi * np.arange(ny) / ny
+    sx, cx = np.sin(X)[None, None, :], np.cos(X)[None, None, :]
+    sy, cy = np.sin(Y)[None, :, None], np.cos(Y)[None, :, None]
+    one = np.ones((nz, 1, 1))
+    n = nx * ny * nz
+    u = np.zeros((3, n))
+    u[0] = (u0 * sx * cy * one).reshape(-1)
+    u[1] = (-u0 * cx * sy * one).reshape(-1)
+    rho = (1.0 + 3.0 * (u0 * u0 / 4.0) * (np.cos(2 * X)[None, None, :] + np.cos(2 * Y)[None, :, None]) * one).reshape(-1)
+    return rho, u
+
+
+def density_noise(nx, ny, nz, noise, seed, box=None):
+    """rho = 1 + noise*(2r-1) on the whole grid or on a (periodically wrapped) sub-box."""
+    if box is None:
+        box = ((0, nx), (0, ny), (0, nz))
+    gx = _axes(nx, *box[0], True)
+    gy = _axes(ny, *box[1], True)
+    gz = _axes(nz, *box[2], True)
+    n = gx.size * gy.size * gz.size
+    if noise == 0.0:
+        return np.ones(n)
+    gi = (gx[None, None, :] + nx * (gy[None, :, None] + ny * gz[:, None, None])).reshape(-1)
+    return 1.0 + noise * (2.0 * hash_uniform(seed, gi) - 1.0)
+
+
+@dataclass
+class Workload:
+    """One BASELINE.json config: geometry, physics parameters and how to make its fields."""
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    Q: int
+    tau: float
+    steps: int
+    face_kind: tuple = (0, 0, 0, 0, 0, 0)
+    face_u: tuple = field(default_factory=lambda: tuple((0.0, 0.0, 0.0) for _ in range(6)))
+    force: tuple = (0.0, 0.0, 0.0)
+    u0: float = 0.0
+    noise: float = 0.0
+    seed: int = 0
+    kind: str = "tgv"  # "tgv" | "rest"
+
+    @property
+    def N(self):
+        return self.nx * self.ny * self.nz
+
+    def fields(self, box=None):
+        """(rho[n], u[3,n]) on the full grid or on a periodically wrapped sub-box."""
+        if self.kind == "tgv":
+            return taylor_green(self.nx, self.ny, self.nz, self.u0, self.noise, self.seed, box)
+        rho = density_noise(self.nx, self.ny, self.nz, self.noise, self.seed, box)
+        return rho, np.zeros((3, rho.size))
+
+    def scaled(self, n, steps=None, name=None):
+        """Same parameters on an n^3 grid (reduced analogue for oracle-affordable parity)."""
+        return Workload(name or f"{self.name}@{n}", n, n, n, self.Q, self.tau, steps or self.steps,
+                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind)
+
+
+_CAVITY_FACES = (FACE_BOUNCE,) * 5 + (FACE_MOVING,)
+_LID_U = tuple((0.0, 0.0, 0.0) for _ in range(5)) + ((0.1, 0.0, 0.0),)
+_CHANNEL_FACES = (FACE_PERIODIC,) * 4 + (FACE_BOUNCE, FACE_BOUNCE)
+
+
+def config(i: int) -> Workload:
+    """BASELINE.json configs[i], i = 0..4 (file order)."""
+    if i == 0:
+        return Workload("cfg0_q19_tgv32", 32, 32, 32, 19, 0.8, 100, u0=0.05, noise=1e-4, seed=SEED_BASE + 1)
+    if i == 1:
+        return Workload("cfg1_q19_tgv128", 128, 128, 128, 19, 0.6, 1000, u0=0.05, noise=1e-4, seed=SEED_BASE + 2)
+    if i == 2:
+        return Workload("cfg2_q19_cavity256", 256, 256, 256, 19, 0.55, 2000, face_kind=_CAVITY_FACES,
+                        face_u=_LID_U, kind="rest")
+    if i == 3:
+        return Workload("cfg3_q19_tgv512", 512, 512, 512, 19, 0.52, 200, u0=0.04, noise=1e-4, seed=SEED_BASE + 4)
+    if i == 4:
+        return Workload("cfg4_q27_channel512", 512, 512, 512, 27, 0.9, 20000, face_kind=_CHANNEL_FACES,
+                        force=(1e-7, 0.0, 0.0), noise=1e-5, seed=SEED_BASE + 5, kind="rest")
+    raise IndexError(i)
