@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS of the fused D3Q19 fp64 stream-collide step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--config i] [--scheme ab|aa] [--store f64|f32] [--block bx,by]
+
+A "step" is one LBM time step = one launch of the fused kernel over the whole grid.  The N=1
+workload is BASELINE.json configs[3] (the headline roofline run: D3Q19 BGK fp64, 512^3 periodic
+Taylor-Green vortex, tau 0.52); --config picks another one.  Prints ONE JSON line on stdout.
+  value     MLUPS with the populations resident in HBM (CUDA events on the launch stream)
+  e2e       MLUPS of the whole job through the host-buffer C-ABI calls: pinned-host rho,u -> device,
+            equilibrium init, K steps, moments + diagnostics, rho,u -> pinned host
+  roofline  algorithmic bytes (2*Q*8 B per cell update) / measured kernel time vs measured HBM peak
+  cpu_baseline  the oracle, as it stands, on this box's host cores, on a bounded sample
+With --gpus N > 1 (torchrun) every rank runs an independent replica (the path does not shard in this
+build); value = total cell updates of all ranks / max-over-ranks device time.
+--impl reference times the CPU oracle (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "mlups_d3q19_fp64_fused_stream_collide"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax.append(float(parts[1]))
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ helpers
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    except (OSError, KeyError, ValueError):
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
+
+
+def ncu_traffic(workload_name: str, scheme: str):
+    """DRAM bytes per launch of the stream-collide kernel from the committed ncu --set full capture
+    (profiles/traffic.csv: workload,scheme,kernel,dram_bytes_per_launch,source), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(p) as fh:
+            for line in fh:
+                parts = [x.strip() for x in line.split(",")]
+                if len(parts) >= 4 and parts[0] == workload_name and parts[1] == scheme:
+                    return float(parts[3])
+    except (OSError, ValueError):
+        pass
+    return None
+
+
+def pick_sample_grid(w, target_cells):
+    n = w.nx
+    while n ** 3 > target_cells and n > 32:
+        n //= 2
+    return n
+
+
+def oracle_mlups(w, n, steps, warmup=1):
+    """Time the oracle as it stands on an n^3 sample of workload w (same tau / walls / force / fields recipe)."""
+    from oracle import Oracle, num_threads
+    ws = w.scaled(n)
+    rho, u = ws.fields()
+    o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force)
+    o.init_equilibrium(rho, u)
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    o.close()
+    return ws.N * steps / dt / 1e6, dt, num_threads()
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def run_reference(args, w):
+    from paper_2201_11330_b200 import replicas
+    rank, _, world = replicas.env_world()
+    if rank != 0:
+        return 0
+    n = pick_sample_grid(w, 128 ** 3)
+    t_all = time.perf_counter()
+    value, dt, cores = oracle_mlups(w, n, args.steps, max(args.warmup, 1))
+    sample = f"{n}^3 sub-grid of {w.name} (same tau, fields recipe, walls, force), {args.steps} oracle steps, {dt:.1f} s"
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "tau": w.tau,
+                   "reference": "CPU oracle (oracle/lbm_oracle.cpp), host cores only"},
+        "cpu_baseline": {"value": value, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "wall_s": time.perf_counter() - t_all,
+    }
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ GPU arm
+def run_gpu(args, w):
+    import numpy as np
+    import torch
+
+    from paper_2201_11330_b200 import lbm, replicas
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CUDA library is the only implementation")
+    lbm.load()
+    rank, local_rank, world = replicas.init()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    scheme = {"ab": lbm.LBM_SCHEME_AB, "aa": lbm.LBM_SCHEME_AA}[args.scheme]
+    store = {"f64": lbm.LBM_STORE_F64, "f32": lbm.LBM_STORE_F32}[args.store]
+    stream = torch.cuda.Stream(device=dev)
+    K, W = args.steps, max(args.warmup, 3)
+
+    # synthetic inputs in pinned host memory (DESIGN.md input recipe)
+    t0 = time.perf_counter()
+    rho, u = w.fields()
+    rho_h = torch.from_numpy(rho).pin_memory()
+    u_h = torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).pin_memory()
+    rho_out = torch.empty(w.N, dtype=torch.float64).pin_memory()
+    u_out = torch.empty(3 * w.N, dtype=torch.float64).pin_memory()
+    del rho, u
+    log(f"[rank {rank}] inputs {w.name} ready in {time.perf_counter() - t0:.1f} s")
+
+    s = lbm.Solver.from_workload(w, scheme=scheme, store=store, stream=stream)
+    if args.block:
+        s.set_block(*[int(v) for v in args.block.split(",")])
+    with torch.cuda.stream(stream):
+        # ---- device-resident measurement -------------------------------------------------------
+        s.init_equilibrium_host(rho_h, u_h)
+        d_init = s.diagnostics()
+        s.step(W)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local_rank)
+        if rank == 0:
+            sampler.start()
+        replicas.barrier()
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = s.launches
+        ev0.record(stream)
+        s.step(K)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        replicas.barrier()
+        launches = s.launches - l0
+        secs = ev0.elapsed_time(ev1) / 1e3
+        clocks = sampler.stop() if rank == 0 else None
+        d_end = s.diagnostics()
+        units, secs_max, ups = replicas.aggregate_throughput(w.N * K, secs, dev)
+
+        # ---- end to end through the host-buffer C-ABI calls ----------------------------------------
+        torch.cuda.synchronize()
+        replicas.barrier()
+        t0 = time.perf_counter()
+        s.init_equilibrium_host(rho_h, u_h)
+        s.step(K)
+        d_e2e = lbm.lbm_moments_host(s.h, rho_out, u_out, True)  # synchronises
+        e2e_secs = time.perf_counter() - t0
+        replicas.barrier()
+        _, e2e_max, e2e_ups = replicas.aggregate_throughput(w.N * K, e2e_secs, dev)
+    s.close()
+
+    if rank != 0:
+        replicas.finalize()
+        return 0
+
+    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8)  # S:§8d algorithmic bytes per lattice update
+    ms_per_launch = secs / launches * 1e3
+    achieved = bytes_per_cell * w.N / (secs / launches) / 1e9
+    peak, peak_src = measured_peak()
+    traffic = ncu_traffic(w.name, args.scheme + ("" if args.store == "f64" else "_f32"))
+    out = {
+        "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "collision": "BGK", "tau": w.tau,
+                   "scheme": args.scheme, "storage": args.store, "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
+                   "l2": f"inputs larger than L2: {bytes_per_cell * w.N / 1e9:.2f} GB touched per step vs 126 MB L2"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_ups / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 32 * w.N / K, "d2h_bytes_per_step": (32 * w.N + 64) / K,
+                "what": "lbm_init_equilibrium_host(pinned rho,u) + lbm_step(K) + lbm_moments_host(pinned rho,u,diagnostics), host wall clock",
+                "seconds": e2e_max},
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                     "kernel": "stream_collide_" + args.scheme, "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch,
+                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+        "checks": {"mass_drift_rel": abs(d_end[0] - d_init[0]) / d_init[0], "nonfinite_cells": d_end[7],
+                   "kinetic_energy_ratio": d_end[4] / d_init[4] if d_init[4] else None, "e2e_mass": d_e2e[0]},
+    }
+    # ---- the oracle on this box's host cores, on a bounded sample (reported baseline, not the target) ----
+    if world == 1 and not args.no_cpu_baseline:
+        n = pick_sample_grid(w, 256 ** 3)
+        t0 = time.perf_counter()
+        v, dt, cores = oracle_mlups(w, n, 8, 1)
+        out["cpu_baseline"] = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle",
+                               "sample": f"{n}^3 sub-grid of {w.name} (same tau, fields recipe, walls, force), 8 oracle steps, {dt:.1f} s"}
+    else:
+        out["cpu_baseline"] = None
+    print(json.dumps(out), flush=True)
+    replicas.finalize()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = 512^3 headline)")
+    ap.add_argument("--scheme", default="ab", choices=["ab", "aa"])
+    ap.add_argument("--store", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--block", default="", help="bx,by block shape override")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2201_11330_b200 import inputs
+    w = inputs.config(args.config)
+    if args.impl == "reference":
+        return run_reference(args, w)
+    return run_gpu(args, w)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,458 @@
+// lbm_abi.cu — the C ABI declared in include/lbm.h: handle, argument checks, kernel dispatch.
+// No torch types, no exceptions across the boundary, no CPU path.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/lbm.h"
+#include "lbm_kernels.cuh"
+
+using namespace lbm;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return LBM_ECUDA;
+}
+#define CUDA_TRY(expr)                                 \
+  do {                                                 \
+    cudaError_t e__ = (expr);                          \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #expr); \
+  } while (0)
+
+constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 SMs
+
+}  // namespace
+
+struct lbm_handle_s {
+  int nx, ny, nz, Q, eq, scheme, f32;
+  long long N;
+  double tau;
+  Params p;
+  bool walls, forced;
+  cudaStream_t stream;
+  void* buf[2];       // A/B: both used, buf[cur] holds S^-1 f;  AA: buf[0] only
+  int cur;
+  int phase;          // AA: 0 = natural layout, 1 = after an even step
+  long long time, launches;
+  double* partials;   // kReduceBlocks * 8
+  double* diag_dev;   // 8
+  double* diag_pinned;  // 8, host
+  void* scratch;
+  size_t scratch_bytes;
+  int bx, by;
+  size_t elem() const { return f32 ? 4 : 8; }
+  size_t buf_bytes() const { return (size_t)N * Q * elem(); }
+};
+
+namespace {
+
+// ---- dispatch over the compile-time variants ------------------------------------------
+// VARIANT(q, eq, walls, force) expands `body` with constexpr Q_, EQ_, WALLS_, FORCE_.
+#define LBM_DISPATCH_QEWF(h, BODY)                                                              \
+  do {                                                                                          \
+    const int key__ = ((h)->Q == 27 ? 8 : 0) | ((h)->eq ? 4 : 0) | ((h)->walls ? 2 : 0) | ((h)->forced ? 1 : 0); \
+    switch (key__) {                                                                            \
+      LBM_CASE(0, 19, 0, false, false, BODY) LBM_CASE(1, 19, 0, false, true, BODY)               \
+      LBM_CASE(2, 19, 0, true, false, BODY) LBM_CASE(3, 19, 0, true, true, BODY)                 \
+      LBM_CASE(4, 19, 1, false, false, BODY) LBM_CASE(5, 19, 1, false, true, BODY)               \
+      LBM_CASE(6, 19, 1, true, false, BODY) LBM_CASE(7, 19, 1, true, true, BODY)                 \
+      LBM_CASE(8, 27, 0, false, false, BODY) LBM_CASE(9, 27, 0, false, true, BODY)               \
+      LBM_CASE(10, 27, 0, true, false, BODY) LBM_CASE(11, 27, 0, true, true, BODY)               \
+      LBM_CASE(12, 27, 1, false, false, BODY) LBM_CASE(13, 27, 1, false, true, BODY)             \
+      LBM_CASE(14, 27, 1, true, false, BODY) LBM_CASE(15, 27, 1, true, true, BODY)               \
+    }                                                                                           \
+  } while (0)
+#define LBM_CASE(k, q, e, w, f, BODY)  \
+  case k: {                            \
+    constexpr int Q_ = q, EQ_ = e;     \
+    constexpr bool WALLS_ = w, FORCE_ = f; \
+    (void)Q_; (void)EQ_; (void)WALLS_; (void)FORCE_; \
+    BODY;                              \
+  } break;
+
+int flat_grid(long long N) {
+  long long b = (N + 255) / 256;
+  return (int)(b < kReduceBlocks ? b : kReduceBlocks);
+}
+
+// canonical-state read mode of the current storage state
+int read_mode(const lbm_handle_s* h) {
+  if (h->scheme == LBM_SCHEME_AB) return MODE_PULL;
+  return h->phase ? MODE_PULL_SWAP : MODE_NATURAL;
+}
+
+template <typename ST>
+int launch_step(lbm_handle_s* h) {
+  dim3 block(h->bx, h->by, 1);
+  dim3 grid((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->nz);
+  if (h->scheme == LBM_SCHEME_AB) {
+    const ST* src = (const ST*)h->buf[h->cur];
+    ST* dst = (ST*)h->buf[h->cur ^ 1];
+    LBM_DISPATCH_QEWF(h, (stream_collide_ab<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(src, dst, h->p)));
+    h->cur ^= 1;
+  } else {
+    ST* b = (ST*)h->buf[0];
+    if (h->phase == 0)
+      LBM_DISPATCH_QEWF(h, (stream_collide_aa_even<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(b, h->p)));
+    else
+      LBM_DISPATCH_QEWF(h, (stream_collide_aa_odd<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(b, h->p)));
+    h->phase ^= 1;
+  }
+  ++h->launches;
+  return LBM_OK;
+}
+
+template <typename ST>
+void launch_export(lbm_handle_s* h, double* out) {
+  const int g = flat_grid(h->N);
+  const ST* b = (const ST*)h->buf[h->cur];
+  switch (read_mode(h)) {
+    case MODE_NATURAL:
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+      break;
+    case MODE_PULL:
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+      break;
+    default:
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+  }
+  ++h->launches;
+}
+
+// canonical fp64 array `in` -> storage buffer `dst_idx` in the layout the scheme wants at an even phase
+template <typename ST>
+void launch_import(lbm_handle_s* h, const double* in, int dst_idx) {
+  const int g = flat_grid(h->N);
+  ST* b = (ST*)h->buf[dst_idx];
+  if (h->scheme == LBM_SCHEME_AB)
+    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(in, b, h->p)));
+  else
+    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(in, b, h->p)));
+  ++h->launches;
+}
+
+template <typename ST>
+void launch_moments(lbm_handle_s* h, double* rho, double* u, double* partials, int g) {
+  const ST* b = (const ST*)h->buf[h->cur];
+  switch (read_mode(h)) {
+    case MODE_NATURAL:
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+      break;
+    case MODE_PULL:
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+      break;
+    default:
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+  }
+  ++h->launches;
+}
+
+int ensure_scratch(lbm_handle_s* h, size_t bytes) {
+  if (h->scratch_bytes >= bytes) return LBM_OK;
+  if (h->scratch) {
+    cudaStreamSynchronize(h->stream);
+    cudaFree(h->scratch);
+    h->scratch = nullptr;
+    h->scratch_bytes = 0;
+  }
+  cudaError_t e = cudaMalloc(&h->scratch, bytes);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(LBM_ENOMEM, "out of device memory for the scratch buffer");
+  }
+  h->scratch_bytes = bytes;
+  return LBM_OK;
+}
+
+// A canonical fp64 Q*N staging area that is free while no step is in flight: the idle A/B buffer
+// when populations are stored as fp64, else the lazily allocated scratch.
+int canonical_staging(lbm_handle_s* h, double** out) {
+  if (h->scheme == LBM_SCHEME_AB && !h->f32) {
+    *out = (double*)h->buf[h->cur ^ 1];
+    return LBM_OK;
+  }
+  int rc = ensure_scratch(h, (size_t)h->N * h->Q * sizeof(double));
+  if (rc) return rc;
+  *out = (double*)h->scratch;
+  return LBM_OK;
+}
+
+int check_launch(const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, what);
+  return LBM_OK;
+}
+
+int do_init(lbm_handle_s* h, const double* rho, const double* u) {
+  double* nat = nullptr;
+  int rc = canonical_staging(h, &nat);
+  if (rc) return rc;
+  const int g = flat_grid(h->N);
+  if (h->eq) {
+    if (h->Q == 19) init_equilibrium_kernel<19, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+    else init_equilibrium_kernel<27, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+  } else {
+    if (h->Q == 19) init_equilibrium_kernel<19, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+    else init_equilibrium_kernel<27, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+  }
+  ++h->launches;
+  if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
+  if (h->f32) launch_import<float>(h, nat, h->cur);
+  else launch_import<double>(h, nat, h->cur);
+  h->phase = 0;
+  h->time = 0;
+  return check_launch("init_equilibrium");
+}
+
+int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
+  const int g = flat_grid(h->N);
+  double* partials = diagnostics ? h->partials : nullptr;
+  if (h->f32) launch_moments<float>(h, rho, u, partials, g);
+  else launch_moments<double>(h, rho, u, partials, g);
+  if (diagnostics) {
+    reduce_final_kernel<<<1, 256, 0, h->stream>>>(h->partials, g, h->diag_dev);
+    ++h->launches;
+  }
+  int rc = check_launch("moments");
+  if (rc) return rc;
+  if (diagnostics) {
+    CUDA_TRY(cudaMemcpyAsync(h->diag_pinned, h->diag_dev, kDiag * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    std::memcpy(diagnostics, h->diag_pinned, kDiag * sizeof(double));
+  }
+  return LBM_OK;
+}
+
+}  // namespace
+
+// =========================================================================================
+extern "C" {
+
+const char* lbm_last_error(void) { return g_err.c_str(); }
+
+int lbm_lattice(int lattice, int32_t* e, double* t) {
+  const int Q = lattice & 0xff;
+  if (!e || !t) return fail(LBM_EINVAL, "lbm_lattice: NULL output");
+  if (Q == 19) {
+    for (int a = 0; a < 19; ++a) {
+      int s = 0;
+      for (int d = 0; d < 3; ++d) {
+        e[3 * a + d] = Lattice<19>::e[a][d];
+        s += e[3 * a + d] * e[3 * a + d];
+      }
+      t[a] = s == 0 ? Lattice<19>::w0 : s == 1 ? Lattice<19>::w1 : Lattice<19>::w2;
+    }
+    return LBM_OK;
+  }
+  if (Q == 27) {
+    for (int a = 0; a < 27; ++a) {
+      int s = 0;
+      for (int d = 0; d < 3; ++d) {
+        e[3 * a + d] = Lattice<27>::e[a][d];
+        s += e[3 * a + d] * e[3 * a + d];
+      }
+      t[a] = s == 0 ? Lattice<27>::w0 : s == 1 ? Lattice<27>::w1 : s == 2 ? Lattice<27>::w2 : Lattice<27>::w3;
+    }
+    return LBM_OK;
+  }
+  return fail(LBM_EINVAL, "lbm_lattice: lattice must be LBM_D3Q19 or LBM_D3Q27");
+}
+
+lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm_bc_t* bc) {
+  const int Q = lattice & 0xff;
+  if (Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
+  if (nx < 1 || ny < 1 || nz < 1) { fail(LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1"); return nullptr; }
+  if (nz > 65535 || ny > 65535) { fail(LBM_EINVAL, "lbm_create: ny or nz exceeds the launch grid limits"); return nullptr; }
+  if (!(tau > 0.5) || !std::isfinite(tau)) { fail(LBM_EINVAL, "lbm_create: tau must be finite and > 0.5"); return nullptr; }
+  int scheme = lattice & (3 << 12);
+  if (scheme == LBM_SCHEME_AUTO) scheme = LBM_SCHEME_AB;
+  if (scheme != LBM_SCHEME_AB && scheme != LBM_SCHEME_AA) { fail(LBM_EINVAL, "lbm_create: unknown storage scheme"); return nullptr; }
+  if (lattice & ~(0xff | LBM_EQ_INCOMP | (3 << 12) | LBM_STORE_F32)) { fail(LBM_EINVAL, "lbm_create: unknown bits in lattice"); return nullptr; }
+
+  lbm_handle_s* h = new (std::nothrow) lbm_handle_s();
+  if (!h) { fail(LBM_ENOMEM, "lbm_create: out of host memory"); return nullptr; }
+  std::memset(h, 0, sizeof(*h));
+  h->nx = nx; h->ny = ny; h->nz = nz; h->Q = Q;
+  h->eq = (lattice & LBM_EQ_INCOMP) ? 1 : 0;
+  h->scheme = scheme;
+  h->f32 = (lattice & LBM_STORE_F32) ? 1 : 0;
+  h->N = (long long)nx * ny * nz;
+  h->tau = tau;
+  Params& p = h->p;
+  p.nx = nx; p.ny = ny; p.nz = nz; p.N = h->N;
+  p.omega = 1.0 / tau;
+  if (bc) {
+    for (int k = 0; k < 6; ++k) {
+      const int kind = bc->face_kind[k];
+      if (kind != LBM_FACE_PERIODIC && kind != LBM_FACE_BOUNCE && kind != LBM_FACE_MOVING) {
+        delete h; fail(LBM_EINVAL, "lbm_create: unknown face kind"); return nullptr;
+      }
+      p.wall[k] = kind != LBM_FACE_PERIODIC;
+      p.moving[k] = kind == LBM_FACE_MOVING;
+      for (int d = 0; d < 3; ++d) {
+        p.face_u[k][d] = p.moving[k] ? bc->face_u[k][d] : 0.0;
+        if (!std::isfinite(p.face_u[k][d])) { delete h; fail(LBM_EINVAL, "lbm_create: non-finite wall velocity"); return nullptr; }
+      }
+      p.any_moving |= p.moving[k];
+    }
+    for (int d = 0; d < 3; ++d) {
+      if (p.wall[2 * d] != p.wall[2 * d + 1]) { delete h; fail(LBM_EINVAL, "lbm_create: periodic must be set on both faces of an axis"); return nullptr; }
+      p.F[d] = bc->force[d];
+      if (!std::isfinite(p.F[d])) { delete h; fail(LBM_EINVAL, "lbm_create: non-finite force"); return nullptr; }
+    }
+    h->stream = (cudaStream_t)bc->stream;
+  }
+  h->walls = p.wall[0] || p.wall[2] || p.wall[4];
+  h->forced = p.F[0] != 0.0 || p.F[1] != 0.0 || p.F[2] != 0.0;
+  // default block: as long along x as the row allows (coalesced, vector-friendly), 256 threads
+  int bx = 32;
+  while (bx < nx && bx < 256) bx *= 2;
+  h->bx = bx; h->by = 256 / bx;
+
+  const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
+  cudaError_t e = cudaSuccess;
+  for (int b = 0; b < nbuf && e == cudaSuccess; ++b) e = cudaMalloc(&h->buf[b], h->buf_bytes());
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->partials, (size_t)kReduceBlocks * kDiag * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->diag_dev, kDiag * sizeof(double));
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&h->diag_pinned, kDiag * sizeof(double));
+  if (e != cudaSuccess) {
+    const bool oom = (e == cudaErrorMemoryAllocation);
+    std::string msg = std::string("lbm_create: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    lbm_destroy(h);
+    fail(oom ? LBM_ENOMEM : LBM_ECUDA, msg);
+    return nullptr;
+  }
+  return h;
+}
+
+void lbm_destroy(lbm_handle h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  for (int b = 0; b < 2; ++b)
+    if (h->buf[b]) cudaFree(h->buf[b]);
+  if (h->partials) cudaFree(h->partials);
+  if (h->diag_dev) cudaFree(h->diag_dev);
+  if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
+  if (h->scratch) cudaFree(h->scratch);
+  cudaGetLastError();
+  delete h;
+}
+
+int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u) {
+  if (!h) return fail(LBM_EINVAL, "lbm_init_equilibrium: NULL handle");
+  return do_init(h, rho, u);
+}
+
+int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host) {
+  if (!h) return fail(LBM_EINVAL, "lbm_init_equilibrium_host: NULL handle");
+  // Stage the 4N doubles in device memory that do_init does not write before it has read them:
+  // the CURRENT storage buffer for fp64 A/B (do_init writes the idle one first), else scratch.
+  double* stage = nullptr;
+  const size_t need = (size_t)h->N * 4 * sizeof(double);
+  if (h->scheme == LBM_SCHEME_AB && !h->f32) {
+    stage = (double*)h->buf[h->cur];
+  } else {
+    // scratch holds the canonical staging (Q*N doubles) followed by the 4N input doubles
+    int rc = ensure_scratch(h, (size_t)h->N * h->Q * sizeof(double) + need);
+    if (rc) return rc;
+    stage = (double*)h->scratch + (size_t)h->N * h->Q;
+  }
+  double* d_rho = nullptr;
+  double* d_u = nullptr;
+  if (rho_host) {
+    d_rho = stage;
+    CUDA_TRY(cudaMemcpyAsync(d_rho, rho_host, (size_t)h->N * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  }
+  if (u_host) {
+    d_u = stage + h->N;
+    CUDA_TRY(cudaMemcpyAsync(d_u, u_host, (size_t)h->N * 3 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  }
+  return do_init(h, d_rho, d_u);
+}
+
+int lbm_step(lbm_handle h, int nsteps) {
+  if (!h) return fail(LBM_EINVAL, "lbm_step: NULL handle");
+  if (nsteps < 0) return fail(LBM_EINVAL, "lbm_step: nsteps must be >= 0");
+  for (int s = 0; s < nsteps; ++s) {
+    if (h->f32) launch_step<float>(h);
+    else launch_step<double>(h);
+    ++h->time;
+  }
+  return nsteps ? check_launch("lbm_step") : LBM_OK;
+}
+
+int lbm_moments(lbm_handle h, double* rho, double* u, double* diagnostics) {
+  if (!h) return fail(LBM_EINVAL, "lbm_moments: NULL handle");
+  if (!rho && !u && !diagnostics) return LBM_OK;
+  return do_moments(h, rho, u, diagnostics);
+}
+
+int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* diagnostics) {
+  if (!h) return fail(LBM_EINVAL, "lbm_moments_host: NULL handle");
+  if (!rho_host && !u_host && !diagnostics) return LBM_OK;
+  double* stage = nullptr;
+  if (rho_host || u_host) {
+    if (h->scheme == LBM_SCHEME_AB && !h->f32) {
+      stage = (double*)h->buf[h->cur ^ 1];
+    } else {
+      int rc = ensure_scratch(h, (size_t)h->N * 4 * sizeof(double));
+      if (rc) return rc;
+      stage = (double*)h->scratch;
+    }
+  }
+  double* d_rho = rho_host ? stage : nullptr;
+  double* d_u = u_host ? stage + h->N : nullptr;
+  int rc = do_moments(h, d_rho, d_u, diagnostics);
+  if (rc) return rc;
+  if (rho_host) CUDA_TRY(cudaMemcpyAsync(rho_host, d_rho, (size_t)h->N * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (u_host) CUDA_TRY(cudaMemcpyAsync(u_host, d_u, (size_t)h->N * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBM_OK;
+}
+
+int lbm_get_populations(lbm_handle h, double* f) {
+  if (!h || !f) return fail(LBM_EINVAL, "lbm_get_populations: NULL argument");
+  if (h->f32) launch_export<float>(h, f);
+  else launch_export<double>(h, f);
+  return check_launch("lbm_get_populations");
+}
+
+int lbm_set_populations(lbm_handle h, const double* f) {
+  if (!h || !f) return fail(LBM_EINVAL, "lbm_set_populations: NULL argument");
+  if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
+  if (h->f32) launch_import<float>(h, f, h->cur);
+  else launch_import<double>(h, f, h->cur);
+  h->phase = 0;
+  return check_launch("lbm_set_populations");
+}
+
+int64_t lbm_time(lbm_handle h) { return h ? h->time : -1; }
+int64_t lbm_launch_count(lbm_handle h) { return h ? h->launches : -1; }
+
+int lbm_set_block(lbm_handle h, int bx, int by) {
+  if (!h) return fail(LBM_EINVAL, "lbm_set_block: NULL handle");
+  if (bx == 0 && by == 0) {
+    bx = 32;
+    while (bx < h->nx && bx < 256) bx *= 2;
+    by = 256 / bx;
+  }
+  if (bx < 1 || by < 1 || bx * by > 256 || (bx * by) % 32 != 0)
+    return fail(LBM_EINVAL, "lbm_set_block: bx*by must be a multiple of 32 and <= 256");
+  if ((h->ny + by - 1) / by > 65535) return fail(LBM_EINVAL, "lbm_set_block: grid.y would exceed 65535");
+  h->bx = bx;
+  h->by = by;
+  return LBM_OK;
+}
+
+}  // extern "C"

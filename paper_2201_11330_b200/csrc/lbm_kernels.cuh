@@ -1,0 +1,542 @@
+// lbm_kernels.cuh — hand-written sm_100a kernels of the fused stream-collide hot path.
+//
+// P:n = PAPER.md line n; D:Rk = DESIGN.md §2 reading k; S:§8 = SURVEY.md hot-path table.
+// Everything here is HBM-bound (S:§8d: 2*Q*8 B per lattice update, ~1 flop/B): no tensor
+// cores, no shared-memory staging; one thread owns one cell, the Q populations live in
+// registers, every per-direction stream is unit-stride in x (SoA f[a][z][y][x]).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace lbm {
+
+// ---------------------------------------------------------------------------------------
+// Compile-time lattice tables (D:R4).  Hand-written; the oracle generates its own.
+template <int Q>
+struct Lattice;
+
+template <>
+struct Lattice<19> {
+  static constexpr int e[19][3] = {
+      {-1, -1, 0}, {-1, 0, -1}, {-1, 0, 0}, {-1, 0, 1}, {-1, 1, 0},                         //  0.. 4
+      {0, -1, -1}, {0, -1, 0},  {0, -1, 1}, {0, 0, -1}, {0, 0, 0},                          //  5.. 9
+      {0, 0, 1},   {0, 1, -1},  {0, 1, 0},  {0, 1, 1},                                      // 10..13
+      {1, -1, 0},  {1, 0, -1},  {1, 0, 0},  {1, 0, 1},  {1, 1, 0}};                         // 14..18
+  static constexpr double w0 = 1.0 / 3.0, w1 = 1.0 / 18.0, w2 = 1.0 / 36.0, w3 = 0.0;
+};
+
+template <>
+struct Lattice<27> {
+  static constexpr int e[27][3] = {
+      {-1, -1, -1}, {-1, -1, 0}, {-1, -1, 1}, {-1, 0, -1}, {-1, 0, 0}, {-1, 0, 1}, {-1, 1, -1}, {-1, 1, 0}, {-1, 1, 1},
+      {0, -1, -1},  {0, -1, 0},  {0, -1, 1},  {0, 0, -1},  {0, 0, 0},  {0, 0, 1},  {0, 1, -1},  {0, 1, 0},  {0, 1, 1},
+      {1, -1, -1},  {1, -1, 0},  {1, -1, 1},  {1, 0, -1},  {1, 0, 0},  {1, 0, 1},  {1, 1, -1},  {1, 1, 0},  {1, 1, 1}};
+  static constexpr double w0 = 8.0 / 27.0, w1 = 2.0 / 27.0, w2 = 1.0 / 54.0, w3 = 1.0 / 216.0;
+};
+
+template <int Q, int A>
+struct Dir {
+  static constexpr int ex = Lattice<Q>::e[A][0], ey = Lattice<Q>::e[A][1], ez = Lattice<Q>::e[A][2];
+  static constexpr int s = ex * ex + ey * ey + ez * ez;
+  static constexpr double t = (s == 0) ? Lattice<Q>::w0 : (s == 1) ? Lattice<Q>::w1 : (s == 2) ? Lattice<Q>::w2 : Lattice<Q>::w3;
+  static constexpr int opp = Q - 1 - A;
+};
+
+template <int I>
+struct IC {
+  static constexpr int value = I;
+};
+template <int I, int N, typename F>
+__device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (I < N) {
+    f(IC<I>{});
+    static_for<I + 1, N>(f);
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+struct Params {
+  int nx, ny, nz;
+  long long N;          // cells = plane stride of the SoA layout (64-bit: 512^3*19 > 2^31)
+  double omega;         // 1/tau (D:R1)
+  double F[3];          // body force (D:R7)
+  int wall[6];          // face is non-periodic (BOUNCE or MOVING), order x-,x+,y-,y+,z-,z+
+  int moving[6];        // face is MOVING
+  double face_u[6][3];  // wall velocity of MOVING faces
+  int any_moving;
+};
+
+enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
+
+// Position of a cell relative to the non-periodic faces.
+template <bool WALLS>
+struct CellFlags {
+  bool lo[3], hi[3];  // cell is in the first / last plane of an axis whose face there is a wall
+  __device__ __forceinline__ CellFlags(const Params& p, int x, int y, int z) {
+    if constexpr (WALLS) {
+      lo[0] = (x == 0) && p.wall[0];
+      hi[0] = (x == p.nx - 1) && p.wall[1];
+      lo[1] = (y == 0) && p.wall[2];
+      hi[1] = (y == p.ny - 1) && p.wall[3];
+      lo[2] = (z == 0) && p.wall[4];
+      hi[2] = (z == p.nz - 1) && p.wall[5];
+    } else {
+      lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
+    }
+  }
+  // true if the node x + s*e_A lies outside the box (s = +1: downstream, s = -1: upstream)
+  template <int Q, int A, int S>
+  __device__ __forceinline__ bool leaves() const {
+    if constexpr (!WALLS) return false;
+    constexpr int dx = S * Dir<Q, A>::ex, dy = S * Dir<Q, A>::ey, dz = S * Dir<Q, A>::ez;
+    bool out = false;
+    if constexpr (dx == -1) out = out || lo[0];
+    if constexpr (dx == 1) out = out || hi[0];
+    if constexpr (dy == -1) out = out || lo[1];
+    if constexpr (dy == 1) out = out || hi[1];
+    if constexpr (dz == -1) out = out || lo[2];
+    if constexpr (dz == 1) out = out || hi[2];
+    return out;
+  }
+};
+
+// Neighbour offsets of one cell with periodic wrap by conditional add (no %).
+struct Neigh {
+  long long ox[3], oy[3], oz[3];  // index 0: coordinate-1, 1: same, 2: coordinate+1
+  long long ic;
+  __device__ __forceinline__ Neigh(const Params& p, int x, int y, int z) {
+    const int xm = (x == 0) ? p.nx - 1 : x - 1, xp = (x == p.nx - 1) ? 0 : x + 1;
+    const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
+    const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
+    const long long sy = p.nx, sz = (long long)p.nx * p.ny;
+    ox[0] = xm; ox[1] = x; ox[2] = xp;
+    oy[0] = ym * sy; oy[1] = y * sy; oy[2] = yp * sy;
+    oz[0] = zm * sz; oz[1] = z * sz; oz[2] = zp * sz;
+    ic = ox[1] + oy[1] + oz[1];
+  }
+  // linear index of x + s*e_A (wrapped)
+  template <int Q, int A, int S>
+  __device__ __forceinline__ long long at() const {
+    return ox[1 + S * Dir<Q, A>::ex] + oy[1 + S * Dir<Q, A>::ey] + oz[1 + S * Dir<Q, A>::ez];
+  }
+};
+
+// ---------------------------------------------------------------------------------------
+// Storage element access.  fp64: the value itself.  fp32 storage (S:§8f NEXT-1): f - t_a is
+// kept as float, arithmetic stays fp64.
+template <typename ST, int Q, int A>
+__device__ __forceinline__ double ld_pop(const ST* __restrict__ p, long long i) {
+  if constexpr (sizeof(ST) == 8) return __ldg(p + i);
+  else return (double)__ldg(p + i) + Dir<Q, A>::t;
+}
+template <typename ST, int Q, int A>
+__device__ __forceinline__ void st_pop(ST* __restrict__ p, long long i, double v) {
+  if constexpr (sizeof(ST) == 8) p[i] = v;
+  else p[i] = (float)(v - Dir<Q, A>::t);
+}
+
+// ---------------------------------------------------------------------------------------
+// Moments (Eq. 8-9; D:R5, D:R7): rho = sum f; u = (sum e f + F/2)/rho  [Eq. 5: /rho0 = 1]
+template <int Q, int EQ, bool FORCE>
+__device__ __forceinline__ void moments(const double (&f)[Q], const Params& p, double& rho, double& ux, double& uy, double& uz) {
+  double r = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    using D = Dir<Q, a>;
+    r += f[a];
+    if constexpr (D::ex == 1) mx += f[a];
+    if constexpr (D::ex == -1) mx -= f[a];
+    if constexpr (D::ey == 1) my += f[a];
+    if constexpr (D::ey == -1) my -= f[a];
+    if constexpr (D::ez == 1) mz += f[a];
+    if constexpr (D::ez == -1) mz -= f[a];
+  });
+  if constexpr (FORCE) {
+    mx += 0.5 * p.F[0];
+    my += 0.5 * p.F[1];
+    mz += 0.5 * p.F[2];
+  }
+  rho = r;
+  if constexpr (EQ == EQ_STANDARD) {
+    const double inv = 1.0 / r;
+    ux = mx * inv; uy = my * inv; uz = mz * inv;
+  } else {
+    ux = mx; uy = my; uz = mz;
+  }
+}
+
+template <int Q, int A>
+__device__ __forceinline__ double edot(double vx, double vy, double vz) {
+  using D = Dir<Q, A>;
+  double r = 0.0;
+  if constexpr (D::ex == 1) r += vx;
+  if constexpr (D::ex == -1) r -= vx;
+  if constexpr (D::ey == 1) r += vy;
+  if constexpr (D::ey == -1) r -= vy;
+  if constexpr (D::ez == 1) r += vz;
+  if constexpr (D::ez == -1) r -= vz;
+  return r;
+}
+
+// Equilibrium: Eq. 2  feq = t rho (1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u)
+//              Eq. 5  feq = t (rho + rho0 (3 e.u + 4.5 (e.u)^2 - 1.5 u.u)), rho0 = 1, rho = p/c_s^2
+template <int Q, int EQ>
+__device__ __forceinline__ void equilibrium(double (&feq)[Q], double rho, double ux, double uy, double uz) {
+  const double usq15 = 1.5 * (ux * ux + uy * uy + uz * uz);
+  const double A = (EQ == EQ_STANDARD) ? rho : 1.0;
+  const double base = (EQ == EQ_STANDARD) ? rho * (1.0 - usq15) : rho - usq15;
+  static_for<0, (Q + 1) / 2>([&](auto AA) {
+    constexpr int a = decltype(AA)::value;
+    using D = Dir<Q, a>;
+    if constexpr (a == D::opp) {
+      feq[a] = D::t * base;
+    } else {
+      const double eu = edot<Q, a>(ux, uy, uz);
+      const double s = D::t * fma(4.5 * A * eu, eu, base);
+      const double d = (3.0 * D::t) * (A * eu);
+      feq[a] = s + d;
+      feq[D::opp] = s - d;
+    }
+  });
+}
+
+// BGK relaxation, Eq. 6: f* = f - omega (f - feq), plus Guo's source (D:R7)
+//   S_a = (1 - omega/2) t_a [3 (e_a - u) + 9 (e_a.u) e_a] . F
+// and, on cells touching a MOVING face, the Ladd term folded into the outgoing wall links
+// (D:R6): the value kept for an outgoing link b is f*_b - 6 t_b rho_w (e_b . u_w), which the
+// bounce-back read f_bbar(x, t+1) = stored_b(x) turns into f*_b + 6 t_bbar rho_w (e_bbar . u_w).
+// f is replaced by the post-collision populations.
+template <int Q, int EQ, bool WALLS, bool FORCE>
+__device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const CellFlags<WALLS>& c) {
+  double rho, ux, uy, uz;
+  moments<Q, EQ, FORCE>(f, p, rho, ux, uy, uz);
+  const double om = p.omega, om1 = 1.0 - p.omega;
+  const double usq15 = 1.5 * (ux * ux + uy * uy + uz * uz);
+  const double A = (EQ == EQ_STANDARD) ? rho : 1.0;
+  const double base = (EQ == EQ_STANDARD) ? rho * (1.0 - usq15) : rho - usq15;
+  double k = 0.0, uF3 = 0.0;
+  if constexpr (FORCE) {
+    k = 1.0 - 0.5 * om;
+    uF3 = 3.0 * (ux * p.F[0] + uy * p.F[1] + uz * p.F[2]);
+  }
+  static_for<0, (Q + 1) / 2>([&](auto AA) {
+    constexpr int a = decltype(AA)::value;
+    using D = Dir<Q, a>;
+    if constexpr (a == D::opp) {
+      double g = (om * D::t) * base;
+      if constexpr (FORCE) g -= (k * D::t) * uF3;
+      f[a] = fma(om1, f[a], g);
+    } else {
+      const double eu = edot<Q, a>(ux, uy, uz);
+      double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
+      double d = (3.0 * om * D::t) * (A * eu);
+      if constexpr (FORCE) {
+        const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
+        s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
+        d = fma(3.0 * k * D::t, eF, d);
+      }
+      f[a] = fma(om1, f[a], s + d);
+      f[D::opp] = fma(om1, f[D::opp], s - d);
+    }
+  });
+  if constexpr (WALLS) {
+    if (p.any_moving) {
+      // moving face crossed by a link leaving along +e on axis d: hi face (2d+1); along -e: lo face (2d)
+      const bool touch = (c.lo[0] && p.moving[0]) || (c.hi[0] && p.moving[1]) || (c.lo[1] && p.moving[2]) ||
+                         (c.hi[1] && p.moving[3]) || (c.lo[2] && p.moving[4]) || (c.hi[2] && p.moving[5]);
+      if (touch) {
+        const double rw = (EQ == EQ_STANDARD) ? rho : 1.0;
+        static_for<0, Q>([&](auto BB) {
+          constexpr int b = decltype(BB)::value;
+          using D = Dir<Q, b>;
+          if constexpr (D::s > 0) {
+            // highest-index MOVING face crossed by x + e_b: test z, then y, then x (D:R6 tie-break)
+            int face = -1;
+            if constexpr (D::ex != 0) {
+              constexpr int fx = (D::ex == 1) ? 1 : 0;
+              if ((D::ex == 1 ? c.hi[0] : c.lo[0]) && p.moving[fx]) face = fx;
+            }
+            if constexpr (D::ey != 0) {
+              constexpr int fy = (D::ey == 1) ? 3 : 2;
+              if ((D::ey == 1 ? c.hi[1] : c.lo[1]) && p.moving[fy]) face = fy;
+            }
+            if constexpr (D::ez != 0) {
+              constexpr int fz = (D::ez == 1) ? 5 : 4;
+              if ((D::ez == 1 ? c.hi[2] : c.lo[2]) && p.moving[fz]) face = fz;
+            }
+            if (face >= 0) {
+              const double euw = edot<Q, b>(p.face_u[face][0], p.face_u[face][1], p.face_u[face][2]);
+              f[b] -= (6.0 * D::t) * rw * euw;
+            }
+          }
+        });
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// A/B scheme ("stream on read").  The buffer holds B = S^-1 f, S the slot permutation of one
+// propagation (Eq. 7 with wall links, Eq. 10):  f_a(x) = B_a(x - e_a)  inside,  = B_abar(x)  at a wall
+// link.  One step = pull (gives the canonical pre-collision f of this time level), collide,
+// store aligned at the own cell into the other buffer (which is again S^-1 of the next f).
+template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= p.nx || y >= p.ny) return;
+  const Neigh nb(p, x, y, z);
+  const CellFlags<WALLS> c(p, x, y, z);
+  double f[Q];
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    const bool wall_link = c.template leaves<Q, a, -1>();
+    const long long idx = wall_link ? (long long)Dir<Q, a>::opp * p.N + nb.ic : (long long)a * p.N + nb.template at<Q, a, -1>();
+    f[a] = wall_link ? ld_pop<ST, Q, Dir<Q, a>::opp>(src, idx) : ld_pop<ST, Q, a>(src, idx);
+  });
+  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    st_pop<ST, Q, a>(dst, (long long)a * p.N + nb.ic, f[a]);
+  });
+}
+
+// AA pattern (one buffer, in place).  Even phase: slot (x,a) holds f_a(x); read local, collide,
+// write f*_a(x) into slot (x, abar) — every access aligned.  Odd phase: f_a(x) = slot(x - e_a, abar)
+// (wall link: slot(x, a)); collide; write f*_a(x) into slot (x + e_a, a) (wall link: slot(x, abar)),
+// after which the buffer is in natural layout again.  Each thread reads and writes exactly its
+// own set of Q slots, so there is no inter-thread hazard in either phase.
+template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256) stream_collide_aa_even(ST* __restrict__ buf, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= p.nx || y >= p.ny) return;
+  const long long ic = x + (long long)p.nx * (y + (long long)p.ny * z);
+  const CellFlags<WALLS> c(p, x, y, z);
+  double f[Q];
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    if constexpr (sizeof(ST) == 8) f[a] = buf[(long long)a * p.N + ic];
+    else f[a] = (double)buf[(long long)a * p.N + ic] + Dir<Q, a>::t;
+  });
+  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    st_pop<ST, Q, a>(buf, (long long)Dir<Q, a>::opp * p.N + ic, f[a]);
+  });
+}
+
+template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256) stream_collide_aa_odd(ST* __restrict__ buf, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= p.nx || y >= p.ny) return;
+  const Neigh nb(p, x, y, z);
+  const CellFlags<WALLS> c(p, x, y, z);
+  double f[Q];
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    constexpr int o = Dir<Q, a>::opp;
+    const bool wall_link = c.template leaves<Q, a, -1>();
+    const long long idx = wall_link ? (long long)a * p.N + nb.ic : (long long)o * p.N + nb.template at<Q, a, -1>();
+    double v;
+    if constexpr (sizeof(ST) == 8) v = buf[idx];
+    else v = (double)buf[idx] + Dir<Q, a>::t;  // t_a == t_abar
+    f[a] = v;
+  });
+  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    constexpr int o = Dir<Q, a>::opp;
+    const bool wall_link = c.template leaves<Q, a, 1>();
+    const long long idx = wall_link ? (long long)o * p.N + nb.ic : (long long)a * p.N + nb.template at<Q, a, 1>();
+    st_pop<ST, Q, a>(buf, idx, f[a]);
+  });
+}
+
+// ---------------------------------------------------------------------------------------
+// Canonical state access (D:R15).  MODE selects how slot contents map to f_a(x):
+//   NATURAL   : f_a(x) = slot(x, a)                                   (AA, even phase)
+//   PULL      : f_a(x) = slot(x - e_a, a),   wall link: slot(x, abar)   (A/B)
+//   PULL_SWAP : f_a(x) = slot(x - e_a, abar), wall link: slot(x, a)      (AA, odd phase)
+enum { MODE_NATURAL = 0, MODE_PULL = 1, MODE_PULL_SWAP = 2 };
+
+template <int Q, bool WALLS, int MODE, typename ST>
+__device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* __restrict__ buf, const Params& p, int x, int y, int z) {
+  const Neigh nb(p, x, y, z);
+  const CellFlags<WALLS> c(p, x, y, z);
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    constexpr int o = Dir<Q, a>::opp;
+    long long idx;
+    if constexpr (MODE == MODE_NATURAL) {
+      idx = (long long)a * p.N + nb.ic;
+    } else {
+      const bool wall_link = c.template leaves<Q, a, -1>();
+      constexpr int q_in = (MODE == MODE_PULL) ? a : o, q_wall = (MODE == MODE_PULL) ? o : a;
+      idx = wall_link ? (long long)q_wall * p.N + nb.ic : (long long)q_in * p.N + nb.template at<Q, a, -1>();
+    }
+    if constexpr (sizeof(ST) == 8) f[a] = buf[idx];
+    else f[a] = (double)buf[idx] + Dir<Q, a>::t;
+  });
+}
+
+__device__ __forceinline__ void decode(const Params& p, long long i, int& x, int& y, int& z) {
+  x = (int)(i % p.nx);
+  const long long r = i / p.nx;
+  y = (int)(r % p.ny);
+  z = (int)(r / p.ny);
+}
+
+// lbm_get_populations: canonical f[a*N+i] (always fp64) out of the storage buffer.
+template <int Q, bool WALLS, int MODE, typename ST>
+__global__ void __launch_bounds__(256) export_canonical(const ST* __restrict__ buf, double* __restrict__ out, const __grid_constant__ Params p) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
+    int x, y, z;
+    decode(p, i, x, y, z);
+    double f[Q];
+    load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      out[(long long)a * p.N + i] = f[a];
+    });
+  }
+}
+
+// lbm_set_populations / init: canonical f[a*N+i] (fp64) into the storage buffer.
+//   NATURAL: slot(x,a) = f_a(x).   PULL (A/B): slot(y,a) = f_a(y + e_a) inside, = f_abar(y) if y + e_a is outside.
+template <int Q, bool WALLS, int MODE, typename ST>
+__global__ void __launch_bounds__(256) import_canonical(const double* __restrict__ in, ST* __restrict__ buf, const __grid_constant__ Params p) {
+  static_assert(MODE != MODE_PULL_SWAP, "imports always land in an even phase");
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
+    int x, y, z;
+    decode(p, i, x, y, z);
+    const Neigh nb(p, x, y, z);
+    const CellFlags<WALLS> c(p, x, y, z);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      constexpr int o = Dir<Q, a>::opp;
+      long long idx;
+      if constexpr (MODE == MODE_NATURAL) {
+        idx = (long long)a * p.N + i;
+      } else {
+        const bool wall_link = c.template leaves<Q, a, 1>();
+        idx = wall_link ? (long long)o * p.N + i : (long long)a * p.N + nb.template at<Q, a, 1>();
+      }
+      st_pop<ST, Q, a>(buf, (long long)a * p.N + i, in[idx]);
+    });
+  }
+}
+
+// InitPDF: canonical f_a(x) = feq_a(rho(x), u(x)), natural fp64 layout.
+template <int Q, int EQ>
+__global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __restrict__ rho, const double* __restrict__ u, double* __restrict__ out, const __grid_constant__ Params p) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
+    const double r = rho ? rho[i] : 1.0;
+    const double ux = u ? u[i] : 0.0, uy = u ? u[p.N + i] : 0.0, uz = u ? u[2 * p.N + i] : 0.0;
+    double feq[Q];
+    equilibrium<Q, EQ>(feq, r, ux, uy, uz);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      out[(long long)a * p.N + i] = feq[a];
+    });
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// PostProcessing + Monitor: rho, u fields and the 8 diagnostics.
+// Per-thread accumulation over a grid-stride loop, warp shuffles, one partial per block,
+// then a single-block final pass in fixed order (deterministic, no floating-point atomics).
+constexpr int kDiag = 8;
+
+__device__ __forceinline__ void diag_combine(double (&a)[kDiag], const double (&b)[kDiag]) {
+  a[0] += b[0]; a[1] += b[1]; a[2] += b[2]; a[3] += b[3]; a[4] += b[4];
+  a[5] = fmax(a[5], b[5]);
+  a[6] = fmin(a[6], b[6]);
+  a[7] += b[7];
+}
+
+__device__ __forceinline__ void block_reduce_diag(double (&acc)[kDiag], double* __restrict__ out) {
+  __shared__ double sh[32][kDiag];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    double o[kDiag];
+#pragma unroll
+    for (int k = 0; k < kDiag; ++k) o[k] = __shfl_down_sync(0xffffffffu, acc[k], off);
+    diag_combine(acc, o);
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < kDiag; ++k) sh[warp][k] = acc[k];
+  }
+  __syncthreads();
+  if (warp == 0) {
+    double v[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
+    if (lane < nwarp) {
+#pragma unroll
+      for (int k = 0; k < kDiag; ++k) v[k] = sh[lane][k];
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      double o[kDiag];
+#pragma unroll
+      for (int k = 0; k < kDiag; ++k) o[k] = __shfl_down_sync(0xffffffffu, v[k], off);
+      diag_combine(v, o);
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int k = 0; k < kDiag; ++k) out[k] = v[k];
+    }
+  }
+}
+
+template <int Q, int EQ, bool WALLS, bool FORCE, int MODE, typename ST>
+__global__ void __launch_bounds__(256) moments_kernel(const ST* __restrict__ buf, double* __restrict__ rho_out, double* __restrict__ u_out,
+                                                      double* __restrict__ partials, const __grid_constant__ Params p) {
+  double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
+    int x, y, z;
+    decode(p, i, x, y, z);
+    double f[Q];
+    load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
+    double rho, ux, uy, uz;
+    moments<Q, EQ, FORCE>(f, p, rho, ux, uy, uz);
+    if (rho_out) rho_out[i] = rho;
+    if (u_out) {
+      u_out[i] = ux;
+      u_out[p.N + i] = uy;
+      u_out[2 * p.N + i] = uz;
+    }
+    const double usq = ux * ux + uy * uy + uz * uz;
+    if (isfinite(rho) && isfinite(usq)) {
+      const double rw = (EQ == EQ_STANDARD) ? rho : 1.0;
+      acc[0] += rho;
+      acc[1] += rw * ux;
+      acc[2] += rw * uy;
+      acc[3] += rw * uz;
+      acc[4] += 0.5 * rw * usq;
+      acc[5] = fmax(acc[5], sqrt(usq));
+      acc[6] = fmin(acc[6], rho);
+    } else {
+      acc[7] += 1.0;
+    }
+  }
+  if (partials) block_reduce_diag(acc, partials + (long long)blockIdx.x * kDiag);
+}
+
+__global__ void __launch_bounds__(256) reduce_final_kernel(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
+  double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+    double v[kDiag];
+#pragma unroll
+    for (int k = 0; k < kDiag; ++k) v[k] = partials[(long long)b * kDiag + k];
+    diag_combine(acc, v);
+  }
+  block_reduce_diag(acc, out);
+}
+
+}  // namespace lbm

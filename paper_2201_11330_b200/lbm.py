@@ -1,0 +1,260 @@
+"""Thin ctypes binding over the C ABI of include/lbm.h (same names, argument marshalling only).
+
+Every step of the path runs in the CUDA library; torch is used for device memory, streams
+and events.  There is no CPU fallback: if the library cannot be loaded, `load()` raises.
+
+Functions mirror the C names one to one (`lbm_create`, `lbm_init_equilibrium`, `lbm_step`,
+`lbm_moments`, ...).  `Solver` is a small convenience wrapper that owns a handle.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+LBM_D3Q19, LBM_D3Q27 = 19, 27
+LBM_EQ_STANDARD, LBM_EQ_INCOMP = 0, 1 << 8
+LBM_SCHEME_AUTO, LBM_SCHEME_AB, LBM_SCHEME_AA = 0, 1 << 12, 2 << 12
+LBM_STORE_F64, LBM_STORE_F32 = 0, 1 << 16
+LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING = 0, 1, 2
+LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
+
+# every symbol include/lbm.h declares (checked by tests/test_abi.py)
+SYMBOLS = (
+    "lbm_create", "lbm_destroy", "lbm_init_equilibrium", "lbm_init_equilibrium_host", "lbm_step",
+    "lbm_moments", "lbm_moments_host", "lbm_get_populations", "lbm_set_populations", "lbm_lattice",
+    "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_last_error",
+)
+
+
+class lbm_bc_t(C.Structure):
+    _fields_ = [
+        ("face_kind", C.c_int32 * 6),
+        ("face_u", (C.c_double * 3) * 6),
+        ("force", C.c_double * 3),
+        ("stream", C.c_void_p),
+    ]
+
+
+class LBMError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"lbm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Load liblbm_b200.so (built in-tree by `python -m paper_2201_11330_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2201_11330_b200.build` "
+            "(the CUDA library is the only implementation; there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, i32, i64 = C.c_void_p, C.c_void_p, C.c_int, C.c_int64
+    lib.lbm_create.restype = vp
+    lib.lbm_create.argtypes = [i32, i32, i32, i32, C.c_double, C.POINTER(lbm_bc_t)]
+    lib.lbm_destroy.restype = None
+    lib.lbm_destroy.argtypes = [vp]
+    for name in ("lbm_init_equilibrium", "lbm_init_equilibrium_host"):
+        getattr(lib, name).restype = i32
+        getattr(lib, name).argtypes = [vp, dp, dp]
+    lib.lbm_step.restype = i32
+    lib.lbm_step.argtypes = [vp, i32]
+    for name in ("lbm_moments", "lbm_moments_host"):
+        getattr(lib, name).restype = i32
+        getattr(lib, name).argtypes = [vp, dp, dp, dp]
+    for name in ("lbm_get_populations", "lbm_set_populations"):
+        getattr(lib, name).restype = i32
+        getattr(lib, name).argtypes = [vp, dp]
+    lib.lbm_lattice.restype = i32
+    lib.lbm_lattice.argtypes = [i32, C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+    lib.lbm_time.restype = i64
+    lib.lbm_time.argtypes = [vp]
+    lib.lbm_launch_count.restype = i64
+    lib.lbm_launch_count.argtypes = [vp]
+    lib.lbm_set_block.restype = i32
+    lib.lbm_set_block.argtypes = [vp, i32, i32]
+    lib.lbm_last_error.restype = C.c_char_p
+    lib.lbm_last_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def lbm_last_error() -> str:
+    return load().lbm_last_error().decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise LBMError(rc, lbm_last_error())
+
+
+def _ptr(t, n=None, device="cuda"):
+    """Raw address of a contiguous float64 torch tensor (or None)."""
+    if t is None:
+        return None
+    import torch
+    assert isinstance(t, torch.Tensor) and t.dtype == torch.float64 and t.is_contiguous(), "need a contiguous float64 tensor"
+    assert t.device.type == device, f"tensor must live on {device}, got {t.device}"
+    assert n is None or t.numel() == n, (t.numel(), n)
+    return t.data_ptr()
+
+
+def make_bc(face_kind=None, face_u=None, force=None, stream=None) -> lbm_bc_t:
+    bc = lbm_bc_t()
+    fk = [0] * 6 if face_kind is None else list(face_kind)
+    fu = np.zeros((6, 3)) if face_u is None else np.asarray(face_u, dtype=np.float64).reshape(6, 3)
+    fo = np.zeros(3) if force is None else np.asarray(force, dtype=np.float64).reshape(3)
+    for k in range(6):
+        bc.face_kind[k] = int(fk[k])
+        for d in range(3):
+            bc.face_u[k][d] = float(fu[k, d])
+    for d in range(3):
+        bc.force[d] = float(fo[d])
+    bc.stream = None if stream is None else int(stream)
+    return bc
+
+
+# ---- one function per C entry point ----------------------------------------------------
+def lbm_create(nx, ny, nz, lattice, tau, bc: lbm_bc_t | None = None):
+    h = load().lbm_create(int(nx), int(ny), int(nz), int(lattice), float(tau), None if bc is None else C.byref(bc))
+    if not h:
+        raise LBMError(LBM_EINVAL, lbm_last_error())
+    return h
+
+
+def lbm_destroy(h):
+    load().lbm_destroy(h)
+
+
+def lbm_init_equilibrium(h, rho=None, u=None):
+    _check(load().lbm_init_equilibrium(h, _ptr(rho), _ptr(u)))
+
+
+def lbm_init_equilibrium_host(h, rho=None, u=None):
+    _check(load().lbm_init_equilibrium_host(h, _ptr(rho, device="cpu"), _ptr(u, device="cpu")))
+
+
+def lbm_step(h, nsteps):
+    _check(load().lbm_step(h, int(nsteps)))
+
+
+def lbm_moments(h, rho=None, u=None, diagnostics=False):
+    """Fills the given device tensors; returns the 8 diagnostics as a numpy array if asked."""
+    diag = np.empty(8) if diagnostics else None
+    _check(load().lbm_moments(h, _ptr(rho), _ptr(u), None if diag is None else diag.ctypes.data))
+    return diag
+
+
+def lbm_moments_host(h, rho=None, u=None, diagnostics=False):
+    diag = np.empty(8) if diagnostics else None
+    _check(load().lbm_moments_host(h, _ptr(rho, device="cpu"), _ptr(u, device="cpu"), None if diag is None else diag.ctypes.data))
+    return diag
+
+
+def lbm_get_populations(h, f):
+    _check(load().lbm_get_populations(h, _ptr(f)))
+
+
+def lbm_set_populations(h, f):
+    _check(load().lbm_set_populations(h, _ptr(f)))
+
+
+def lbm_lattice(lattice):
+    Q = lattice & 0xFF
+    e = (C.c_int32 * (3 * Q))()
+    t = (C.c_double * Q)()
+    _check(load().lbm_lattice(int(lattice), e, t))
+    return np.array(e, dtype=np.int32).reshape(Q, 3), np.array(t, dtype=np.float64)
+
+
+def lbm_time(h) -> int:
+    return int(load().lbm_time(h))
+
+
+def lbm_launch_count(h) -> int:
+    return int(load().lbm_launch_count(h))
+
+
+def lbm_set_block(h, bx, by):
+    _check(load().lbm_set_block(h, int(bx), int(by)))
+
+
+# ---- convenience wrapper ----------------------------------------------------------------
+class Solver:
+    """Owns one handle.  All tensors are torch float64, on the solver's CUDA device unless the
+    method name says host."""
+
+    def __init__(self, nx, ny, nz, Q=19, tau=0.8, eq=LBM_EQ_STANDARD, scheme=LBM_SCHEME_AUTO, store=LBM_STORE_F64,
+                 face_kind=None, face_u=None, force=None, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2201_11330_b200 needs a CUDA device (no CPU fallback)")
+        self.nx, self.ny, self.nz, self.Q = int(nx), int(ny), int(nz), int(Q)
+        self.N = self.nx * self.ny * self.nz
+        self.torch_stream = stream  # torch.cuda.Stream or None
+        raw = None if stream is None else stream.cuda_stream
+        self.bc = make_bc(face_kind, face_u, force, raw)
+        self.h = lbm_create(nx, ny, nz, int(Q) | eq | scheme | store, tau, self.bc)
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        return cls(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u, force=w.force, **kw)
+
+    def close(self):
+        if getattr(self, "h", None):
+            lbm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def init_equilibrium(self, rho=None, u=None):
+        lbm_init_equilibrium(self.h, rho, u)
+
+    def init_equilibrium_host(self, rho=None, u=None):
+        lbm_init_equilibrium_host(self.h, rho, u)
+
+    def step(self, n=1):
+        lbm_step(self.h, n)
+
+    def moments(self, fields=True, diagnostics=True):
+        import torch
+        rho = torch.empty(self.N, dtype=torch.float64, device="cuda") if fields else None
+        u = torch.empty(3 * self.N, dtype=torch.float64, device="cuda") if fields else None
+        diag = lbm_moments(self.h, rho, u, diagnostics)
+        return rho, (None if u is None else u.view(3, self.N)), diag
+
+    def diagnostics(self):
+        return lbm_moments(self.h, None, None, True)
+
+    def get_populations(self, out=None):
+        import torch
+        f = torch.empty(self.Q * self.N, dtype=torch.float64, device="cuda") if out is None else out
+        lbm_get_populations(self.h, f)
+        return f.view(self.Q, self.N)
+
+    def set_populations(self, f):
+        lbm_set_populations(self.h, f.contiguous().view(-1))
+
+    @property
+    def time(self):
+        return lbm_time(self.h)
+
+    @property
+    def launches(self):
+        return lbm_launch_count(self.h)
+
+    def set_block(self, bx, by):
+        lbm_set_block(self.h, bx, by)

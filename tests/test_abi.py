@@ -1,0 +1,94 @@
+"""CPU-only checks of the C-ABI library: it loads without a GPU, exports every symbol that
+include/lbm.h declares, validates arguments before touching CUDA, and documents a lattice order
+identical to the oracle's (each side wrote its own table)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import lattice as oracle_lattice
+from paper_2201_11330_b200 import build as lbm_build
+from paper_2201_11330_b200 import lbm
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    lbm_build.build()
+    return lbm.load()
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lbm_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(lib):
+    names = _declared_functions()
+    assert set(names) == set(lbm.SYMBOLS), (names, lbm.SYMBOLS)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/lbm.h but not exported"
+
+
+def test_signatures_have_no_torch_types():
+    src = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    assert 'extern "C"' in src
+    code = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    assert "torch" not in code.lower() and "at::" not in code and "#include <stdint.h>" in code
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+def test_lattice_order_matches_oracle(lib, Q):
+    e, t = lbm.lbm_lattice(Q)
+    eo, to = oracle_lattice(Q)
+    assert (e == eo).all()
+    assert (t == to).all()
+
+
+def test_invalid_arguments_fail_before_cuda(lib):
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(8, 8, 8, 19, 0.5)  # tau <= 0.5
+    assert "tau" in lbm.lbm_last_error()
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(8, 8, 8, 15, 0.8)  # unknown lattice
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(0, 8, 8, 19, 0.8)
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(8, 8, 8, 19, 0.8, lbm.make_bc(face_kind=[1, 0, 0, 0, 0, 0]))  # unpaired periodic
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(8, 8, 8, 19, 0.8, lbm.make_bc(face_kind=[7, 7, 0, 0, 0, 0]))
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create(8, 8, 8, 19 | (3 << 12), 0.8)  # unknown scheme
+    assert lib.lbm_step(None, 1) == lbm.LBM_EINVAL
+    assert lib.lbm_init_equilibrium(None, None, None) == lbm.LBM_EINVAL
+    assert lib.lbm_moments(None, None, None, None) == lbm.LBM_EINVAL
+    assert lib.lbm_time(None) == -1
+    lib.lbm_destroy(None)  # no-op
+    assert lbm.lbm_lattice(19)[0].shape == (19, 3)
+    e = (C.c_int32 * 3)()
+    assert lib.lbm_lattice(5, e, (C.c_double * 1)()) == lbm.LBM_EINVAL
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    monkeypatch.setattr(lbm, "_lib", None)
+    monkeypatch.setattr(lbm, "LIB_PATH", str(tmp_path / "nope.so"))
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        lbm.load()
+
+
+def test_product_never_imports_oracle():
+    """The product path must not route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2201_11330_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", txt, flags=re.M), fn
+                assert "lbm_oracle" not in txt, fn
+    otxt = open(os.path.join(ROOT, "oracle", "lbm_oracle.cpp")).read() + open(os.path.join(ROOT, "oracle", "binding.py")).read()
+    assert "paper_2201_11330_b200" not in re.sub(r"//.*|#.*", "", otxt)
+    assert "lbm_kernels" not in re.sub(r"//.*", "", otxt)

@@ -1,0 +1,415 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances (BASELINE.json north_star): max |df| <= 1e-12 for fp64
+storage, <= 2e-5 relative for the fp32-storage variant.  Run with `pytest -m gpu` on a B200.
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from oracle.binding import EQ_INCOMP, EQ_STANDARD
+from paper_2201_11330_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+TOL = 1e-12
+
+B, M, P = inputs.FACE_BOUNCE, inputs.FACE_MOVING, inputs.FACE_PERIODIC
+
+
+@pytest.fixture(scope="module")
+def lbm():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2201_11330_b200 import lbm as _lbm
+    _lbm.load()  # raises loudly if the CUDA library is missing
+    return _lbm
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def eq_flag(lbm, eq):
+    return lbm.LBM_EQ_INCOMP if eq == EQ_INCOMP else lbm.LBM_EQ_STANDARD
+
+
+def make_pair(lbm, dims, Q, tau, eq=EQ_STANDARD, scheme=None, face_kind=None, face_u=None, force=None, store=0):
+    nx, ny, nz = dims
+    o = Oracle(nx, ny, nz, Q, tau, eq=eq, face_kind=face_kind, face_u=face_u, force=force)
+    s = lbm.Solver(nx, ny, nz, Q, tau, eq=eq_flag(lbm, eq), scheme=scheme or lbm.LBM_SCHEME_AB, store=store,
+                   face_kind=face_kind, face_u=face_u, force=force)
+    return o, s
+
+
+def random_f(Q, N, seed, amp=0.2):
+    """Random non-equilibrium populations around the weights (from the oracle-independent lattice rule:
+    weights only matter as a positive scale here)."""
+    rng = np.random.default_rng(seed)
+    base = np.full((Q, 1), 1.0 / Q)
+    return base * (1.0 + amp * rng.uniform(-1, 1, (Q, N)))
+
+
+def schemes(lbm):
+    return [("ab", lbm.LBM_SCHEME_AB), ("aa", lbm.LBM_SCHEME_AA)]
+
+
+FACE_CASES = {
+    "periodic": ([P] * 6, None),
+    "channel_z": ([P, P, P, P, B, B], None),
+    "cavity": ([B, B, B, B, B, M], {5: (0.1, 0.0, 0.0)}),
+    "mixed": ([B, M, P, P, M, B], {1: (0.0, 0.03, -0.02), 4: (0.05, 0.01, 0.0)}),
+    "all_moving": ([M] * 6, {k: (0.01 * (k + 1), -0.02, 0.005 * k) for k in range(6)}),
+}
+
+
+def face_u_of(spec):
+    fu = np.zeros((6, 3))
+    for k, v in (spec or {}).items():
+        fu[k] = v
+    return fu
+
+
+# --------------------------------------------------------------------------- element-wise parity, all variants
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+@pytest.mark.parametrize("faces", list(FACE_CASES))
+@pytest.mark.parametrize("Q,eq,forced", [(19, EQ_STANDARD, False), (19, EQ_STANDARD, True), (19, EQ_INCOMP, False),
+                                         (19, EQ_INCOMP, True), (27, EQ_STANDARD, False), (27, EQ_STANDARD, True),
+                                         (27, EQ_INCOMP, True)])
+def test_random_populations_ragged_grid(lbm, scheme, faces, Q, eq, forced):
+    """Ragged 37x21x13 grid (several 32-wide tiles + a tail in x, odd y and z), random non-equilibrium
+    populations, 7 steps (odd: the AA scheme is compared in its swapped phase too)."""
+    dims = (37, 21, 13)
+    N = dims[0] * dims[1] * dims[2]
+    fk, fu = FACE_CASES[faces]
+    fu = face_u_of(fu)
+    F = (2e-4, -1e-4, 3e-4) if forced else None
+    o, s = make_pair(lbm, dims, Q, 0.77, eq, dict(schemes(lbm))[scheme], fk, fu, F)
+    f0 = random_f(Q, N, seed=Q + 100 * eq)
+    o.set_f(f0)
+    s.set_populations(dev(f0))
+    assert np.abs(s.get_populations().cpu().numpy() - f0).max() == 0.0  # import/export round trip is exact
+    for nsteps in (1, 2, 4):  # compare after 1, 3 and 7 steps
+        o.step(nsteps)
+        s.step(nsteps)
+        got = s.get_populations().cpu().numpy()
+        assert np.abs(got - o.get_f()).max() <= TOL
+    rho, u, d = s.moments()
+    ro, uo, do = o.moments()
+    assert np.abs(rho.cpu().numpy() - ro).max() <= 1e-13
+    assert np.abs(u.cpu().numpy() - uo).max() <= 1e-13
+    np.testing.assert_allclose(d[:5], do[:5], rtol=1e-12, atol=1e-12)
+    np.testing.assert_allclose(d[5:7], do[5:7], rtol=1e-14)
+    assert d[7] == do[7] == 0
+    s.close()
+
+
+@pytest.mark.parametrize("dims", [(1, 1, 1), (2, 3, 1), (4, 4, 4), (3, 2, 5), (300, 5, 3), (64, 64, 2), (33, 1, 7)])
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_degenerate_and_edge_sizes(lbm, dims, scheme):
+    """Smallest grids (wrap onto itself), a row longer than one 256-thread block, single-plane grids."""
+    N = dims[0] * dims[1] * dims[2]
+    for fk, fu in (([P] * 6, None), ([B, B, B, B, B, M], {5: (0.1, 0.0, 0.0)})):
+        o, s = make_pair(lbm, dims, 19, 0.6, EQ_STANDARD, dict(schemes(lbm))[scheme], fk, face_u_of(fu), (1e-5, 0, 2e-5))
+        f0 = random_f(19, N, seed=N)
+        o.set_f(f0)
+        s.set_populations(dev(f0))
+        o.step(5)
+        s.step(5)
+        assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+        s.close()
+
+
+@pytest.mark.parametrize("bx,by", [(32, 1), (32, 8), (64, 4), (128, 2), (256, 1), (32, 4)])
+def test_block_shapes_give_identical_results(lbm, bx, by):
+    dims = (70, 19, 6)
+    N = dims[0] * dims[1] * dims[2]
+    f0 = random_f(19, N, seed=5)
+    ref = None
+    for shape in ((0, 0), (bx, by)):
+        s = lbm.Solver(*dims, 19, 0.7)
+        s.set_block(*shape)
+        s.set_populations(dev(f0))
+        s.step(3)
+        got = s.get_populations().cpu().numpy()
+        s.close()
+        if ref is None:
+            ref = got
+        else:
+            assert (got == ref).all()
+
+
+# --------------------------------------------------------------------------- init, moments, host variants
+
+@pytest.mark.parametrize("Q,eq", [(19, EQ_STANDARD), (27, EQ_STANDARD), (19, EQ_INCOMP)])
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_init_equilibrium_matches_oracle(lbm, Q, eq, scheme):
+    dims = (20, 9, 11)
+    N = dims[0] * dims[1] * dims[2]
+    rng = np.random.default_rng(11)
+    rho = 1 + 0.05 * rng.standard_normal(N)
+    u = 0.05 * rng.standard_normal((3, N))
+    fk, fu = FACE_CASES["cavity"]
+    o, s = make_pair(lbm, dims, Q, 0.8, eq, dict(schemes(lbm))[scheme], fk, face_u_of(fu))
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= 1e-15
+    assert s.time == 0
+    # NULL fields: rho = 1, u = 0
+    o.init_equilibrium(None, None)
+    s.init_equilibrium(None, None)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= 1e-16
+    s.close()
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_host_entry_points_equal_device_ones(lbm, scheme):
+    w = inputs.config(0).scaled(24, steps=9)
+    rho, u = w.fields()
+    a = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme])
+    b = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme])
+    a.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    rho_h = torch.from_numpy(rho).pin_memory()
+    u_h = torch.from_numpy(u.reshape(-1).copy()).pin_memory()
+    b.init_equilibrium_host(rho_h, u_h)
+    a.step(w.steps)
+    b.step(w.steps)
+    assert (a.get_populations() == b.get_populations()).all()
+    ra, ua, da = a.moments()
+    rb = torch.empty(w.N, dtype=torch.float64).pin_memory()
+    ub = torch.empty(3 * w.N, dtype=torch.float64).pin_memory()
+    db = lbm.lbm_moments_host(b.h, rb, ub, True)
+    assert (ra.cpu() == rb).all() and (ua.cpu().reshape(-1) == ub).all() and (da == db).all()
+    # stepping still works after the idle buffer was used as staging
+    a.step(2)
+    b.step(2)
+    assert (a.get_populations() == b.get_populations()).all()
+    a.close()
+    b.close()
+
+
+def test_nonfinite_cells_are_counted(lbm):
+    dims = (8, 8, 8)
+    s = lbm.Solver(*dims, 19, 0.8)
+    f0 = random_f(19, 512, seed=1)
+    f0[3, 17] = np.nan
+    f0[5, 100] = np.inf
+    s.set_populations(dev(f0))
+    d = s.diagnostics()
+    assert d[7] == 2 and np.isfinite(d[:7]).all()
+    s.close()
+
+
+def test_step_zero_and_time_counter(lbm):
+    s = lbm.Solver(8, 8, 8, 19, 0.8)
+    s.init_equilibrium()
+    s.step(0)
+    assert s.time == 0
+    s.step(3)
+    assert s.time == 3
+    with pytest.raises(lbm.LBMError):
+        s.step(-1)
+    s.close()
+
+
+# --------------------------------------------------------------------------- BASELINE.json configs
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_config0_tgv32_full_length(lbm, scheme):
+    """configs[0]: 32^3 periodic Taylor-Green, tau 0.8, 100 steps: parity, energy decay, conservation."""
+    w = inputs.config(0)
+    rho, u = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau)
+    s = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme])
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    d0 = s.diagnostics()
+    E = [d0[4]]
+    for _ in range(w.steps):
+        s.step(1)
+        E.append(s.diagnostics()[4])
+    o.step(w.steps)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    d1 = s.diagnostics()
+    do = o.moments(False)[2]
+    np.testing.assert_allclose(d1[:5], do[:5], rtol=1e-12, atol=1e-12)
+    nu, k2 = (w.tau - 0.5) / 3, 3 * (2 * np.pi / w.nx) ** 2
+    slope = np.polyfit(np.arange(10, 101), np.log(E[10:101]), 1)[0]
+    assert abs(slope / (-2 * nu * k2) - 1) < 0.03
+    assert abs(d1[0] - d0[0]) / d0[0] < 1e-13
+    np.testing.assert_allclose(d1[1:4], d0[1:4], atol=1e-11)
+    s.close()
+
+
+def test_config1_tgv128_full_length(lbm):
+    """configs[1]: 128^3 periodic Taylor-Green, tau 0.6, 1000 steps, full-length parity against the oracle."""
+    w = inputs.config(1)
+    rho, u = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau)
+    s = lbm.Solver.from_workload(w)
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    o.step(w.steps)
+    s.step(w.steps)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    s.close()
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_config2_cavity_analogue_full_length(lbm, scheme):
+    """configs[2] on a 32^3 analogue for the full 2000 steps (the 256^3 oracle run costs 3.4e10 updates)."""
+    w = inputs.config(2).scaled(32)
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u)
+    s = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme])
+    o.init_equilibrium(None, None)
+    s.init_equilibrium(None, None)
+    o.step(w.steps)
+    s.step(w.steps)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    rho, u, d = s.moments()
+    assert abs(d[0] - w.N) / w.N < 1e-12  # mass
+    uy = u[1].cpu().numpy().reshape(32, 32, 32)
+    assert np.abs(uy + uy[:, ::-1, :]).max() < 1e-13  # mirror antisymmetry
+    s.close()
+
+
+def test_config2_cavity256_first_steps(lbm):
+    """configs[2] at its full 256^3 size, first 10 steps, element-wise."""
+    w = inputs.config(2)
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u)
+    s = lbm.Solver.from_workload(w)
+    o.init_equilibrium(None, None)
+    s.init_equilibrium(None, None)
+    o.step(10)
+    s.step(10)
+    got = s.get_populations().cpu().numpy()
+    assert np.abs(got - o.get_f()).max() <= TOL
+    s.close()
+
+
+def _subbox_check(lbm, w, solver, k, centers, halo=2):
+    """Sampled parity at full size: f after k steps at a cell depends only on the initial fields within
+    distance k, so the oracle runs on a small sub-box cut around each sample (global walls kept where the
+    box touches them, cut sides are far enough away) and its core cells are compared with the GPU's."""
+    Q = w.Q
+    fgpu = solver.get_populations().view(Q, w.nz, w.ny, w.nx)
+    n = (w.nx, w.ny, w.nz)
+    worst = 0.0
+    for c in centers:
+        lo, hi, fk, core = [], [], list(w.face_kind), []
+        for d in range(3):
+            a, b = c[d] - k - halo, c[d] + k + halo + 1
+            periodic = w.face_kind[2 * d] == P
+            if not periodic:
+                a, b = max(a, 0), min(b, n[d])
+            lo.append(a)
+            hi.append(b)
+            # cut sides of a non-periodic axis get a resting wall (garbage confined to k cells from it)
+            if not periodic:
+                fk[2 * d] = w.face_kind[2 * d] if a == 0 else B
+                fk[2 * d + 1] = w.face_kind[2 * d + 1] if b == n[d] else B
+            cl = a + (0 if (not periodic and a == 0) else k + 1)
+            ch = b - (0 if (not periodic and b == n[d]) else k + 1)
+            core.append((cl, ch))
+        box = tuple((lo[d], hi[d]) for d in range(3))
+        rho, u = w.fields(box)
+        dims = [hi[d] - lo[d] for d in range(3)]
+        o = Oracle(dims[0], dims[1], dims[2], Q, w.tau, face_kind=fk, face_u=w.face_u, force=w.force)
+        o.init_equilibrium(rho, u)
+        o.step(k)
+        fo = o.get_f().reshape(Q, dims[2], dims[1], dims[0])
+        for gz in range(core[2][0], core[2][1]):
+            for gy in range(core[1][0], core[1][1]):
+                xs = np.arange(core[0][0], core[0][1])
+                ref = fo[:, gz - lo[2], gy - lo[1], xs - lo[0]]
+                got = fgpu[:, gz % n[2], gy % n[1], torch.from_numpy(xs % n[0]).cuda()].cpu().numpy()
+                worst = max(worst, np.abs(got - ref).max())
+    return worst
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_config3_tgv512_sampled(lbm, scheme):
+    """configs[3] (headline, 512^3): sampled sub-box parity after 3 steps at corners, edges, faces and
+    interior points, plus mass/momentum conservation over the steps (properties that hold at any size)."""
+    w = inputs.config(3)
+    rho, u = w.fields()
+    s = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme])
+    rho_h = torch.from_numpy(rho).pin_memory()
+    u_h = torch.from_numpy(u.reshape(-1)).pin_memory()
+    s.init_equilibrium_host(rho_h, u_h)
+    d0 = s.diagnostics()
+    k = 3
+    s.step(k)
+    centers = [(0, 0, 0), (511, 511, 511), (0, 255, 511), (256, 0, 17), (100, 200, 300), (255, 256, 511), (31, 32, 33)]
+    assert _subbox_check(lbm, w, s, k, centers) <= TOL
+    s.step(20 - k)
+    d1 = s.diagnostics()
+    assert abs(d1[0] - d0[0]) / d0[0] < 1e-13
+    np.testing.assert_allclose(d1[1:4], d0[1:4], atol=1e-9)
+    assert d1[7] == 0 and d1[4] < d0[4]
+    s.close()
+
+
+def test_config4_channel512_sampled(lbm):
+    """configs[4] (D3Q27, 512^3 forced channel): sampled sub-box parity after 3 steps next to both walls and
+    inside, and the plane-averaged profile against the analytic start-up series after 200 steps."""
+    w = inputs.config(4)
+    rho, u = w.fields()
+    s = lbm.Solver.from_workload(w)
+    s.init_equilibrium_host(torch.from_numpy(rho).pin_memory(), None)
+    k = 3
+    s.step(k)
+    centers = [(0, 0, 0), (511, 511, 511), (17, 300, 1), (200, 5, 510), (256, 256, 256), (511, 0, 2)]
+    assert _subbox_check(lbm, w, s, k, centers) <= TOL
+    steps = 200
+    s.step(steps - k)
+    _, uf, d = s.moments()
+    prof = uf[0].view(512, 512 * 512).mean(dim=1).cpu().numpy()
+    H, F, nu = 512, w.force[0], (w.tau - 0.5) / 3
+    z = np.arange(H) + 0.5
+    u_an = F * z * (H - z) / (2 * nu)
+    for n_ in range(1, 4000, 2):
+        u_an -= 4 * F * H * H / (nu * np.pi**3 * n_**3) * np.sin(n_ * np.pi * z / H) * np.exp(-n_ * n_ * np.pi**2 * nu * steps / H**2)
+    assert np.linalg.norm(prof - u_an) / np.linalg.norm(u_an) < 1e-2
+    assert abs(d[0] / w.N - 1) < 1e-5 and d[7] == 0
+    s.close()
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+def test_channel_steady_state_small_H(lbm, Q):
+    """configs[4] physics on the converged nz = 16 analogue through the GPU: parabola + BGK slip constant."""
+    H, tau, F = 16, 0.9, 1e-7
+    nu = (tau - 0.5) / 3
+    fk = [P, P, P, P, B, B]
+    o, s = make_pair(lbm, (4, 4, H), Q, tau, face_kind=fk, force=(F, 0, 0))
+    o.init_equilibrium(None, None)
+    s.init_equilibrium(None, None)
+    o.step(20000)
+    s.step(20000)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    _, u, _ = s.moments()
+    prof = u[0].cpu().numpy().reshape(H, 16).mean(axis=1)
+    z = np.arange(H) + 0.5
+    ref = F * z * (H - z) / (2 * nu) + F / (2 * nu) * (4 * (tau - 0.5) ** 2 / 3 - 0.25)
+    assert np.abs(prof - ref).max() / ref.max() < 1e-9
+    s.close()
+
+
+# --------------------------------------------------------------------------- fp32-storage variant (S:§8f NEXT-1)
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_fp32_storage_variant(lbm, scheme):
+    """BASELINE.json north_star: populations match the oracle within 2e-5 relative with fp32 storage."""
+    w = inputs.config(0)
+    rho, u = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau)
+    s = lbm.Solver.from_workload(w, scheme=dict(schemes(lbm))[scheme], store=lbm.LBM_STORE_F32)
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    o.step(w.steps)
+    s.step(w.steps)
+    ref = o.get_f()
+    got = s.get_populations().cpu().numpy()
+    assert (np.abs(got - ref) / np.abs(ref)).max() <= 2e-5
+    s.close()
