@@ -74,12 +74,12 @@ struct CellFlags {
   bool lo[3], hi[3];  // cell is in the first / last plane of an axis whose face there is a wall
   __device__ __forceinline__ CellFlags(const Params& p, int x, int y, int z) {
     if constexpr (WALLS) {
-      lo[0] = (x == 0) && p.wall[0];
-      hi[0] = (x == p.nx - 1) && p.wall[1];
-      lo[1] = (y == 0) && p.wall[2];
-      hi[1] = (y == p.ny - 1) && p.wall[3];
-      lo[2] = (z == 0) && p.wall[4];
-      hi[2] = (z == p.nz - 1) && p.wall[5];
+      lo[0] = (x == 0) & (p.wall[0] != 0);
+      hi[0] = (x == p.nx - 1) & (p.wall[1] != 0);
+      lo[1] = (y == 0) & (p.wall[2] != 0);
+      hi[1] = (y == p.ny - 1) & (p.wall[3] != 0);
+      lo[2] = (z == 0) & (p.wall[4] != 0);
+      hi[2] = (z == p.nz - 1) & (p.wall[5] != 0);
     } else {
       lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
     }
@@ -89,13 +89,14 @@ struct CellFlags {
   __device__ __forceinline__ bool leaves() const {
     if constexpr (!WALLS) return false;
     constexpr int dx = S * Dir<Q, A>::ex, dy = S * Dir<Q, A>::ey, dz = S * Dir<Q, A>::ez;
+    // bitwise OR on purpose: a short-circuit || makes ptxas branch around the loads it guards
     bool out = false;
-    if constexpr (dx == -1) out = out || lo[0];
-    if constexpr (dx == 1) out = out || hi[0];
-    if constexpr (dy == -1) out = out || lo[1];
-    if constexpr (dy == 1) out = out || hi[1];
-    if constexpr (dz == -1) out = out || lo[2];
-    if constexpr (dz == 1) out = out || hi[2];
+    if constexpr (dx == -1) out = out | lo[0];
+    if constexpr (dx == 1) out = out | hi[0];
+    if constexpr (dy == -1) out = out | lo[1];
+    if constexpr (dy == 1) out = out | hi[1];
+    if constexpr (dz == -1) out = out | lo[2];
+    if constexpr (dz == 1) out = out | hi[2];
     return out;
   }
 };
@@ -293,7 +294,7 @@ __global__ void __launch_bounds__(256) stream_collide_ab(const ST* __restrict__ 
     constexpr int a = decltype(A)::value;
     const bool wall_link = c.template leaves<Q, a, -1>();
     const long long idx = wall_link ? (long long)Dir<Q, a>::opp * p.N + nb.ic : (long long)a * p.N + nb.template at<Q, a, -1>();
-    f[a] = wall_link ? ld_pop<ST, Q, Dir<Q, a>::opp>(src, idx) : ld_pop<ST, Q, a>(src, idx);
+    f[a] = ld_pop<ST, Q, a>(src, idx);  // t_a == t_abar, so one load serves both cases
   });
   collide<Q, EQ, WALLS, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
