@@ -49,7 +49,8 @@ struct lbm_handle_s {
   double* diag_pinned;  // 8, host
   void* scratch;
   size_t scratch_bytes;
-  int bx, by;
+  int bx, by;         // block shape of the fused kernel (lbm_set_block)
+  int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
   size_t elem() const { return f32 ? 4 : 8; }
   size_t buf_bytes() const { return (size_t)N * Q * elem(); }
 };
@@ -80,8 +81,10 @@ namespace {
     BODY;                              \
   } break;
 
-int flat_grid(long long N) {
-  long long b = (N + 255) / 256;
+// blocks of the row-wise sweeps (for_each_cell): 256/fbx rows per block, at most one wave
+int flat_grid(const lbm_handle_s* h) {
+  const long long rows = (long long)h->ny * h->nz, by = 256 / h->fbx;
+  const long long b = (rows + by - 1) / by;
   return (int)(b < kReduceBlocks ? b : kReduceBlocks);
 }
 
@@ -114,17 +117,17 @@ int launch_step(lbm_handle_s* h) {
 
 template <typename ST>
 void launch_export(lbm_handle_s* h, double* out) {
-  const int g = flat_grid(h->N);
+  const int g = flat_grid(h);
   const ST* b = (const ST*)h->buf[h->cur];
   switch (read_mode(h)) {
     case MODE_NATURAL:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
       break;
     case MODE_PULL:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
       break;
     default:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, out, h->p)));
+      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
   }
   ++h->launches;
 }
@@ -132,12 +135,12 @@ void launch_export(lbm_handle_s* h, double* out) {
 // canonical fp64 array `in` -> storage buffer `dst_idx` in the layout the scheme wants at an even phase
 template <typename ST>
 void launch_import(lbm_handle_s* h, const double* in, int dst_idx) {
-  const int g = flat_grid(h->N);
+  const int g = flat_grid(h);
   ST* b = (ST*)h->buf[dst_idx];
   if (h->scheme == LBM_SCHEME_AB)
-    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(in, b, h->p)));
+    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(in, b, h->fbx, h->p)));
   else
-    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(in, b, h->p)));
+    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(in, b, h->fbx, h->p)));
   ++h->launches;
 }
 
@@ -146,13 +149,13 @@ void launch_moments(lbm_handle_s* h, double* rho, double* u, double* partials, i
   const ST* b = (const ST*)h->buf[h->cur];
   switch (read_mode(h)) {
     case MODE_NATURAL:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
       break;
     case MODE_PULL:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
       break;
     default:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->p)));
+      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
   }
   ++h->launches;
 }
@@ -197,13 +200,13 @@ int do_init(lbm_handle_s* h, const double* rho, const double* u) {
   double* nat = nullptr;
   int rc = canonical_staging(h, &nat);
   if (rc) return rc;
-  const int g = flat_grid(h->N);
+  const int g = flat_grid(h);
   if (h->eq) {
-    if (h->Q == 19) init_equilibrium_kernel<19, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
-    else init_equilibrium_kernel<27, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+    if (h->Q == 19) init_equilibrium_kernel<19, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
+    else init_equilibrium_kernel<27, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
   } else {
-    if (h->Q == 19) init_equilibrium_kernel<19, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
-    else init_equilibrium_kernel<27, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->p);
+    if (h->Q == 19) init_equilibrium_kernel<19, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
+    else init_equilibrium_kernel<27, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
   }
   ++h->launches;
   if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
@@ -215,7 +218,7 @@ int do_init(lbm_handle_s* h, const double* rho, const double* u) {
 }
 
 int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
-  const int g = flat_grid(h->N);
+  const int g = flat_grid(h);
   double* partials = diagnostics ? h->partials : nullptr;
   if (h->f32) launch_moments<float>(h, rho, u, partials, g);
   else launch_moments<double>(h, rho, u, partials, g);
@@ -272,6 +275,7 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
   const int Q = lattice & 0xff;
   if (Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
   if (nx < 1 || ny < 1 || nz < 1) { fail(LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1"); return nullptr; }
+  if ((long long)nx * ny * nz >= (1LL << 31)) { fail(LBM_EUNSUPPORTED, "lbm_create: nx*ny*nz must be < 2^31 (in-plane offsets are 32-bit)"); return nullptr; }
   if (nz > 65535 || ny > 65535) { fail(LBM_EINVAL, "lbm_create: ny or nz exceeds the launch grid limits"); return nullptr; }
   if (!(tau > 0.5) || !std::isfinite(tau)) { fail(LBM_EINVAL, "lbm_create: tau must be finite and > 0.5"); return nullptr; }
   int scheme = lattice & (3 << 12);
@@ -318,6 +322,7 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
   int bx = 32;
   while (bx < nx && bx < 256) bx *= 2;
   h->bx = bx; h->by = 256 / bx;
+  h->fbx = bx;
 
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
   cudaError_t e = cudaSuccess;

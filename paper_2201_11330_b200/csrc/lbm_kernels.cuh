@@ -54,6 +54,13 @@ __device__ __forceinline__ void static_for(F&& f) {
   }
 }
 
+// Resident 256-thread blocks per SM the fused kernels are compiled for (register cap 80 / 128).
+// Measured on B200: the A/B D3Q19 kernels fit 80 registers without spilling and need the third block
+// (the fp32-storage variant loses 15 % of its bandwidth at two); the forced and in-place variants
+// and D3Q27 spill below 128.
+template <int Q, bool FORCE, bool INPLACE>
+constexpr int kMinBlocks = (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
+
 // ---------------------------------------------------------------------------------------
 struct Params {
   int nx, ny, nz;
@@ -101,37 +108,51 @@ struct CellFlags {
   }
 };
 
-// Neighbour offsets of one cell with periodic wrap by conditional add (no %).
+// Neighbour offsets of one cell with periodic wrap by conditional add (no %).  Offsets inside one
+// direction plane are 32-bit (lbm_create refuses N >= 2^31); the plane base alpha*N is 64-bit and
+// thread-invariant, so it lives in uniform registers and an address costs one IMAD.WIDE.
 struct Neigh {
-  long long ox[3], oy[3], oz[3];  // index 0: coordinate-1, 1: same, 2: coordinate+1
-  long long ic;
+  int ox[3], oy[3], oz[3];  // index 0: coordinate-1, 1: same, 2: coordinate+1
+  int ic;
   __device__ __forceinline__ Neigh(const Params& p, int x, int y, int z) {
     const int xm = (x == 0) ? p.nx - 1 : x - 1, xp = (x == p.nx - 1) ? 0 : x + 1;
     const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
     const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
-    const long long sy = p.nx, sz = (long long)p.nx * p.ny;
+    const int sy = p.nx, sz = p.nx * p.ny;
     ox[0] = xm; ox[1] = x; ox[2] = xp;
     oy[0] = ym * sy; oy[1] = y * sy; oy[2] = yp * sy;
     oz[0] = zm * sz; oz[1] = z * sz; oz[2] = zp * sz;
     ic = ox[1] + oy[1] + oz[1];
   }
-  // linear index of x + s*e_A (wrapped)
+  // in-plane index of x + s*e_A (wrapped)
   template <int Q, int A, int S>
-  __device__ __forceinline__ long long at() const {
+  __device__ __forceinline__ int at() const {
     return ox[1 + S * Dir<Q, A>::ex] + oy[1 + S * Dir<Q, A>::ey] + oz[1 + S * Dir<Q, A>::ez];
   }
 };
+
+// Base of direction plane A of a population buffer (64-bit, thread-invariant).
+template <int A, typename T>
+__device__ __forceinline__ T* plane(T* buf, long long N) {
+  return buf + (long long)A * N;
+}
 
 // ---------------------------------------------------------------------------------------
 // Storage element access.  fp64: the value itself.  fp32 storage (S:§8f NEXT-1): f - t_a is
 // kept as float, arithmetic stays fp64.
 template <typename ST, int Q, int A>
-__device__ __forceinline__ double ld_pop(const ST* __restrict__ p, long long i) {
+__device__ __forceinline__ double ld_pop(const ST* __restrict__ p, int i) {
   if constexpr (sizeof(ST) == 8) return __ldg(p + i);
   else return (double)__ldg(p + i) + Dir<Q, A>::t;
 }
+// same through a plain (coherent) load: the in-place kernels read the buffer they write
 template <typename ST, int Q, int A>
-__device__ __forceinline__ void st_pop(ST* __restrict__ p, long long i, double v) {
+__device__ __forceinline__ double ld_pop_rw(const ST* p, int i) {
+  if constexpr (sizeof(ST) == 8) return p[i];
+  else return (double)p[i] + Dir<Q, A>::t;
+}
+template <typename ST, int Q, int A>
+__device__ __forceinline__ void st_pop(ST* __restrict__ p, int i, double v) {
   if constexpr (sizeof(ST) == 8) p[i] = v;
   else p[i] = (float)(v - Dir<Q, A>::t);
 }
@@ -282,7 +303,7 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
 // link.  One step = pull (gives the canonical pre-collision f of this time level), collide,
 // store aligned at the own cell into the other buffer (which is again S^-1 of the next f).
 template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
@@ -292,14 +313,16 @@ __global__ void __launch_bounds__(256) stream_collide_ab(const ST* __restrict__ 
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    const bool wall_link = c.template leaves<Q, a, -1>();
-    const long long idx = wall_link ? (long long)Dir<Q, a>::opp * p.N + nb.ic : (long long)a * p.N + nb.template at<Q, a, -1>();
-    f[a] = ld_pop<ST, Q, a>(src, idx);  // t_a == t_abar, so one load serves both cases
+    const ST* q = plane<a>(src, p.N) + nb.template at<Q, a, -1>();
+    if constexpr (WALLS) {
+      if (c.template leaves<Q, a, -1>()) q = plane<Dir<Q, a>::opp>(src, p.N) + nb.ic;  // a select, not a branch
+    }
+    f[a] = ld_pop<ST, Q, a>(q, 0);  // t_a == t_abar: one load serves both cases
   });
   collide<Q, EQ, WALLS, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    st_pop<ST, Q, a>(dst, (long long)a * p.N + nb.ic, f[a]);
+    st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
   });
 }
 
@@ -307,30 +330,30 @@ __global__ void __launch_bounds__(256) stream_collide_ab(const ST* __restrict__ 
 // write f*_a(x) into slot (x, abar) — every access aligned.  Odd phase: f_a(x) = slot(x - e_a, abar)
 // (wall link: slot(x, a)); collide; write f*_a(x) into slot (x + e_a, a) (wall link: slot(x, abar)),
 // after which the buffer is in natural layout again.  Each thread reads and writes exactly its
-// own set of Q slots, so there is no inter-thread hazard in either phase.
+// own set of Q slots (the odd phase writes f*_a where it read f_abar), so there is no
+// inter-thread hazard in either phase.
 template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256) stream_collide_aa_even(ST* __restrict__ buf, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_even(ST* buf, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
-  const long long ic = x + (long long)p.nx * (y + (long long)p.ny * z);
+  const int ic = x + p.nx * (y + p.ny * z);
   const CellFlags<WALLS> c(p, x, y, z);
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    if constexpr (sizeof(ST) == 8) f[a] = buf[(long long)a * p.N + ic];
-    else f[a] = (double)buf[(long long)a * p.N + ic] + Dir<Q, a>::t;
+    f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), ic);
   });
   collide<Q, EQ, WALLS, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    st_pop<ST, Q, a>(buf, (long long)Dir<Q, a>::opp * p.N + ic, f[a]);
+    st_pop<ST, Q, a>(plane<Dir<Q, a>::opp>(buf, p.N), ic, f[a]);
   });
 }
 
 template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256) stream_collide_aa_odd(ST* __restrict__ buf, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_odd(ST* buf, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
@@ -338,23 +361,25 @@ __global__ void __launch_bounds__(256) stream_collide_aa_odd(ST* __restrict__ bu
   const Neigh nb(p, x, y, z);
   const CellFlags<WALLS> c(p, x, y, z);
   double f[Q];
+  // f_a(x) comes from the slot that f*_abar(x) goes to (link x <-> x - e_a traversed both ways)
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
-    const bool wall_link = c.template leaves<Q, a, -1>();
-    const long long idx = wall_link ? (long long)a * p.N + nb.ic : (long long)o * p.N + nb.template at<Q, a, -1>();
-    double v;
-    if constexpr (sizeof(ST) == 8) v = buf[idx];
-    else v = (double)buf[idx] + Dir<Q, a>::t;  // t_a == t_abar
-    f[a] = v;
+    const ST* q = plane<o>(buf, p.N) + nb.template at<Q, a, -1>();
+    if constexpr (WALLS) {
+      if (c.template leaves<Q, a, -1>()) q = plane<a>(buf, p.N) + nb.ic;
+    }
+    f[a] = ld_pop_rw<ST, Q, a>(q, 0);
   });
   collide<Q, EQ, WALLS, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
-    const bool wall_link = c.template leaves<Q, a, 1>();
-    const long long idx = wall_link ? (long long)o * p.N + nb.ic : (long long)a * p.N + nb.template at<Q, a, 1>();
-    st_pop<ST, Q, a>(buf, idx, f[a]);
+    ST* q = plane<a>(buf, p.N) + nb.template at<Q, a, 1>();
+    if constexpr (WALLS) {
+      if (c.template leaves<Q, a, 1>()) q = plane<o>(buf, p.N) + nb.ic;
+    }
+    st_pop<ST, Q, a>(q, 0, f[a]);
   });
 }
 
@@ -366,85 +391,88 @@ __global__ void __launch_bounds__(256) stream_collide_aa_odd(ST* __restrict__ bu
 enum { MODE_NATURAL = 0, MODE_PULL = 1, MODE_PULL_SWAP = 2 };
 
 template <int Q, bool WALLS, int MODE, typename ST>
-__device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* __restrict__ buf, const Params& p, int x, int y, int z) {
+__device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, const Params& p, int x, int y, int z) {
   const Neigh nb(p, x, y, z);
   const CellFlags<WALLS> c(p, x, y, z);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
-    long long idx;
+    const ST* q;
     if constexpr (MODE == MODE_NATURAL) {
-      idx = (long long)a * p.N + nb.ic;
+      q = plane<a>(buf, p.N) + nb.ic;
     } else {
-      const bool wall_link = c.template leaves<Q, a, -1>();
       constexpr int q_in = (MODE == MODE_PULL) ? a : o, q_wall = (MODE == MODE_PULL) ? o : a;
-      idx = wall_link ? (long long)q_wall * p.N + nb.ic : (long long)q_in * p.N + nb.template at<Q, a, -1>();
+      q = plane<q_in>(buf, p.N) + nb.template at<Q, a, -1>();
+      if constexpr (WALLS) {
+        if (c.template leaves<Q, a, -1>()) q = plane<q_wall>(buf, p.N) + nb.ic;
+      }
     }
-    if constexpr (sizeof(ST) == 8) f[a] = buf[idx];
-    else f[a] = (double)buf[idx] + Dir<Q, a>::t;
+    f[a] = ld_pop_rw<ST, Q, a>(q, 0);
   });
 }
 
-__device__ __forceinline__ void decode(const Params& p, long long i, int& x, int& y, int& z) {
-  x = (int)(i % p.nx);
-  const long long r = i / p.nx;
-  y = (int)(r % p.ny);
-  z = (int)(r / p.ny);
+// Row-wise grid-stride loop of the sweeps off the per-step path: a 256-thread block is bx x (256/bx)
+// with bx a power of two covering the row (or 256); rows (y,z) are dealt to the blocks round-robin.
+// One 32-bit division per row, none per cell; x stays the coalesced direction.
+template <typename F>
+__device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body) {
+  const int tx = threadIdx.x & (bx - 1), ty = threadIdx.x / bx, by = blockDim.x / bx;
+  const int rows = p.ny * p.nz;
+  for (int r = blockIdx.x * by + ty; r < rows; r += gridDim.x * by) {
+    const int z = r / p.ny, y = r - z * p.ny;
+    for (int x = tx; x < p.nx; x += bx) body(x, y, z, x + p.nx * r);
+  }
 }
 
 // lbm_get_populations: canonical f[a*N+i] (always fp64) out of the storage buffer.
 template <int Q, bool WALLS, int MODE, typename ST>
-__global__ void __launch_bounds__(256) export_canonical(const ST* __restrict__ buf, double* __restrict__ out, const __grid_constant__ Params p) {
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
-    int x, y, z;
-    decode(p, i, x, y, z);
+__global__ void __launch_bounds__(256, 2) export_canonical(const ST* buf, double* __restrict__ out, int bx, const __grid_constant__ Params p) {
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
     double f[Q];
     load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
-      out[(long long)a * p.N + i] = f[a];
+      plane<a>(out, p.N)[i] = f[a];
     });
-  }
+  });
 }
 
 // lbm_set_populations / init: canonical f[a*N+i] (fp64) into the storage buffer.
 //   NATURAL: slot(x,a) = f_a(x).   PULL (A/B): slot(y,a) = f_a(y + e_a) inside, = f_abar(y) if y + e_a is outside.
 template <int Q, bool WALLS, int MODE, typename ST>
-__global__ void __launch_bounds__(256) import_canonical(const double* __restrict__ in, ST* __restrict__ buf, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256) import_canonical(const double* __restrict__ in, ST* __restrict__ buf, int bx, const __grid_constant__ Params p) {
   static_assert(MODE != MODE_PULL_SWAP, "imports always land in an even phase");
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
-    int x, y, z;
-    decode(p, i, x, y, z);
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
     const Neigh nb(p, x, y, z);
     const CellFlags<WALLS> c(p, x, y, z);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       constexpr int o = Dir<Q, a>::opp;
-      long long idx;
-      if constexpr (MODE == MODE_NATURAL) {
-        idx = (long long)a * p.N + i;
-      } else {
-        const bool wall_link = c.template leaves<Q, a, 1>();
-        idx = wall_link ? (long long)o * p.N + i : (long long)a * p.N + nb.template at<Q, a, 1>();
+      const double* q = plane<a>(in, p.N) + i;
+      if constexpr (MODE != MODE_NATURAL) {
+        q = plane<a>(in, p.N) + nb.template at<Q, a, 1>();
+        if constexpr (WALLS) {
+          if (c.template leaves<Q, a, 1>()) q = plane<o>(in, p.N) + i;
+        }
       }
-      st_pop<ST, Q, a>(buf, (long long)a * p.N + i, in[idx]);
+      st_pop<ST, Q, a>(plane<a>(buf, p.N), i, __ldg(q));
     });
-  }
+  });
 }
 
 // InitPDF: canonical f_a(x) = feq_a(rho(x), u(x)), natural fp64 layout.
 template <int Q, int EQ>
-__global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __restrict__ rho, const double* __restrict__ u, double* __restrict__ out, const __grid_constant__ Params p) {
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
+__global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __restrict__ rho, const double* __restrict__ u, double* __restrict__ out, int bx, const __grid_constant__ Params p) {
+  for_each_cell(p, bx, [&](int, int, int, int i) {
     const double r = rho ? rho[i] : 1.0;
-    const double ux = u ? u[i] : 0.0, uy = u ? u[p.N + i] : 0.0, uz = u ? u[2 * p.N + i] : 0.0;
+    const double ux = u ? u[i] : 0.0, uy = u ? plane<1>(u, p.N)[i] : 0.0, uz = u ? plane<2>(u, p.N)[i] : 0.0;
     double feq[Q];
     equilibrium<Q, EQ>(feq, r, ux, uy, uz);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
-      out[(long long)a * p.N + i] = feq[a];
+      plane<a>(out, p.N)[i] = feq[a];
     });
-  }
+  });
 }
 
 // ---------------------------------------------------------------------------------------
@@ -496,12 +524,10 @@ __device__ __forceinline__ void block_reduce_diag(double (&acc)[kDiag], double* 
 }
 
 template <int Q, int EQ, bool WALLS, bool FORCE, int MODE, typename ST>
-__global__ void __launch_bounds__(256) moments_kernel(const ST* __restrict__ buf, double* __restrict__ rho_out, double* __restrict__ u_out,
-                                                      double* __restrict__ partials, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256, 2) moments_kernel(const ST* buf, double* __restrict__ rho_out, double* __restrict__ u_out,
+                                                      double* __restrict__ partials, int bx, const __grid_constant__ Params p) {
   double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.N; i += (long long)gridDim.x * blockDim.x) {
-    int x, y, z;
-    decode(p, i, x, y, z);
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
     double f[Q];
     load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
     double rho, ux, uy, uz;
@@ -509,8 +535,8 @@ __global__ void __launch_bounds__(256) moments_kernel(const ST* __restrict__ buf
     if (rho_out) rho_out[i] = rho;
     if (u_out) {
       u_out[i] = ux;
-      u_out[p.N + i] = uy;
-      u_out[2 * p.N + i] = uz;
+      plane<1>(u_out, p.N)[i] = uy;
+      plane<2>(u_out, p.N)[i] = uz;
     }
     const double usq = ux * ux + uy * uy + uz * uz;
     if (isfinite(rho) && isfinite(usq)) {
@@ -525,7 +551,7 @@ __global__ void __launch_bounds__(256) moments_kernel(const ST* __restrict__ buf
     } else {
       acc[7] += 1.0;
     }
-  }
+  });
   if (partials) block_reduce_diag(acc, partials + (long long)blockIdx.x * kDiag);
 }
 
