@@ -14,6 +14,7 @@ from .build import build
 _lib = None
 
 EQ_STANDARD, EQ_INCOMP = 0, 1
+WALL_HALFWAY, WALL_NODAL = 0, 1
 FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
@@ -37,6 +38,9 @@ def _load():
         for name in ("orc_get_f", "orc_get_fb", "orc_set_f"):
             getattr(lib, name).argtypes = [C.c_void_p, _dp]
         lib.orc_get_f_cells.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int64, _dp]
+        lib.orc_set_geometry.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        lib.orc_get_active.argtypes = [C.c_void_p, C.c_void_p]
+        lib.orc_boundary_force.argtypes = [C.c_void_p, _dp]
         lib.orc_num_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -97,6 +101,24 @@ class Oracle:
             self._h = None
 
     __del__ = close
+
+    def set_geometry(self, geo=None, wall_model=WALL_HALFWAY):
+        """geo: N uint8 (non-zero = solid node) or None; call before init_equilibrium / set_f."""
+        g = None if geo is None else np.ascontiguousarray(geo, dtype=np.uint8).reshape(-1)
+        assert g is None or g.size == self.N
+        rc = self._lib.orc_set_geometry(self._h, None if g is None else g.ctypes.data, int(wall_model))
+        if rc != 0:
+            raise ValueError("unknown wall model")
+
+    def active(self):
+        out = np.empty(self.N, dtype=np.uint8)
+        self._lib.orc_get_active(self._h, out.ctypes.data)
+        return out
+
+    def boundary_force(self):
+        F = np.empty(3)
+        self._lib.orc_boundary_force(self._h, _p(F))
+        return F
 
     def init_equilibrium(self, rho=None, u=None):
         rho, u = _f64(rho, self.N), _f64(u, 3 * self.N)

@@ -23,6 +23,12 @@
 //   indexing .................. pinned: independent brute-force gather on 4^3 (long double)
 //   D3Q27 ..................... pinned only through the same invariants and closed forms;
 //                               no D3Q27-specific printed value exists in the paper.
+//   solid mask `geo` .......... pinned: brute-force gather with a mask; staircase channel built from
+//                               the mask equals the face-built channel bit for bit
+//   nodal bounce-back (Eq. 10)  pinned: second-order convergence of the channel profile (the
+//                               paper's own claim), wall position, mirror symmetry
+//   momentum exchange (Eq. 13)  pinned: exact momentum balance of the fluid region per step;
+//                               steady drag = total body force
 //
 // Floating point: IEEE double throughout ("double precision"); compile with
 // -ffp-contract=off so that no FMA contraction happens.  Reductions for the
@@ -77,6 +83,10 @@ bool make_lattice(int Q, Lattice& L) {
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };              // Eq. 2 | Eq. 5
 enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2 };
+// D:R3 / D:R16.  HALFWAY: the wall lies half a link beyond the last fluid node (BASELINE.json
+// configs).  NODAL: the paper's "modified nodal bounce back" (Eq. 10): wall nodes lie on
+// the wall, receive f_alpha = f_abar for the directions no node streams into them, and collide.
+enum { WALL_HALFWAY = 0, WALL_NODAL = 1 };
 
 struct Oracle {
   int nx, ny, nz;
@@ -91,6 +101,9 @@ struct Oracle {
   std::vector<double> f;      // P:208 `f`:  pre-collision populations, AoS f[id*Q+iq]
   std::vector<double> fb;     // P:208 `fb`: "backup" = post-collision populations
   std::vector<double> rho_w;  // density seen by the collision sweep, kept for the wall term (D:R6)
+  std::vector<uint8_t> geo;     // P:210 `geo`: 1 = solid node, 0 = fluid node (all fluid by default)
+  std::vector<uint8_t> active;  // node takes part in collision and propagation (D:R16)
+  int wall_model = WALL_HALFWAY;
   int64_t steps_done = 0;
 
   int64_t cell(int x, int y, int z) const { return (int64_t)x + (int64_t)nx * ((int64_t)y + (int64_t)ny * z); }
@@ -125,7 +138,76 @@ inline void moments_of(const Oracle& o, const double* fc, double& rho, double u[
   for (int d = 0; d < 3; ++d) u[d] = (m[d] + 0.5 * o.F[d]) / div;
 }
 
-// InitPDF: f(x, 0) = feq(rho0(x), u0(x)).
+// Node x + s*e_iq with periodic wrap.  Returns false if it lies outside the box through a
+// non-periodic face; then `moving_face` is the MOVING face crossed (D:R6 tie-break: the highest
+// face index among the MOVING faces crossed) or -1.
+inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int out[3], int* moving_face) {
+  const int c[3] = {x, y, z}, n[3] = {o.nx, o.ny, o.nz};
+  bool inside = true;
+  if (moving_face) *moving_face = -1;
+  for (int d = 0; d < 3; ++d) {
+    out[d] = c[d] + sgn * o.L.e[iq][d];
+    if (out[d] < 0 || out[d] >= n[d]) {
+      const int face = 2 * d + (out[d] < 0 ? 0 : 1);
+      if (o.face_kind[face] == FACE_PERIODIC) {
+        out[d] = ((out[d] % n[d]) + n[d]) % n[d];
+      } else {
+        inside = false;
+        if (moving_face && o.face_kind[face] == FACE_MOVING && face > *moving_face) *moving_face = face;
+      }
+    }
+  }
+  return inside;
+}
+
+// D:R16.  HALFWAY: the active nodes are the fluid nodes (geo = 0).  NODAL: also every solid node
+// with at least one fluid node among its lattice neighbours — these are the wall nodes on which
+// "a collision operation is then applied ... like in the fluid bulk"; deeper solid nodes
+// take no part.
+void classify_nodes(Oracle& o) {
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x) {
+        const int64_t i = o.cell(x, y, z);
+        uint8_t a = o.geo[i] == 0;
+        if (!a && o.wall_model == WALL_NODAL) {
+          for (int iq = 0; iq < o.L.Q && !a; ++iq) {
+            int s[3];
+            if (neighbour(o, x, y, z, iq, +1, s, nullptr) && o.geo[o.cell(s[0], s[1], s[2])] == 0) a = 1;
+          }
+        }
+        o.active[i] = a;
+      }
+}
+
+// Eq. 10 on the wall nodes of the NODAL model: a direction alpha that no active node
+// streams into the node ("unknown") takes the value of its opposite, f_alpha = f_abar, when abar
+// itself arrived from an active node.  D:R17: if both ends of the link are inactive (an edge or
+// corner of the wall) the pair keeps what `keep` holds for it (propagation passes the node's own
+// post-collision fb_abar, i.e. plain bounce-back; init/set pass nothing and leave f untouched).
+void replicate_nodal(Oracle& o, int x, int y, int z, const double* keep /* fb of this node or NULL */) {
+  const int Q = o.L.Q;
+  const int64_t i = o.cell(x, y, z);
+  for (int iq = 0; iq < Q; ++iq) {
+    int up[3], dn[3];
+    const bool up_active = neighbour(o, x, y, z, iq, -1, up, nullptr) && o.active[o.cell(up[0], up[1], up[2])];
+    if (up_active) continue;
+    const bool dn_active = neighbour(o, x, y, z, iq, +1, dn, nullptr) && o.active[o.cell(dn[0], dn[1], dn[2])];
+    if (dn_active) o.f[i * Q + iq] = o.f[i * Q + (Q - 1 - iq)];
+    else if (keep) o.f[i * Q + iq] = keep[Q - 1 - iq];
+  }
+}
+
+void make_state_consistent(Oracle& o) {
+  if (o.wall_model != WALL_NODAL) return;
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x)
+        if (o.active[o.cell(x, y, z)]) replicate_nodal(o, x, y, z, nullptr);
+}
+
+// InitPDF: f(x, 0) = feq(rho0(x), u0(x)).  D:R17: under the NODAL model the state
+// is then made consistent with Eq. 10 on the wall nodes.
 void init_pdf(Oracle& o, const double* rho, const double* u /* SoA u[c*N+i] */) {
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < o.N; ++i) {
@@ -135,6 +217,7 @@ void init_pdf(Oracle& o, const double* rho, const double* u /* SoA u[c*N+i] */) 
       for (int d = 0; d < 3; ++d) uu[d] = u[(int64_t)d * o.N + i];
     for (int iq = 0; iq < o.L.Q; ++iq) o.f[i * o.L.Q + iq] = feq_value(o, iq, r, uu);
   }
+  make_state_consistent(o);
   o.steps_done = 0;
 }
 
@@ -146,6 +229,7 @@ void collision(Oracle& o) {
   const bool forced = (o.F[0] != 0.0 || o.F[1] != 0.0 || o.F[2] != 0.0);
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < o.N; ++i) {
+    if (!o.active[i]) continue;  // the loop runs over `fluid_id` (here: the active nodes, D:R16)
     const double* fc = &o.f[i * Q];
     double rho, u[3];
     moments_of(o, fc, rho, u);
@@ -171,43 +255,33 @@ void collision(Oracle& o) {
 // pre-propagation form of Eq. 10 for a wall half-way between nodes (D:R3).
 void boundary_condition(Oracle&) {}
 
-// Sweep 3 — Propagation (Eq. 7):  f_alpha(x, t) = fb_alpha(x - e_alpha, t - 1).
-// If x - e_alpha leaves the box through a non-periodic face the link is a wall link:
-//   f_alpha(x) = fb_opp(alpha)(x)                                  [Eq. 10; opp = Q-1-alpha, P:49]
-//              + 6 t_alpha rho_w (e_alpha . u_w)                   [D:R6, Ladd; u_w = 0 on resting walls]
+// Sweep 3 — Propagation (Eq. 7):  f_alpha(x, t) = fb_alpha(x - e_alpha, t - 1), for every
+// active node x.  If x - e_alpha is not an active node (it is a solid node of `geo`, or lies
+// outside the box through a non-periodic face) nothing streams in along alpha:
+//   HALFWAY (D:R3):  f_alpha(x) = fb_opp(alpha)(x)                  [Eq. 10; opp = Q-1-alpha, P:49]
+//                               + 6 t_alpha rho_w (e_alpha . u_w)   [D:R6, Ladd; only through a MOVING face]
+//   NODAL: f_alpha(x) = f_opp(alpha)(x), the value that has just arrived at the wall
+//                    node from the fluid side (Eq. 10 applied after propagation); D:R17 for
+//                    links with no active node at either end.
 // D:R6 tie-break: when the upstream node lies beyond several non-periodic faces, a MOVING
 // face takes precedence over BOUNCE faces; among several MOVING faces the highest face
 // index (z+ > z- > y+ > y- > x+ > x-) is used.
 void propagation(Oracle& o) {
   const int Q = o.L.Q;
-  const int n[3] = {o.nx, o.ny, o.nz};
 #pragma omp parallel for schedule(static)
   for (int z = 0; z < o.nz; ++z)
     for (int y = 0; y < o.ny; ++y)
       for (int x = 0; x < o.nx; ++x) {
-        const int c[3] = {x, y, z};
         const int64_t i = o.cell(x, y, z);
+        if (!o.active[i]) continue;
         for (int iq = 0; iq < Q; ++iq) {
-          int s[3];
-          bool outside = false;
-          int moving_face = -1;
-          for (int d = 0; d < 3; ++d) {
-            s[d] = c[d] - o.L.e[iq][d];
-            if (s[d] < 0 || s[d] >= n[d]) {
-              const int face = 2 * d + (s[d] < 0 ? 0 : 1);
-              if (o.face_kind[face] == FACE_PERIODIC) {
-                s[d] = ((s[d] % n[d]) + n[d]) % n[d];
-              } else {
-                outside = true;
-                if (o.face_kind[face] == FACE_MOVING && face > moving_face) moving_face = face;
-              }
-            }
-          }
-          if (!outside) {
+          int s[3], moving_face;
+          const bool inside = neighbour(o, x, y, z, iq, -1, s, &moving_face);
+          if (inside && o.active[o.cell(s[0], s[1], s[2])]) {
             o.f[i * Q + iq] = o.fb[o.cell(s[0], s[1], s[2]) * Q + iq];
-          } else {
+          } else if (o.wall_model == WALL_HALFWAY) {
             double v = o.fb[i * Q + (Q - 1 - iq)];
-            if (moving_face >= 0) {
+            if (!inside && moving_face >= 0) {
               double eduw = 0.0;
               for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * o.face_u[moving_face][d];
               v += 6.0 * o.L.t[iq] * o.rho_w[i] * eduw;
@@ -215,13 +289,39 @@ void propagation(Oracle& o) {
             o.f[i * Q + iq] = v;
           }
         }
+        if (o.wall_model == WALL_NODAL) replicate_nodal(o, x, y, z, &o.fb[i * Q]);
       }
+}
+
+// Momentum-exchange force on the solid nodes of `geo` (Eq. 13), for the step that
+// has just been taken (fb = post-collision populations f* of time t, f = populations after
+// propagation):
+//   F = sum over fluid nodes x next to the body, sum over outgoing directions alpha
+//       (x + e_alpha is a solid node of geo):  [ f*_alpha(x, t) + f_abar(x, t + dt) ] e_alpha
+// "Fluid node" = geo 0.  Box-face walls are not part of the body.  Defined after >= 1 step.
+void boundary_force(const Oracle& o, double F[3]) {
+  const int Q = o.L.Q;
+  long double acc[3] = {0, 0, 0};
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x) {
+        const int64_t i = o.cell(x, y, z);
+        if (o.geo[i] != 0 || !o.active[i]) continue;
+        for (int iq = 0; iq < Q; ++iq) {
+          int d3[3];
+          if (!neighbour(o, x, y, z, iq, +1, d3, nullptr)) continue;
+          if (o.geo[o.cell(d3[0], d3[1], d3[2])] == 0) continue;
+          const double term = o.fb[i * Q + iq] + o.f[i * Q + (Q - 1 - iq)];
+          for (int d = 0; d < 3; ++d) acc[d] += (long double)term * o.L.e[iq][d];
+        }
+      }
+  for (int d = 0; d < 3; ++d) F[d] = (double)acc[d];
 }
 
 // Sweep 4 — PostProcessing (Eq. 8-9) and Monitor, on
 // demand.  diagnostics[8] = { sum rho, sum rho u_x, sum rho u_y, sum rho u_z,
 // 1/2 sum rho |u|^2, max |u|, min rho, number of cells with a non-finite rho or u }.
-// Under Eq. 5 "rho u" and "rho |u|^2" use rho0 (D:R5).  D:R13: 3-component magnitude,
+// Sums run over the active nodes (D:R16).  Under Eq. 5 "rho u" and "rho |u|^2" use rho0 (D:R5).  D:R13: 3-component magnitude,
 // all cells (the listing's 2-D magnitude and idn=1 start are typos of the extraction).
 void post_processing(const Oracle& o, double* rho_out, double* u_out, double* diag) {
   long double s_rho = 0, s_m[3] = {0, 0, 0}, s_e = 0;
@@ -229,6 +329,12 @@ void post_processing(const Oracle& o, double* rho_out, double* u_out, double* di
   int64_t bad = 0;
   for (int64_t i = 0; i < o.N; ++i) {
     double rho, u[3];
+    if (!o.active[i]) {  // Monitor runs over the fluid nodes only; inactive nodes report 0
+      if (rho_out) rho_out[i] = 0.0;
+      if (u_out)
+        for (int d = 0; d < 3; ++d) u_out[(int64_t)d * o.N + i] = 0.0;
+      continue;
+    }
     moments_of(o, &o.f[i * o.L.Q], rho, u);
     if (rho_out) rho_out[i] = rho;
     if (u_out)
@@ -289,10 +395,30 @@ void* orc_create(int nx, int ny, int nz, int Q, int eq, double tau, const int* f
   o->f.assign((size_t)o->N * Q, 0.0);
   o->fb.assign((size_t)o->N * Q, 0.0);
   o->rho_w.assign((size_t)o->N, 1.0);
+  o->geo.assign((size_t)o->N, 0);
+  o->active.assign((size_t)o->N, 1);
   return o;
 }
 
 void orc_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+// SetGeometry: geo[i] != 0 marks a solid node (NULL = all fluid); wall_model is
+// WALL_HALFWAY (0) or WALL_NODAL (1).  Re-classifies the nodes; call before init / set_f.
+int orc_set_geometry(void* h, const uint8_t* geo, int wall_model) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (wall_model != WALL_HALFWAY && wall_model != WALL_NODAL) return -1;
+  o.wall_model = wall_model;
+  for (int64_t i = 0; i < o.N; ++i) o.geo[i] = (geo && geo[i]) ? 1 : 0;
+  classify_nodes(o);
+  return 0;
+}
+
+void orc_get_active(void* h, uint8_t* out) {
+  const Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t i = 0; i < o.N; ++i) out[i] = o.active[i];
+}
+
+void orc_boundary_force(void* h, double* F) { boundary_force(*static_cast<Oracle*>(h), F); }
 
 // Lattice tables in the oracle's order: e_out[3*Q] (e[iq*3+d], the paper's e(iq*dim+ind),
 // P:373) and t_out[Q].
@@ -337,7 +463,7 @@ void orc_moments(void* h, double* rho, double* u, double* diag) { post_processin
 
 static void export_soa(const Oracle& o, const std::vector<double>& a, double* out) {
   for (int iq = 0; iq < o.L.Q; ++iq)
-    for (int64_t i = 0; i < o.N; ++i) out[(int64_t)iq * o.N + i] = a[i * o.L.Q + iq];
+    for (int64_t i = 0; i < o.N; ++i) out[(int64_t)iq * o.N + i] = o.active[i] ? a[i * o.L.Q + iq] : 0.0;  // inactive nodes report 0
 }
 
 void orc_get_f(void* h, double* out) { export_soa(*static_cast<Oracle*>(h), static_cast<Oracle*>(h)->f, out); }
@@ -347,6 +473,7 @@ void orc_set_f(void* h, const double* in) {
   Oracle& o = *static_cast<Oracle*>(h);
   for (int iq = 0; iq < o.L.Q; ++iq)
     for (int64_t i = 0; i < o.N; ++i) o.f[i * o.L.Q + iq] = in[(int64_t)iq * o.N + i];
+  make_state_consistent(o);  // D:R17
 }
 
 // Populations of selected cells only: out[k*Q + iq] for cell index cells[k].
