@@ -1,7 +1,7 @@
 /* include/lbm.h — C ABI of the B200-native lattice-Boltzmann hot path.
  *
  * The operation: the per-time-step fused streaming + BGK collision update of the
- * D3Q19 / D3Q27 populations of IMEXLBM (arXiv 2201.11330) on an nx*ny*nz box, fp64.
+ * D3Q19 / D3Q27 (and D2Q9) populations of IMEXLBM (arXiv 2201.11330) on an nx*ny*nz box, fp64.
  * "P:n" = line n of the paper text; "D:Rk" = reading k in DESIGN.md §2.
  *
  *   collision    f*_a = f_a - omega (f_a - feq_a)                 P:61-63, Eq. 6
@@ -44,8 +44,9 @@ typedef struct lbm_handle_s* lbm_handle; /* opaque, owned by the library */
 
 /* `lattice` argument of lbm_create: velocity set | equilibrium | storage scheme | storage type */
 enum {
-  LBM_D3Q19 = 19,           /* low byte: number of velocities                                  */
-  LBM_D3Q27 = 27,
+  LBM_D2Q9 = 9,             /* low byte: number of velocities.  D2Q9 exactly as printed in      */
+  LBM_D3Q19 = 19,           /* Eq. 3-4, e_z = 0: every z-plane is an independent 2-D     */
+  LBM_D3Q27 = 27,           /* domain (use nz = 1 for one)                                      */
   LBM_EQ_STANDARD = 0,      /* Eq. 2, weakly compressible (default)                            */
   LBM_EQ_INCOMP = 1 << 8,   /* Eq. 5, incompressible model with rho0 = 1               */
   LBM_SCHEME_AUTO = 0,      /* = LBM_SCHEME_AB                                                 */
@@ -56,6 +57,12 @@ enum {
 };
 
 enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2 };
+
+/* Wall model of lbm_set_geometry (D:R3, D:R16, D:R17). */
+enum {
+  LBM_WALL_HALFWAY = 0, /* link-wise bounce-back, wall half a link beyond the last fluid node (default) */
+  LBM_WALL_NODAL = 1    /* the paper's modified nodal bounce-back (Eq. 10): wall ON the nodes  */
+};
 
 enum {
   LBM_OK = 0,
@@ -86,8 +93,34 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
 /* Free all device memory of the handle (synchronises its stream).  NULL is a no-op. */
 void lbm_destroy(lbm_handle h);
 
+/* SetGeometry (`geo` P:210) and the wall model.  geo: N bytes (DEVICE pointer), non-zero =
+ * solid node, or NULL = no solid nodes.  Call before lbm_init_equilibrium / lbm_set_populations.
+ *   Active nodes (D:R16): HALFWAY: the fluid nodes (geo = 0).  NODAL: also every solid node with
+ *   a fluid node among its lattice neighbours (the wall nodes, which collide "like in the fluid
+ *   bulk"); with geo = NULL the first / last planes of BOUNCE faces are the wall nodes.
+ *   Only active nodes are updated; inactive nodes report 0 in every output and are excluded
+ *   from the diagnostics.  A link whose upstream node x - e_a is not active (solid, or beyond a
+ *   non-periodic face) is resolved as
+ *     HALFWAY: f_a(x, t+1) = f*_abar(x, t)                  (+ the Ladd term through a MOVING face)
+ *     NODAL  : f_a(x, t+1) = f_abar(x, t+1) (Eq. 10: the value that has just arrived along abar)
+ *              if x + e_a is active, else f*_abar(x, t) (D:R17: links inside the wall)
+ * One 32-bit link mask per node is built here and read by the step kernel (+4 B per node and
+ * step); (NULL, LBM_WALL_HALFWAY) returns to the mask-free analytic box.  LBM_WALL_NODAL with
+ * LBM_FACE_MOVING faces returns LBM_EUNSUPPORTED.  Synchronises the stream. */
+int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model);
+/* Same with a HOST pointer to the N mask bytes. */
+int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model);
+
+/* Momentum-exchange force on the solid nodes of geo (Eq. 13) for the last step taken:
+ *   F = sum over fluid nodes x, over a with x + e_a a solid node of geo (inside the box):
+ *       [ f*_a(x, t) + f_abar(x, t + 1) ] e_a
+ * F: HOST pointer to 3 doubles.  Box-face walls are not part of the body.  Needs a geometry and
+ * at least one lbm_step since the populations were last set (else LBM_EINVAL).  Synchronises. */
+int lbm_boundary_force(lbm_handle h, double* F);
+
 /* P:82, P:276-278 (InitPDF): f_a(x, 0) = feq_a(rho(x), u(x)); resets the step counter.
- * rho: N doubles or NULL (= 1 everywhere); u: 3N doubles or NULL (= 0).  Device pointers. */
+ * rho: N doubles or NULL (= 1 everywhere); u: 3N doubles or NULL (= 0).  Device pointers.
+ * Under LBM_WALL_NODAL the wall nodes then satisfy Eq. 10 (D:R17). */
 int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u);
 /* Same with HOST pointers; the fields are copied to the device on the handle's stream. */
 int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host);
@@ -113,7 +146,7 @@ int lbm_get_populations(lbm_handle h, double* f);
 int lbm_set_populations(lbm_handle h, const double* f);
 
 /* Lattice tables in the library's order (HOST pointers): e[3*Q] as e[a*3 + d], t[Q].  `lattice`
- * is LBM_D3Q19 or LBM_D3Q27 (other bits ignored). */
+ * is LBM_D2Q9, LBM_D3Q19 or LBM_D3Q27 (other bits ignored). */
 int lbm_lattice(int lattice, int32_t* e, double* t);
 
 /* Number of time steps taken since the last lbm_init_equilibrium (or -1 for a NULL handle). */

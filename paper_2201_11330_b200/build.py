@@ -1,10 +1,13 @@
 """Build the CUDA library (csrc/*.cu -> paper_2201_11330_b200/liblbm_b200.so) for sm_100a.
 
-`python -m paper_2201_11330_b200.build [--force] [--verbose]`.  nvcc cross-compiles without a
-GPU.  The .so is built in-tree (git-ignored) so that it travels to the GPU box with the repo.
+`python -m paper_2201_11330_b200.build [--force] [--verbose] [--ptxas]`.  nvcc cross-compiles
+without a GPU.  The kernel instantiations (csrc/lbm_inst.cu) are compiled once per lattice and
+part into separate objects, in parallel, then linked with the C ABI (csrc/lbm_abi.cu).  The .so
+is built in-tree (git-ignored) so that it travels to the GPU box with the repo.
 """
 from __future__ import annotations
 
+import concurrent.futures as cf
 import os
 import shutil
 import subprocess
@@ -13,14 +16,16 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbm_b200.so")
-SOURCES = ["lbm_abi.cu"]
-DEPS = ["lbm_abi.cu", "lbm_kernels.cuh", os.path.join(ROOT, "include", "lbm.h")]
+DEPS = ["lbm_abi.cu", "lbm_inst.cu", "lbm_kernels.cuh", "lbm_launch.cuh", os.path.join(ROOT, "include", "lbm.h")]
+LATTICES = (9, 19, 27)
+PARTS = (0, 1, 2, 3, 4)  # A/B step, AA even, AA odd, export/import/init/geometry, moments/force
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo", "--fmad=true",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-diag-suppress", "177",
+    "-Xcompiler", "-fPIC", "-diag-suppress", "177",
 ]
 
 
@@ -42,13 +47,46 @@ def needs_build() -> bool:
     return False
 
 
+def _units():
+    """(object path, source, extra defines) of every translation unit."""
+    units = [(os.path.join(OBJ, "lbm_abi.o"), os.path.join(CSRC, "lbm_abi.cu"), [])]
+    for q in LATTICES:
+        for part in PARTS:
+            units.append((os.path.join(OBJ, f"lbm_inst_q{q}_p{part}.o"), os.path.join(CSRC, "lbm_inst.cu"),
+                          [f"-DLBM_Q={q}", f"-DLBM_PART={part}"]))
+    return units
+
+
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    nvcc = _nvcc()
+    os.makedirs(OBJ, exist_ok=True)
+    units = _units()
+
+    def compile_one(unit):
+        obj, src, defs = unit
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *defs, "-c", "-o", obj, src]
+        if verbose:
+            print(" ".join(cmd), file=sys.stderr)
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        return unit, r
+
+    # biggest units first (D3Q27 steps) so that the pool stays busy
+    order = sorted(units, key=lambda u: (("-DLBM_Q=27" in u[2]) * 2 + ("-DLBM_Q=19" in u[2])), reverse=True)
+    with cf.ThreadPoolExecutor(max_workers=max(1, min(len(units), os.cpu_count() or 1))) as pool:
+        results = list(pool.map(compile_one, order))
+    failed = False
+    for (obj, src, defs), r in results:
+        if r.returncode != 0 or (r.stderr.strip() and (verbose or extra)):
+            print(f"--- nvcc {' '.join(defs)} {os.path.basename(src)}\n{r.stdout}{r.stderr}", file=sys.stderr)
+        failed |= r.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed (see messages above)")
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-o", LIB] + [u[0] for u in units]
     if verbose:
-        print(" ".join(cmd), file=sys.stderr)
-    subprocess.run(cmd, check=True)
+        print(" ".join(link), file=sys.stderr)
+    subprocess.run(link, check=True)
     return LIB
 
 

@@ -7,7 +7,7 @@
 #include <string>
 
 #include "../../include/lbm.h"
-#include "lbm_kernels.cuh"
+#include "lbm_launch.cuh"
 
 using namespace lbm;
 
@@ -39,6 +39,12 @@ struct lbm_handle_s {
   double tau;
   Params p;
   bool walls, forced;
+  int wall_model;     // LBM_WALL_HALFWAY / LBM_WALL_NODAL (lbm_set_geometry)
+  bool has_geo;       // the BC_GEO kernels are in use (a solid mask and/or the nodal model was set)
+  uint8_t* geo;       // N, device: 1 = solid node
+  uint8_t* active;    // N, device: node takes part in collision and propagation (D:R16)
+  uint32_t* links;    // N, device: per-cell link mask read by the BC_GEO kernels
+  bool stepped;       // at least one step since the populations were last set (lbm_boundary_force)
   cudaStream_t stream;
   void* buf[2];       // A/B: both used, buf[cur] holds S^-1 f;  AA: buf[0] only
   int cur;
@@ -57,29 +63,15 @@ struct lbm_handle_s {
 
 namespace {
 
-// ---- dispatch over the compile-time variants ------------------------------------------
-// VARIANT(q, eq, walls, force) expands `body` with constexpr Q_, EQ_, WALLS_, FORCE_.
-#define LBM_DISPATCH_QEWF(h, BODY)                                                              \
-  do {                                                                                          \
-    const int key__ = ((h)->Q == 27 ? 8 : 0) | ((h)->eq ? 4 : 0) | ((h)->walls ? 2 : 0) | ((h)->forced ? 1 : 0); \
-    switch (key__) {                                                                            \
-      LBM_CASE(0, 19, 0, false, false, BODY) LBM_CASE(1, 19, 0, false, true, BODY)               \
-      LBM_CASE(2, 19, 0, true, false, BODY) LBM_CASE(3, 19, 0, true, true, BODY)                 \
-      LBM_CASE(4, 19, 1, false, false, BODY) LBM_CASE(5, 19, 1, false, true, BODY)               \
-      LBM_CASE(6, 19, 1, true, false, BODY) LBM_CASE(7, 19, 1, true, true, BODY)                 \
-      LBM_CASE(8, 27, 0, false, false, BODY) LBM_CASE(9, 27, 0, false, true, BODY)               \
-      LBM_CASE(10, 27, 0, true, false, BODY) LBM_CASE(11, 27, 0, true, true, BODY)               \
-      LBM_CASE(12, 27, 1, false, false, BODY) LBM_CASE(13, 27, 1, false, true, BODY)             \
-      LBM_CASE(14, 27, 1, true, false, BODY) LBM_CASE(15, 27, 1, true, true, BODY)               \
-    }                                                                                           \
+// Q dispatch: the per-lattice launchers live in lbm_inst.cu (one object per lattice and part).
+#define LBM_Q_CALL(h, fn, ...)                 \
+  do {                                         \
+    if ((h)->Q == 19) fn<19>(__VA_ARGS__);     \
+    else if ((h)->Q == 27) fn<27>(__VA_ARGS__); \
+    else fn<9>(__VA_ARGS__);                   \
   } while (0)
-#define LBM_CASE(k, q, e, w, f, BODY)  \
-  case k: {                            \
-    constexpr int Q_ = q, EQ_ = e;     \
-    constexpr bool WALLS_ = w, FORCE_ = f; \
-    (void)Q_; (void)EQ_; (void)WALLS_; (void)FORCE_; \
-    BODY;                              \
-  } break;
+
+Ctx make_ctx(const lbm_handle_s* h);
 
 // blocks of the row-wise sweeps (for_each_cell): 256/fbx rows per block, at most one wave
 int flat_grid(const lbm_handle_s* h) {
@@ -88,75 +80,43 @@ int flat_grid(const lbm_handle_s* h) {
   return (int)(b < kReduceBlocks ? b : kReduceBlocks);
 }
 
+Ctx make_ctx(const lbm_handle_s* h) {
+  Ctx c;
+  c.eq = h->eq ? EQ_INCOMP : EQ_STANDARD;
+  c.bc = h->has_geo ? BC_GEO : (h->walls ? BC_WALLS : BC_PERIODIC);
+  c.forced = h->forced;
+  c.f32 = h->f32;
+  c.block = dim3(h->bx, h->by, 1);
+  c.grid = dim3((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->nz);
+  c.flat_grid = flat_grid(h);
+  c.fbx = h->fbx;
+  c.stream = h->stream;
+  c.p = h->p;
+  return c;
+}
+
 // canonical-state read mode of the current storage state
 int read_mode(const lbm_handle_s* h) {
   if (h->scheme == LBM_SCHEME_AB) return MODE_PULL;
   return h->phase ? MODE_PULL_SWAP : MODE_NATURAL;
 }
 
-template <typename ST>
-int launch_step(lbm_handle_s* h) {
-  dim3 block(h->bx, h->by, 1);
-  dim3 grid((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->nz);
+void launch_step(lbm_handle_s* h, const Ctx& c) {
   if (h->scheme == LBM_SCHEME_AB) {
-    const ST* src = (const ST*)h->buf[h->cur];
-    ST* dst = (ST*)h->buf[h->cur ^ 1];
-    LBM_DISPATCH_QEWF(h, (stream_collide_ab<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(src, dst, h->p)));
+    LBM_Q_CALL(h, launch_step_ab, c, h->buf[h->cur], h->buf[h->cur ^ 1]);
     h->cur ^= 1;
   } else {
-    ST* b = (ST*)h->buf[0];
-    if (h->phase == 0)
-      LBM_DISPATCH_QEWF(h, (stream_collide_aa_even<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(b, h->p)));
-    else
-      LBM_DISPATCH_QEWF(h, (stream_collide_aa_odd<Q_, EQ_, WALLS_, FORCE_, ST><<<grid, block, 0, h->stream>>>(b, h->p)));
+    if (h->phase == 0) LBM_Q_CALL(h, launch_step_aa_even, c, h->buf[0]);
+    else LBM_Q_CALL(h, launch_step_aa_odd, c, h->buf[0]);
     h->phase ^= 1;
-  }
-  ++h->launches;
-  return LBM_OK;
-}
-
-template <typename ST>
-void launch_export(lbm_handle_s* h, double* out) {
-  const int g = flat_grid(h);
-  const ST* b = (const ST*)h->buf[h->cur];
-  switch (read_mode(h)) {
-    case MODE_NATURAL:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
-      break;
-    case MODE_PULL:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
-      break;
-    default:
-      LBM_DISPATCH_QEWF(h, (export_canonical<Q_, WALLS_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, out, h->fbx, h->p)));
   }
   ++h->launches;
 }
 
 // canonical fp64 array `in` -> storage buffer `dst_idx` in the layout the scheme wants at an even phase
-template <typename ST>
-void launch_import(lbm_handle_s* h, const double* in, int dst_idx) {
-  const int g = flat_grid(h);
-  ST* b = (ST*)h->buf[dst_idx];
-  if (h->scheme == LBM_SCHEME_AB)
-    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(in, b, h->fbx, h->p)));
-  else
-    LBM_DISPATCH_QEWF(h, (import_canonical<Q_, WALLS_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(in, b, h->fbx, h->p)));
-  ++h->launches;
-}
-
-template <typename ST>
-void launch_moments(lbm_handle_s* h, double* rho, double* u, double* partials, int g) {
-  const ST* b = (const ST*)h->buf[h->cur];
-  switch (read_mode(h)) {
-    case MODE_NATURAL:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_NATURAL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
-      break;
-    case MODE_PULL:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
-      break;
-    default:
-      LBM_DISPATCH_QEWF(h, (moments_kernel<Q_, EQ_, WALLS_, FORCE_, MODE_PULL_SWAP, ST><<<g, 256, 0, h->stream>>>(b, rho, u, partials, h->fbx, h->p)));
-  }
+void do_import(lbm_handle_s* h, const double* in, int dst_idx) {
+  const Ctx c = make_ctx(h);
+  LBM_Q_CALL(h, launch_import, c, h->scheme == LBM_SCHEME_AB ? MODE_PULL : MODE_NATURAL, in, h->buf[dst_idx]);
   ++h->launches;
 }
 
@@ -200,30 +160,24 @@ int do_init(lbm_handle_s* h, const double* rho, const double* u) {
   double* nat = nullptr;
   int rc = canonical_staging(h, &nat);
   if (rc) return rc;
-  const int g = flat_grid(h);
-  if (h->eq) {
-    if (h->Q == 19) init_equilibrium_kernel<19, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
-    else init_equilibrium_kernel<27, EQ_INCOMP><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
-  } else {
-    if (h->Q == 19) init_equilibrium_kernel<19, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
-    else init_equilibrium_kernel<27, EQ_STANDARD><<<g, 256, 0, h->stream>>>(rho, u, nat, h->fbx, h->p);
-  }
+  const Ctx c = make_ctx(h);
+  LBM_Q_CALL(h, launch_init, c, rho, u, nat);
   ++h->launches;
   if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
-  if (h->f32) launch_import<float>(h, nat, h->cur);
-  else launch_import<double>(h, nat, h->cur);
+  do_import(h, nat, h->cur);
   h->phase = 0;
   h->time = 0;
+  h->stepped = false;
   return check_launch("init_equilibrium");
 }
 
 int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
-  const int g = flat_grid(h);
+  const Ctx c = make_ctx(h);
   double* partials = diagnostics ? h->partials : nullptr;
-  if (h->f32) launch_moments<float>(h, rho, u, partials, g);
-  else launch_moments<double>(h, rho, u, partials, g);
+  LBM_Q_CALL(h, launch_moments, c, read_mode(h), h->buf[h->cur], rho, u, partials);
+  ++h->launches;
   if (diagnostics) {
-    reduce_final_kernel<<<1, 256, 0, h->stream>>>(h->partials, g, h->diag_dev);
+    reduce_final_kernel<><<<1, 256, 0, h->stream>>>(h->partials, c.flat_grid, h->diag_dev);
     ++h->launches;
   }
   int rc = check_launch("moments");
@@ -236,6 +190,58 @@ int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
   return LBM_OK;
 }
 
+void free_geometry(lbm_handle_s* h) {
+  if (h->geo) cudaFree(h->geo);
+  if (h->active) cudaFree(h->active);
+  if (h->links) cudaFree(h->links);
+  h->geo = h->active = nullptr;
+  h->links = nullptr;
+  h->has_geo = false;
+  h->wall_model = LBM_WALL_HALFWAY;
+  h->p.links = nullptr;
+  h->p.nodal = 0;
+}
+
+int alloc_geometry(lbm_handle_s* h) {
+  if (h->geo) return LBM_OK;
+  cudaError_t e = cudaMalloc((void**)&h->geo, (size_t)h->N);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->active, (size_t)h->N);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->links, (size_t)h->N * sizeof(uint32_t));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    free_geometry(h);
+    return fail(LBM_ENOMEM, "lbm_set_geometry: out of device memory for the geometry arrays");
+  }
+  return LBM_OK;
+}
+
+// geo_dev: device pointer to N bytes (must not alias h->geo or h->active), or NULL (all fluid)
+int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
+  if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
+    return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
+  if (wall_model == LBM_WALL_NODAL && h->p.any_moving)
+    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING faces is not supported");
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (!geo_dev && wall_model == LBM_WALL_HALFWAY) {  // back to the analytic box
+    free_geometry(h);
+    return LBM_OK;
+  }
+  {
+    int rc = alloc_geometry(h);
+    if (rc) return rc;
+  }
+  h->wall_model = wall_model;
+  h->has_geo = true;
+  h->p.links = h->links;
+  h->p.nodal = wall_model == LBM_WALL_NODAL;
+  const Ctx c = make_ctx(h);
+  // the kernels read the caller's mask directly (no runtime memcpy on a pointer the library does not own)
+  LBM_Q_CALL(h, launch_geometry, c, geo_dev, h->geo, h->active, h->links, h->p.nodal);
+  h->launches += 2;
+  h->stepped = false;
+  return check_launch("lbm_set_geometry");
+}
+
 }  // namespace
 
 // =========================================================================================
@@ -246,34 +252,27 @@ const char* lbm_last_error(void) { return g_err.c_str(); }
 int lbm_lattice(int lattice, int32_t* e, double* t) {
   const int Q = lattice & 0xff;
   if (!e || !t) return fail(LBM_EINVAL, "lbm_lattice: NULL output");
-  if (Q == 19) {
-    for (int a = 0; a < 19; ++a) {
+  auto fill = [&](auto L, int q) {
+    using Lt = decltype(L);
+    for (int a = 0; a < q; ++a) {
       int s = 0;
       for (int d = 0; d < 3; ++d) {
-        e[3 * a + d] = Lattice<19>::e[a][d];
+        e[3 * a + d] = Lt::e[a][d];
         s += e[3 * a + d] * e[3 * a + d];
       }
-      t[a] = s == 0 ? Lattice<19>::w0 : s == 1 ? Lattice<19>::w1 : Lattice<19>::w2;
+      t[a] = s == 0 ? Lt::w0 : s == 1 ? Lt::w1 : s == 2 ? Lt::w2 : Lt::w3;
     }
-    return LBM_OK;
-  }
-  if (Q == 27) {
-    for (int a = 0; a < 27; ++a) {
-      int s = 0;
-      for (int d = 0; d < 3; ++d) {
-        e[3 * a + d] = Lattice<27>::e[a][d];
-        s += e[3 * a + d] * e[3 * a + d];
-      }
-      t[a] = s == 0 ? Lattice<27>::w0 : s == 1 ? Lattice<27>::w1 : s == 2 ? Lattice<27>::w2 : Lattice<27>::w3;
-    }
-    return LBM_OK;
-  }
-  return fail(LBM_EINVAL, "lbm_lattice: lattice must be LBM_D3Q19 or LBM_D3Q27");
+  };
+  if (Q == 9) fill(Lattice<9>{}, 9);
+  else if (Q == 19) fill(Lattice<19>{}, 19);
+  else if (Q == 27) fill(Lattice<27>{}, 27);
+  else return fail(LBM_EINVAL, "lbm_lattice: lattice must be LBM_D2Q9, LBM_D3Q19 or LBM_D3Q27");
+  return LBM_OK;
 }
 
 lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm_bc_t* bc) {
   const int Q = lattice & 0xff;
-  if (Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
+  if (Q != 9 && Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D2Q9, LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
   if (nx < 1 || ny < 1 || nz < 1) { fail(LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1"); return nullptr; }
   if ((long long)nx * ny * nz >= (1LL << 31)) { fail(LBM_EUNSUPPORTED, "lbm_create: nx*ny*nz must be < 2^31 (in-plane offsets are 32-bit)"); return nullptr; }
   if (nz > 65535 || ny > 65535) { fail(LBM_EINVAL, "lbm_create: ny or nz exceeds the launch grid limits"); return nullptr; }
@@ -350,8 +349,48 @@ void lbm_destroy(lbm_handle h) {
   if (h->diag_dev) cudaFree(h->diag_dev);
   if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
   if (h->scratch) cudaFree(h->scratch);
+  free_geometry(h);
   cudaGetLastError();
   delete h;
+}
+
+int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model) {
+  if (!h) return fail(LBM_EINVAL, "lbm_set_geometry: NULL handle");
+  return do_set_geometry(h, geo, wall_model);
+}
+
+int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model) {
+  if (!h) return fail(LBM_EINVAL, "lbm_set_geometry_host: NULL handle");
+  if (!geo_host) return do_set_geometry(h, nullptr, wall_model);
+  if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
+    return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
+  if (wall_model == LBM_WALL_NODAL && h->p.any_moving)
+    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING faces is not supported");
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  {
+    int rc = alloc_geometry(h);
+    if (rc) return rc;
+  }
+  // stage the host mask in the link-mask array (4N bytes, rebuilt last by do_set_geometry)
+  uint8_t* stage = (uint8_t*)h->links + (size_t)h->N * 3;
+  CUDA_TRY(cudaMemcpyAsync(stage, geo_host, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+  return do_set_geometry(h, stage, wall_model);
+}
+
+int lbm_boundary_force(lbm_handle h, double* F) {
+  if (!h || !F) return fail(LBM_EINVAL, "lbm_boundary_force: NULL argument");
+  if (!h->has_geo) return fail(LBM_EINVAL, "lbm_boundary_force: no geometry set (lbm_set_geometry)");
+  if (!h->stepped) return fail(LBM_EINVAL, "lbm_boundary_force: defined only after at least one lbm_step since the populations were set");
+  const Ctx c = make_ctx(h);
+  LBM_Q_CALL(h, launch_boundary_force, c, read_mode(h), h->buf[h->cur], h->geo, h->partials);
+  reduce_final_kernel<><<<1, 256, 0, h->stream>>>(h->partials, c.flat_grid, h->diag_dev);
+  h->launches += 2;
+  int rc = check_launch("lbm_boundary_force");
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(h->diag_pinned, h->diag_dev, kDiag * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  for (int d = 0; d < 3; ++d) F[d] = h->diag_pinned[d];
+  return LBM_OK;
 }
 
 int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u) {
@@ -389,12 +428,14 @@ int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double
 int lbm_step(lbm_handle h, int nsteps) {
   if (!h) return fail(LBM_EINVAL, "lbm_step: NULL handle");
   if (nsteps < 0) return fail(LBM_EINVAL, "lbm_step: nsteps must be >= 0");
+  if (nsteps == 0) return LBM_OK;
+  const Ctx c = make_ctx(h);
   for (int s = 0; s < nsteps; ++s) {
-    if (h->f32) launch_step<float>(h);
-    else launch_step<double>(h);
+    launch_step(h, c);
     ++h->time;
   }
-  return nsteps ? check_launch("lbm_step") : LBM_OK;
+  h->stepped = true;
+  return check_launch("lbm_step");
 }
 
 int lbm_moments(lbm_handle h, double* rho, double* u, double* diagnostics) {
@@ -428,17 +469,18 @@ int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* dia
 
 int lbm_get_populations(lbm_handle h, double* f) {
   if (!h || !f) return fail(LBM_EINVAL, "lbm_get_populations: NULL argument");
-  if (h->f32) launch_export<float>(h, f);
-  else launch_export<double>(h, f);
+  const Ctx c = make_ctx(h);
+  LBM_Q_CALL(h, launch_export, c, read_mode(h), h->buf[h->cur], f);
+  ++h->launches;
   return check_launch("lbm_get_populations");
 }
 
 int lbm_set_populations(lbm_handle h, const double* f) {
   if (!h || !f) return fail(LBM_EINVAL, "lbm_set_populations: NULL argument");
   if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
-  if (h->f32) launch_import<float>(h, f, h->cur);
-  else launch_import<double>(h, f, h->cur);
+  do_import(h, f, h->cur);
   h->phase = 0;
+  h->stepped = false;
   return check_launch("lbm_set_populations");
 }
 

@@ -1,0 +1,149 @@
+// lbm_inst.cu — kernel instantiations.  Compiled once per (LBM_Q, LBM_PART) by build.py, in parallel:
+//   LBM_Q    9 | 19 | 27
+//   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
+// Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
+#include "lbm_launch.cuh"
+
+#ifndef LBM_Q
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..4"
+#endif
+
+namespace lbm {
+namespace {
+
+// Runtime flags -> compile-time variant: f(IC<EQ>, IC<BC>, IC<FORCE>, storage type tag).
+template <typename F>
+void dispatch_storage(const Ctx& c, F&& f) {
+  if (c.f32) f(float{});
+  else f(double{});
+}
+template <typename F>
+void dispatch_bc(const Ctx& c, F&& f) {
+  switch (c.bc) {
+    case BC_PERIODIC: f(IC<BC_PERIODIC>{}); break;
+    case BC_WALLS: f(IC<BC_WALLS>{}); break;
+    default: f(IC<BC_GEO>{}); break;
+  }
+}
+template <typename F>
+void dispatch_eq(const Ctx& c, F&& f) {
+  if (c.eq) f(IC<EQ_INCOMP>{});
+  else f(IC<EQ_STANDARD>{});
+}
+template <typename F>
+void dispatch_force(const Ctx& c, F&& f) {
+  if (c.forced) f(IC<1>{});
+  else f(IC<0>{});
+}
+template <typename F>
+void dispatch_step(const Ctx& c, F&& f) {
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_bc(c, [&](auto bc) {
+      dispatch_force(c, [&](auto force) { dispatch_storage(c, [&](auto st) { f(eq, bc, force, st); }); });
+    });
+  });
+}
+template <typename F>
+void dispatch_mode(int mode, F&& f) {
+  switch (mode) {
+    case MODE_NATURAL: f(IC<MODE_NATURAL>{}); break;
+    case MODE_PULL: f(IC<MODE_PULL>{}); break;
+    default: f(IC<MODE_PULL_SWAP>{}); break;
+  }
+}
+
+}  // namespace
+
+constexpr int Q_ = LBM_Q;
+
+#if LBM_PART == 0
+template <>
+void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    stream_collide_ab<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
+        <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+  });
+}
+#elif LBM_PART == 1
+template <>
+void launch_step_aa_even<Q_>(const Ctx& c, void* buf) {
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    stream_collide_aa_even<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
+        <<<c.grid, c.block, 0, c.stream>>>((ST*)buf, c.p);
+  });
+}
+#elif LBM_PART == 2
+template <>
+void launch_step_aa_odd<Q_>(const Ctx& c, void* buf) {
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    stream_collide_aa_odd<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
+        <<<c.grid, c.block, 0, c.stream>>>((ST*)buf, c.p);
+  });
+}
+#elif LBM_PART == 3
+template <>
+void launch_export<Q_>(const Ctx& c, int mode, const void* buf, double* out) {
+  dispatch_mode(mode, [&](auto m) {
+    dispatch_bc(c, [&](auto bc) {
+      dispatch_storage(c, [&](auto st) {
+        using ST = decltype(st);
+        export_canonical<Q_, decltype(bc)::value, decltype(m)::value, ST><<<c.flat_grid, 256, 0, c.stream>>>((const ST*)buf, out, c.fbx, c.p);
+      });
+    });
+  });
+}
+template <>
+void launch_import<Q_>(const Ctx& c, int mode, const double* in, void* buf) {
+  dispatch_bc(c, [&](auto bc) {
+    dispatch_storage(c, [&](auto st) {
+      using ST = decltype(st);
+      if (mode == MODE_PULL)
+        import_canonical<Q_, decltype(bc)::value, MODE_PULL, ST><<<c.flat_grid, 256, 0, c.stream>>>(in, (ST*)buf, c.fbx, c.p);
+      else
+        import_canonical<Q_, decltype(bc)::value, MODE_NATURAL, ST><<<c.flat_grid, 256, 0, c.stream>>>(in, (ST*)buf, c.fbx, c.p);
+    });
+  });
+}
+template <>
+void launch_init<Q_>(const Ctx& c, const double* rho, const double* u, double* out) {
+  dispatch_eq(c, [&](auto eq) {
+    init_equilibrium_kernel<Q_, decltype(eq)::value><<<c.flat_grid, 256, 0, c.stream>>>(rho, u, out, c.fbx, c.p);
+  });
+}
+template <>
+void launch_geometry<Q_>(const Ctx& c, const uint8_t* geo_in, uint8_t* geo, uint8_t* active, uint32_t* links, int nodal) {
+  classify_nodes_kernel<Q_><<<c.flat_grid, 256, 0, c.stream>>>(geo_in, geo, active, nodal, c.fbx, c.p);
+  build_links_kernel<Q_><<<c.flat_grid, 256, 0, c.stream>>>(active, links, c.fbx, c.p);
+}
+#elif LBM_PART == 4
+template <>
+void launch_moments<Q_>(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials) {
+  dispatch_mode(mode, [&](auto m) {
+    dispatch_eq(c, [&](auto eq) {
+      dispatch_bc(c, [&](auto bc) {
+        dispatch_storage(c, [&](auto st) {
+          using ST = decltype(st);
+          moments_kernel<Q_, decltype(eq)::value, decltype(bc)::value, decltype(m)::value, ST>
+              <<<c.flat_grid, 256, 0, c.stream>>>((const ST*)buf, rho, u, partials, c.fbx, c.p);
+        });
+      });
+    });
+  });
+}
+template <>
+void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const uint8_t* geo, double* partials) {
+  dispatch_mode(mode, [&](auto m) {
+    dispatch_storage(c, [&](auto st) {
+      using ST = decltype(st);
+      boundary_force_kernel<Q_, decltype(m)::value, ST><<<c.flat_grid, 256, 0, c.stream>>>((const ST*)buf, geo, partials, c.fbx, c.p);
+    });
+  });
+}
+#else
+#error "LBM_PART must be 0..4"
+#endif
+
+}  // namespace lbm

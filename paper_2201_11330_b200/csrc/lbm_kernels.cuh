@@ -15,6 +15,14 @@ namespace lbm {
 template <int Q>
 struct Lattice;
 
+// D2Q9 exactly as printed in the paper (Eq. 3-4), embedded with e_z = 0.
+template <>
+struct Lattice<9> {
+  static constexpr int e[9][3] = {{-1, -1, 0}, {-1, 0, 0}, {-1, 1, 0}, {0, -1, 0}, {0, 0, 0},
+                                  {0, 1, 0},   {1, -1, 0}, {1, 0, 0},  {1, 1, 0}};
+  static constexpr double w0 = 4.0 / 9.0, w1 = 1.0 / 9.0, w2 = 1.0 / 36.0, w3 = 0.0;
+};
+
 template <>
 struct Lattice<19> {
   static constexpr int e[19][3] = {
@@ -59,9 +67,16 @@ __device__ __forceinline__ void static_for(F&& f) {
 // (the fp32-storage variant loses 15 % of its bandwidth at two); the forced and in-place variants
 // and D3Q27 spill below 128.
 template <int Q, bool FORCE, bool INPLACE>
-constexpr int kMinBlocks = (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
+constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
 
 // ---------------------------------------------------------------------------------------
+// How a cell finds out that a link has no upstream node (template parameter BC):
+//   BC_PERIODIC  never                                           (no test at all)
+//   BC_WALLS     coordinate tests against the non-periodic faces (0 B/cell)
+//   BC_GEO       one 32-bit link mask per cell, built once by build_links_kernel from the
+//                solid mask `geo` and the faces           (4 B/cell read per step)
+enum { BC_PERIODIC = 0, BC_WALLS = 1, BC_GEO = 2 };
+
 struct Params {
   int nx, ny, nz;
   long long N;          // cells = plane stride of the SoA layout (64-bit: 512^3*19 > 2^31)
@@ -71,16 +86,21 @@ struct Params {
   int moving[6];        // face is MOVING
   double face_u[6][3];  // wall velocity of MOVING faces
   int any_moving;
+  // BC_GEO only (D:R16): bit a (a != rest) of links[i]: node i - e_a is not an active node (solid,
+  // or beyond a non-periodic face); bit `rest`: node i itself is inactive.
+  const uint32_t* links;
+  int nodal;            // D:R3/R17: the paper's modified nodal bounce-back (Eq. 10) instead of halfway
 };
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
 
-// Position of a cell relative to the non-periodic faces.
-template <bool WALLS>
+// Position of a cell relative to the non-periodic faces, and (BC_GEO) its link mask.
+template <int BC>
 struct CellFlags {
   bool lo[3], hi[3];  // cell is in the first / last plane of an axis whose face there is a wall
-  __device__ __forceinline__ CellFlags(const Params& p, int x, int y, int z) {
-    if constexpr (WALLS) {
+  uint32_t m;
+  __device__ __forceinline__ CellFlags(const Params& p, int x, int y, int z, int ic) {
+    if constexpr (BC != BC_PERIODIC) {
       lo[0] = (x == 0) & (p.wall[0] != 0);
       hi[0] = (x == p.nx - 1) & (p.wall[1] != 0);
       lo[1] = (y == 0) & (p.wall[2] != 0);
@@ -90,11 +110,13 @@ struct CellFlags {
     } else {
       lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
     }
+    if constexpr (BC == BC_GEO) m = __ldg(p.links + ic);
+    else m = 0u;
   }
   // true if the node x + s*e_A lies outside the box (s = +1: downstream, s = -1: upstream)
   template <int Q, int A, int S>
-  __device__ __forceinline__ bool leaves() const {
-    if constexpr (!WALLS) return false;
+  __device__ __forceinline__ bool leaves_box() const {
+    if constexpr (BC == BC_PERIODIC) return false;
     constexpr int dx = S * Dir<Q, A>::ex, dy = S * Dir<Q, A>::ey, dz = S * Dir<Q, A>::ez;
     // bitwise OR on purpose: a short-circuit || makes ptxas branch around the loads it guards
     bool out = false;
@@ -105,6 +127,22 @@ struct CellFlags {
     if constexpr (dz == -1) out = out | lo[2];
     if constexpr (dz == 1) out = out | hi[2];
     return out;
+  }
+  // true if there is no active node at x + s*e_A (beyond a wall face, or — BC_GEO — solid)
+  template <int Q, int A, int S>
+  __device__ __forceinline__ bool leaves() const {
+    if constexpr (Dir<Q, A>::s == 0) return false;
+    if constexpr (BC == BC_GEO) {
+      constexpr int bit = (S == -1) ? A : Dir<Q, A>::opp;  // x + e_A = x - e_opp(A)
+      return (m >> bit) & 1u;
+    } else {
+      return leaves_box<Q, A, S>();
+    }
+  }
+  template <int Q>
+  __device__ __forceinline__ bool active() const {
+    if constexpr (BC == BC_GEO) return !((m >> ((Q - 1) / 2)) & 1u);
+    return true;
   }
 };
 
@@ -228,8 +266,8 @@ __device__ __forceinline__ void equilibrium(double (&feq)[Q], double rho, double
 // (D:R6): the value kept for an outgoing link b is f*_b - 6 t_b rho_w (e_b . u_w), which the
 // bounce-back read f_bbar(x, t+1) = stored_b(x) turns into f*_b + 6 t_bbar rho_w (e_bbar . u_w).
 // f is replaced by the post-collision populations.
-template <int Q, int EQ, bool WALLS, bool FORCE>
-__device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const CellFlags<WALLS>& c) {
+template <int Q, int EQ, int BC, bool FORCE>
+__device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const CellFlags<BC>& c) {
   double rho, ux, uy, uz;
   moments<Q, EQ, FORCE>(f, p, rho, ux, uy, uz);
   const double om = p.omega, om1 = 1.0 - p.omega;
@@ -261,7 +299,7 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
       f[D::opp] = fma(om1, f[D::opp], s - d);
     }
   });
-  if constexpr (WALLS) {
+  if constexpr (BC != BC_PERIODIC) {
     if (p.any_moving) {
       // moving face crossed by a link leaving along +e on axis d: hi face (2d+1); along -e: lo face (2d)
       const bool touch = (c.lo[0] && p.moving[0]) || (c.hi[0] && p.moving[1]) || (c.lo[1] && p.moving[2]) ||
@@ -297,29 +335,51 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
   }
 }
 
+// Eq. 10 of the paper's modified nodal bounce-back (D:R17), applied to the populations a
+// wall node has just gathered: a direction a nothing streamed in along (link bit a set) takes the
+// value that arrived along its opposite, f_a = f_abar, if abar did arrive from an active node (bit
+// abar clear).  When neither end of the link is active the halfway value already in f[a] stays.
+template <int Q, int BC>
+__device__ __forceinline__ void nodal_replicate(double (&f)[Q], const Params& p, const CellFlags<BC>& c) {
+  if constexpr (BC == BC_GEO) {
+    if (p.nodal && (c.m != 0u)) {
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        constexpr int o = Dir<Q, a>::opp;
+        if constexpr (a != o) {
+          // each +- pair is touched at most once: the condition excludes its mirror image
+          if (((c.m >> a) & 1u) && !((c.m >> o) & 1u)) f[a] = f[o];
+        }
+      });
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------
-// A/B scheme ("stream on read").  The buffer holds B = S^-1 f, S the slot permutation of one
-// propagation (Eq. 7 with wall links, Eq. 10):  f_a(x) = B_a(x - e_a)  inside,  = B_abar(x)  at a wall
-// link.  One step = pull (gives the canonical pre-collision f of this time level), collide,
-// store aligned at the own cell into the other buffer (which is again S^-1 of the next f).
-template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+// A/B scheme ("stream on read").  The buffer holds the post-collision populations aligned at their
+// own cell, B = S^-1 f, S the slot permutation of one propagation (Eq. 7 with wall links, Eq. 10):
+// f_a(x) = B_a(x - e_a)  inside,  = B_abar(x)  at a wall link.  One step = pull (gives the canonical
+// pre-collision f of this time level), collide, store aligned at the own cell into the other buffer.
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
 __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
-  const CellFlags<WALLS> c(p, x, y, z);
+  const CellFlags<BC> c(p, x, y, z, nb.ic);
+  if (!c.template active<Q>()) return;  // solid interior: no traffic at all
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     const ST* q = plane<a>(src, p.N) + nb.template at<Q, a, -1>();
-    if constexpr (WALLS) {
+    if constexpr (BC != BC_PERIODIC) {
       if (c.template leaves<Q, a, -1>()) q = plane<Dir<Q, a>::opp>(src, p.N) + nb.ic;  // a select, not a branch
     }
     f[a] = ld_pop<ST, Q, a>(q, 0);  // t_a == t_abar: one load serves both cases
   });
-  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  nodal_replicate<Q, BC>(f, p, c);
+  collide<Q, EQ, BC, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
@@ -332,51 +392,55 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false>) stream_colli
 // after which the buffer is in natural layout again.  Each thread reads and writes exactly its
 // own set of Q slots (the odd phase writes f*_a where it read f_abar), so there is no
 // inter-thread hazard in either phase.
-template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
 __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_even(ST* buf, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   const int ic = x + p.nx * (y + p.ny * z);
-  const CellFlags<WALLS> c(p, x, y, z);
+  const CellFlags<BC> c(p, x, y, z, ic);
+  if (!c.template active<Q>()) return;
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), ic);
   });
-  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  nodal_replicate<Q, BC>(f, p, c);
+  collide<Q, EQ, BC, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     st_pop<ST, Q, a>(plane<Dir<Q, a>::opp>(buf, p.N), ic, f[a]);
   });
 }
 
-template <int Q, int EQ, bool WALLS, bool FORCE, typename ST>
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
 __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_odd(ST* buf, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
-  const CellFlags<WALLS> c(p, x, y, z);
+  const CellFlags<BC> c(p, x, y, z, nb.ic);
+  if (!c.template active<Q>()) return;
   double f[Q];
   // f_a(x) comes from the slot that f*_abar(x) goes to (link x <-> x - e_a traversed both ways)
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
     const ST* q = plane<o>(buf, p.N) + nb.template at<Q, a, -1>();
-    if constexpr (WALLS) {
+    if constexpr (BC != BC_PERIODIC) {
       if (c.template leaves<Q, a, -1>()) q = plane<a>(buf, p.N) + nb.ic;
     }
     f[a] = ld_pop_rw<ST, Q, a>(q, 0);
   });
-  collide<Q, EQ, WALLS, FORCE>(f, p, c);
+  nodal_replicate<Q, BC>(f, p, c);
+  collide<Q, EQ, BC, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
     ST* q = plane<a>(buf, p.N) + nb.template at<Q, a, 1>();
-    if constexpr (WALLS) {
+    if constexpr (BC != BC_PERIODIC) {
       if (c.template leaves<Q, a, 1>()) q = plane<o>(buf, p.N) + nb.ic;
     }
     st_pop<ST, Q, a>(q, 0, f[a]);
@@ -388,12 +452,11 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
 //   NATURAL   : f_a(x) = slot(x, a)                                   (AA, even phase)
 //   PULL      : f_a(x) = slot(x - e_a, a),   wall link: slot(x, abar)   (A/B)
 //   PULL_SWAP : f_a(x) = slot(x - e_a, abar), wall link: slot(x, a)      (AA, odd phase)
+// followed by Eq. 10 on wall nodes under the nodal model.
 enum { MODE_NATURAL = 0, MODE_PULL = 1, MODE_PULL_SWAP = 2 };
 
-template <int Q, bool WALLS, int MODE, typename ST>
-__device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, const Params& p, int x, int y, int z) {
-  const Neigh nb(p, x, y, z);
-  const CellFlags<WALLS> c(p, x, y, z);
+template <int Q, int BC, int MODE, typename ST>
+__device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, const Params& p, const Neigh& nb, const CellFlags<BC>& c) {
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
@@ -403,12 +466,13 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
     } else {
       constexpr int q_in = (MODE == MODE_PULL) ? a : o, q_wall = (MODE == MODE_PULL) ? o : a;
       q = plane<q_in>(buf, p.N) + nb.template at<Q, a, -1>();
-      if constexpr (WALLS) {
+      if constexpr (BC != BC_PERIODIC) {
         if (c.template leaves<Q, a, -1>()) q = plane<q_wall>(buf, p.N) + nb.ic;
       }
     }
     f[a] = ld_pop_rw<ST, Q, a>(q, 0);
   });
+  nodal_replicate<Q, BC>(f, p, c);
 }
 
 // Row-wise grid-stride loop of the sweeps off the per-step path: a 256-thread block is bx x (256/bx)
@@ -424,12 +488,18 @@ __device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body)
   }
 }
 
-// lbm_get_populations: canonical f[a*N+i] (always fp64) out of the storage buffer.
-template <int Q, bool WALLS, int MODE, typename ST>
+// lbm_get_populations: canonical f[a*N+i] (always fp64) out of the storage buffer; inactive nodes report 0.
+template <int Q, int BC, int MODE, typename ST>
 __global__ void __launch_bounds__(256, 2) export_canonical(const ST* buf, double* __restrict__ out, int bx, const __grid_constant__ Params p) {
   for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+    const Neigh nb(p, x, y, z);
+    const CellFlags<BC> c(p, x, y, z, i);
     double f[Q];
-    load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
+    if (c.template active<Q>()) {
+      load_canonical<Q, BC, MODE, ST>(f, buf, p, nb, c);
+    } else {
+      static_for<0, Q>([&](auto A) { f[decltype(A)::value] = 0.0; });
+    }
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       plane<a>(out, p.N)[i] = f[a];
@@ -438,20 +508,21 @@ __global__ void __launch_bounds__(256, 2) export_canonical(const ST* buf, double
 }
 
 // lbm_set_populations / init: canonical f[a*N+i] (fp64) into the storage buffer.
-//   NATURAL: slot(x,a) = f_a(x).   PULL (A/B): slot(y,a) = f_a(y + e_a) inside, = f_abar(y) if y + e_a is outside.
-template <int Q, bool WALLS, int MODE, typename ST>
+//   NATURAL: slot(x,a) = f_a(x).   PULL (A/B): slot(y,a) = f_a(y + e_a) if y + e_a is an active node, else f_abar(y).
+template <int Q, int BC, int MODE, typename ST>
 __global__ void __launch_bounds__(256) import_canonical(const double* __restrict__ in, ST* __restrict__ buf, int bx, const __grid_constant__ Params p) {
   static_assert(MODE != MODE_PULL_SWAP, "imports always land in an even phase");
   for_each_cell(p, bx, [&](int x, int y, int z, int i) {
     const Neigh nb(p, x, y, z);
-    const CellFlags<WALLS> c(p, x, y, z);
+    const CellFlags<BC> c(p, x, y, z, i);
+    if (!c.template active<Q>()) return;
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       constexpr int o = Dir<Q, a>::opp;
       const double* q = plane<a>(in, p.N) + i;
       if constexpr (MODE != MODE_NATURAL) {
         q = plane<a>(in, p.N) + nb.template at<Q, a, 1>();
-        if constexpr (WALLS) {
+        if constexpr (BC != BC_PERIODIC) {
           if (c.template leaves<Q, a, 1>()) q = plane<o>(in, p.N) + i;
         }
       }
@@ -472,6 +543,51 @@ __global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __r
       constexpr int a = decltype(A)::value;
       plane<a>(out, p.N)[i] = feq[a];
     });
+  });
+}
+
+// ---------------------------------------------------------------------------------------
+// SetGeometry (D:R16).  classify: a node is active if it is fluid (geo = 0) or — nodal
+// model — a solid node with at least one fluid node among its lattice neighbours (the wall nodes
+// Eq. 10 and the collision act on).  links: the per-cell mask the BC_GEO kernels read.
+template <int Q>
+__global__ void __launch_bounds__(256) classify_nodes_kernel(const uint8_t* __restrict__ geo_in, uint8_t* __restrict__ geo, uint8_t* __restrict__ active,
+                                                             int nodal, int bx, const __grid_constant__ Params p) {
+  // geo_in: the caller's mask (any device-readable memory; NULL = no solid nodes); geo: the library's 0/1 copy
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+    const bool solid = geo_in ? geo_in[i] != 0 : false;
+    bool a = !solid;
+    if (solid && nodal) {
+      const Neigh nb(p, x, y, z);
+      const CellFlags<BC_WALLS> c(p, x, y, z, i);
+      static_for<0, Q>([&](auto A) {
+        constexpr int b = decltype(A)::value;
+        if constexpr (Dir<Q, b>::s > 0) {
+          if (!c.template leaves_box<Q, b, 1>()) a = a | (geo_in[nb.template at<Q, b, 1>()] == 0);
+        }
+      });
+    }
+    geo[i] = solid ? 1 : 0;
+    active[i] = a ? 1 : 0;
+  });
+}
+
+template <int Q>
+__global__ void __launch_bounds__(256) build_links_kernel(const uint8_t* __restrict__ active, uint32_t* __restrict__ links, int bx,
+                                                          const __grid_constant__ Params p) {
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+    const Neigh nb(p, x, y, z);
+    const CellFlags<BC_WALLS> c(p, x, y, z, i);
+    uint32_t m = active[i] ? 0u : (1u << ((Q - 1) / 2));
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      if constexpr (Dir<Q, a>::s > 0) {
+        bool none = c.template leaves_box<Q, a, -1>();
+        if (!none) none = active[nb.template at<Q, a, -1>()] == 0;
+        m |= none ? (1u << a) : 0u;
+      }
+    });
+    links[i] = m;
   });
 }
 
@@ -523,15 +639,27 @@ __device__ __forceinline__ void block_reduce_diag(double (&acc)[kDiag], double* 
   }
 }
 
-template <int Q, int EQ, bool WALLS, bool FORCE, int MODE, typename ST>
+// The F/2 shift of D:R7 is always applied (adding 0.5*0 is exact), so there is no FORCE variant here.
+template <int Q, int EQ, int BC, int MODE, typename ST>
 __global__ void __launch_bounds__(256, 2) moments_kernel(const ST* buf, double* __restrict__ rho_out, double* __restrict__ u_out,
                                                       double* __restrict__ partials, int bx, const __grid_constant__ Params p) {
   double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
   for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+    const Neigh nb(p, x, y, z);
+    const CellFlags<BC> c(p, x, y, z, i);
+    if (!c.template active<Q>()) {  // Monitor runs over the fluid nodes; inactive nodes report 0
+      if (rho_out) rho_out[i] = 0.0;
+      if (u_out) {
+        u_out[i] = 0.0;
+        plane<1>(u_out, p.N)[i] = 0.0;
+        plane<2>(u_out, p.N)[i] = 0.0;
+      }
+      return;
+    }
     double f[Q];
-    load_canonical<Q, WALLS, MODE, ST>(f, buf, p, x, y, z);
+    load_canonical<Q, BC, MODE, ST>(f, buf, p, nb, c);
     double rho, ux, uy, uz;
-    moments<Q, EQ, FORCE>(f, p, rho, ux, uy, uz);
+    moments<Q, EQ, true>(f, p, rho, ux, uy, uz);
     if (rho_out) rho_out[i] = rho;
     if (u_out) {
       u_out[i] = ux;
@@ -555,6 +683,8 @@ __global__ void __launch_bounds__(256, 2) moments_kernel(const ST* buf, double* 
   if (partials) block_reduce_diag(acc, partials + (long long)blockIdx.x * kDiag);
 }
 
+// (a template only so that the definition may live in this header, which several units include)
+template <int K = kDiag>
 __global__ void __launch_bounds__(256) reduce_final_kernel(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
   double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
   for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
@@ -564,6 +694,58 @@ __global__ void __launch_bounds__(256) reduce_final_kernel(const double* __restr
     diag_combine(acc, v);
   }
   block_reduce_diag(acc, out);
+}
+
+// Momentum-exchange force on the solid nodes of `geo` (Eq. 13) for the step just taken:
+//   F = sum over fluid nodes x (geo = 0), sum over a with x + e_a a solid node of geo (inside the box):
+//       [ f*_a(x, t) + f_abar(x, t + dt) ] e_a
+// f_abar(x, t+dt) is the canonical state; the post-collision f*_a(x, t) is still in the storage:
+//   A/B                : slot(x, a) of the current buffer
+//   AA after even step : slot(x, abar)
+//   AA after odd step  : slot(x + e_a, a) if x + e_a is active (a nodal wall node), else slot(x, abar)
+// partials[b*8 + 0..2] receive the block sums (slots 3..7 stay neutral).
+template <int Q, int MODE, typename ST>
+__global__ void __launch_bounds__(256, 2) boundary_force_kernel(const ST* buf, const uint8_t* __restrict__ geo, double* __restrict__ partials, int bx,
+                                                             const __grid_constant__ Params p) {
+  double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
+  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+    if (geo[i] != 0) return;
+    const Neigh nb(p, x, y, z);
+    const CellFlags<BC_GEO> c(p, x, y, z, i);
+    uint32_t solid = 0u;  // bit a: x + e_a is a solid node of geo
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      if constexpr (Dir<Q, a>::s > 0) {
+        if (!c.template leaves_box<Q, a, 1>()) solid |= (geo[nb.template at<Q, a, 1>()] != 0) ? (1u << a) : 0u;
+      }
+    });
+    if (solid == 0u) return;
+    double f[Q];
+    load_canonical<Q, BC_GEO, MODE, ST>(f, buf, p, nb, c);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      constexpr int o = Dir<Q, a>::opp;
+      using D = Dir<Q, a>;
+      if constexpr (D::s > 0) {
+        if ((solid >> a) & 1u) {
+          double post;
+          if constexpr (MODE == MODE_PULL) {
+            post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), i);
+          } else if constexpr (MODE == MODE_PULL_SWAP) {
+            post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.N), i);
+          } else {
+            if (c.template leaves<Q, a, 1>()) post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.N), i);
+            else post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), nb.template at<Q, a, 1>());
+          }
+          const double term = post + f[o];
+          if constexpr (D::ex != 0) acc[0] += D::ex * term;
+          if constexpr (D::ey != 0) acc[1] += D::ey * term;
+          if constexpr (D::ez != 0) acc[2] += D::ez * term;
+        }
+      }
+    });
+  });
+  block_reduce_diag(acc, partials + (long long)blockIdx.x * kDiag);
 }
 
 }  // namespace lbm

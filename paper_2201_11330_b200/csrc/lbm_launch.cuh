@@ -1,0 +1,34 @@
+// lbm_launch.cuh — host-side launch interface between the C ABI (lbm_abi.cu) and the kernel
+// instantiation units (lbm_inst.cu compiled once per lattice and part, in parallel).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "lbm_kernels.cuh"
+
+namespace lbm {
+
+// Everything a launcher needs to pick the compile-time variant and the launch shape.
+struct Ctx {
+  int eq;        // EQ_STANDARD / EQ_INCOMP
+  int bc;        // BC_PERIODIC / BC_WALLS / BC_GEO
+  int forced;    // body force != 0
+  int f32;       // populations stored as float
+  dim3 grid, block;  // fused stream-collide kernels
+  int flat_grid, fbx;  // row-wise sweeps off the per-step path (for_each_cell)
+  cudaStream_t stream;
+  Params p;
+};
+
+// One explicit specialisation of each per lattice Q in {9, 19, 27} (lbm_inst.cu).
+template <int Q> void launch_step_ab(const Ctx& c, const void* src, void* dst);
+template <int Q> void launch_step_aa_even(const Ctx& c, void* buf);
+template <int Q> void launch_step_aa_odd(const Ctx& c, void* buf);
+template <int Q> void launch_export(const Ctx& c, int mode, const void* buf, double* out);
+template <int Q> void launch_import(const Ctx& c, int mode, const double* in, void* buf);
+template <int Q> void launch_init(const Ctx& c, const double* rho, const double* u, double* out);
+template <int Q> void launch_moments(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials);
+template <int Q> void launch_geometry(const Ctx& c, const uint8_t* geo_in, uint8_t* geo, uint8_t* active, uint32_t* links, int nodal);
+template <int Q> void launch_boundary_force(const Ctx& c, int mode, const void* buf, const uint8_t* geo, double* partials);
+
+}  // namespace lbm

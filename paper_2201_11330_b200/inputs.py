@@ -21,6 +21,7 @@ SEED_BASE = 0x22011330
 
 FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING = 0, 1, 2
 EQ_STANDARD, EQ_INCOMP = 0, 1
+WALL_HALFWAY, WALL_NODAL = 0, 1
 
 _M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
 
@@ -101,6 +102,14 @@ def density_noise(nx, ny, nz, noise, seed, box=None):
     return 1.0 + noise * (2.0 * hash_uniform(seed, gi) - 1.0)
 
 
+def sphere_mask(nx, ny, nz, centre, radius):
+    """uint8[N]: 1 where (x-cx)^2 + (y-cy)^2 + (z-cz)^2 <= r^2 (lattice nodes inside or on the sphere)."""
+    x = np.arange(nx)[None, None, :] - centre[0]
+    y = np.arange(ny)[None, :, None] - centre[1]
+    z = np.arange(nz)[:, None, None] - centre[2]
+    return ((x * x + y * y + z * z) <= radius * radius).astype(np.uint8).reshape(-1)
+
+
 @dataclass
 class Workload:
     """One BASELINE.json config: geometry, physics parameters and how to make its fields."""
@@ -118,10 +127,30 @@ class Workload:
     noise: float = 0.0
     seed: int = 0
     kind: str = "tgv"  # "tgv" | "rest"
+    eq: int = EQ_STANDARD
+    wall_model: int = WALL_HALFWAY
+    sphere: tuple | None = None  # (cx, cy, cz, r): nodes with |x - c| <= r are solid
 
     @property
     def N(self):
         return self.nx * self.ny * self.nz
+
+    @property
+    def has_geometry(self):
+        return self.sphere is not None or self.wall_model != WALL_HALFWAY
+
+    def geo(self):
+        """Solid mask (uint8[N], 1 = solid node; the paper's `geo`) or None."""
+        if self.sphere is None:
+            return None
+        return sphere_mask(self.nx, self.ny, self.nz, self.sphere[:3], self.sphere[3])
+
+    def shrunk(self, k, steps=None):
+        """Same workload with every length (grid, sphere) divided by k."""
+        sp = None if self.sphere is None else tuple(v / k for v in self.sphere)
+        return Workload(f"{self.name}/{k}", self.nx // k, self.ny // k, self.nz // k, self.Q, self.tau, steps or self.steps,
+                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind, self.eq,
+                        self.wall_model, sp)
 
     def fields(self, box=None):
         """(rho[n], u[3,n]) on the full grid or on a periodically wrapped sub-box."""
@@ -132,8 +161,10 @@ class Workload:
 
     def scaled(self, n, steps=None, name=None):
         """Same parameters on an n^3 grid (reduced analogue for oracle-affordable parity)."""
+        sp = None if self.sphere is None else tuple(v * n / self.ny for v in self.sphere)
         return Workload(name or f"{self.name}@{n}", n, n, n, self.Q, self.tau, steps or self.steps,
-                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind)
+                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind, self.eq,
+                        self.wall_model, sp)
 
 
 _CAVITY_FACES = (FACE_BOUNCE,) * 5 + (FACE_MOVING,)
@@ -142,7 +173,7 @@ _CHANNEL_FACES = (FACE_PERIODIC,) * 4 + (FACE_BOUNCE, FACE_BOUNCE)
 
 
 def config(i: int) -> Workload:
-    """BASELINE.json configs[i], i = 0..4 (file order)."""
+    """BASELINE.json configs[i], i = 0..4 (file order); 5 = the paper's sphere case (S:§8f NEXT-2)."""
     if i == 0:
         return Workload("cfg0_q19_tgv32", 32, 32, 32, 19, 0.8, 100, u0=0.05, noise=1e-4, seed=SEED_BASE + 1)
     if i == 1:
@@ -155,4 +186,12 @@ def config(i: int) -> Workload:
     if i == 4:
         return Workload("cfg4_q27_channel512", 512, 512, 512, 27, 0.9, 20000, face_kind=_CHANNEL_FACES,
                         force=(1e-7, 0.0, 0.0), noise=1e-5, seed=SEED_BASE + 5, kind="rest")
+    if i == 5:
+        # Not in BASELINE.json: the paper's own profiled / validated case — D3Q27, 512 x 128 x 128,
+        # sphere of radius 8 at (64,64,64), the incompressible model the paper's code runs (Eq. 5) with its nodal
+        # bounce-back on the sphere.  The inlet / outlet / symmetric sides have no formulae in the paper, so the
+        # box is periodic and the flow is driven by a body force.
+        return Workload("cfg5_q27_sphere512x128x128", 512, 128, 128, 27, 1.0 / 1.8, 6401, force=(1e-6, 0.0, 0.0),
+                        noise=1e-5, seed=SEED_BASE + 6, kind="rest", eq=EQ_INCOMP, wall_model=WALL_NODAL,
+                        sphere=(64.0, 64.0, 64.0, 8.0))
     raise IndexError(i)

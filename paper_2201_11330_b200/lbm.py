@@ -13,11 +13,12 @@ import os
 
 import numpy as np
 
-LBM_D3Q19, LBM_D3Q27 = 19, 27
+LBM_D2Q9, LBM_D3Q19, LBM_D3Q27 = 9, 19, 27
 LBM_EQ_STANDARD, LBM_EQ_INCOMP = 0, 1 << 8
 LBM_SCHEME_AUTO, LBM_SCHEME_AB, LBM_SCHEME_AA = 0, 1 << 12, 2 << 12
 LBM_STORE_F64, LBM_STORE_F32 = 0, 1 << 16
 LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING = 0, 1, 2
+LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
@@ -27,6 +28,7 @@ SYMBOLS = (
     "lbm_create", "lbm_destroy", "lbm_init_equilibrium", "lbm_init_equilibrium_host", "lbm_step",
     "lbm_moments", "lbm_moments_host", "lbm_get_populations", "lbm_set_populations", "lbm_lattice",
     "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_last_error",
+    "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
 )
 
 
@@ -82,6 +84,11 @@ def load():
     lib.lbm_launch_count.argtypes = [vp]
     lib.lbm_set_block.restype = i32
     lib.lbm_set_block.argtypes = [vp, i32, i32]
+    for name in ("lbm_set_geometry", "lbm_set_geometry_host"):
+        getattr(lib, name).restype = i32
+        getattr(lib, name).argtypes = [vp, C.c_void_p, i32]
+    lib.lbm_boundary_force.restype = i32
+    lib.lbm_boundary_force.argtypes = [vp, C.c_void_p]
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_last_error.argtypes = []
     _lib = lib
@@ -133,6 +140,30 @@ def lbm_create(nx, ny, nz, lattice, tau, bc: lbm_bc_t | None = None):
 
 def lbm_destroy(h):
     load().lbm_destroy(h)
+
+
+def _u8ptr(t, n, device):
+    if t is None:
+        return None
+    import torch
+    assert isinstance(t, torch.Tensor) and t.dtype == torch.uint8 and t.is_contiguous(), "need a contiguous uint8 tensor"
+    assert t.device.type == device and t.numel() == n, (t.device, t.numel(), n)
+    return t.data_ptr()
+
+
+def lbm_set_geometry(h, geo, wall_model, n):
+    """geo: uint8 CUDA tensor of n = N bytes (non-zero = solid) or None."""
+    _check(load().lbm_set_geometry(h, _u8ptr(geo, n, "cuda"), int(wall_model)))
+
+
+def lbm_set_geometry_host(h, geo, wall_model, n):
+    _check(load().lbm_set_geometry_host(h, _u8ptr(geo, n, "cpu"), int(wall_model)))
+
+
+def lbm_boundary_force(h):
+    F = np.empty(3)
+    _check(load().lbm_boundary_force(h, F.ctypes.data))
+    return F
 
 
 def lbm_init_equilibrium(h, rho=None, u=None):
@@ -207,7 +238,14 @@ class Solver:
 
     @classmethod
     def from_workload(cls, w, **kw):
-        return cls(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u, force=w.force, **kw)
+        """Solver for an inputs.Workload, geometry (solid mask, wall model) included."""
+        import torch
+        eq = LBM_EQ_INCOMP if getattr(w, "eq", 0) else LBM_EQ_STANDARD
+        s = cls(w.nx, w.ny, w.nz, w.Q, w.tau, eq=eq, face_kind=w.face_kind, face_u=w.face_u, force=w.force, **kw)
+        if getattr(w, "has_geometry", False):
+            geo = w.geo()
+            s.set_geometry(None if geo is None else torch.from_numpy(geo), w.wall_model)
+        return s
 
     def close(self):
         if getattr(self, "h", None):
@@ -219,6 +257,16 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+    def set_geometry(self, geo=None, wall_model=LBM_WALL_HALFWAY):
+        """geo: uint8 tensor of N bytes (CUDA or CPU; non-zero = solid) or None."""
+        if geo is not None and geo.device.type == "cpu":
+            lbm_set_geometry_host(self.h, geo, wall_model, self.N)
+        else:
+            lbm_set_geometry(self.h, geo, wall_model, self.N)
+
+    def boundary_force(self):
+        return lbm_boundary_force(self.h)
 
     def init_equilibrium(self, rho=None, u=None):
         lbm_init_equilibrium(self.h, rho, u)

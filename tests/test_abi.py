@@ -32,6 +32,7 @@ def test_header_symbols_are_exported(lib):
     assert set(names) == set(lbm.SYMBOLS), (names, lbm.SYMBOLS)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/lbm.h but not exported"
+        assert getattr(lib, n).argtypes is not None, f"{n}: the binding sets no argtypes (pointers would be truncated)"
 
 
 def test_signatures_have_no_torch_types():
@@ -41,7 +42,23 @@ def test_signatures_have_no_torch_types():
     assert "torch" not in code.lower() and "at::" not in code and "#include <stdint.h>" in code
 
 
-@pytest.mark.parametrize("Q", [19, 27])
+def test_d2q9_table_is_the_papers_eq3_eq4(lib):
+    """The library's D2Q9 table against the values the paper prints (tests/golden/d2q9_eq3_eq4.txt)."""
+    from fractions import Fraction
+    rows = {}
+    with open(os.path.join(ROOT, "tests", "golden", "d2q9_eq3_eq4.txt")) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                k, *v = line.split()
+                rows[k] = v
+    e, t = lbm.lbm_lattice(lbm.LBM_D2Q9)
+    assert e[:, 0].tolist() == [int(v) for v in rows["ex"]]
+    assert e[:, 1].tolist() == [int(v) for v in rows["ey"]]
+    assert (e[:, 2] == 0).all()
+    assert t.tolist() == [float(Fraction(v)) for v in rows["t"]]
+
+
+@pytest.mark.parametrize("Q", [9, 19, 27])
 def test_lattice_order_matches_oracle(lib, Q):
     e, t = lbm.lbm_lattice(Q)
     eo, to = oracle_lattice(Q)

@@ -76,7 +76,7 @@ def face_u_of(spec):
 @pytest.mark.parametrize("faces", list(FACE_CASES))
 @pytest.mark.parametrize("Q,eq,forced", [(19, EQ_STANDARD, False), (19, EQ_STANDARD, True), (19, EQ_INCOMP, False),
                                          (19, EQ_INCOMP, True), (27, EQ_STANDARD, False), (27, EQ_STANDARD, True),
-                                         (27, EQ_INCOMP, True)])
+                                         (27, EQ_INCOMP, True), (9, EQ_STANDARD, False), (9, EQ_INCOMP, True)])
 def test_random_populations_ragged_grid(lbm, scheme, faces, Q, eq, forced):
     """Ragged 37x21x13 grid (several 32-wide tiles + a tail in x, odd y and z), random non-equilibrium
     populations, 7 steps (odd: the AA scheme is compared in its swapped phase too)."""
@@ -85,6 +85,10 @@ def test_random_populations_ragged_grid(lbm, scheme, faces, Q, eq, forced):
     fk, fu = FACE_CASES[faces]
     fu = face_u_of(fu)
     F = (2e-4, -1e-4, 3e-4) if forced else None
+    if Q == 9:
+        # D2Q9 has no z-links: z faces must be periodic for the comparison to mean anything, and MOVING z faces
+        # would never be crossed.  Keep the x / y face kinds of the case.
+        fk = list(fk[:4]) + [P, P]
     o, s = make_pair(lbm, dims, Q, 0.77, eq, dict(schemes(lbm))[scheme], fk, fu, F)
     f0 = random_f(Q, N, seed=Q + 100 * eq)
     o.set_f(f0)
@@ -393,6 +397,51 @@ def test_channel_steady_state_small_H(lbm, Q):
     z = np.arange(H) + 0.5
     ref = F * z * (H - z) / (2 * nu) + F / (2 * nu) * (4 * (tau - 0.5) ** 2 / 3 - 0.25)
     assert np.abs(prof - ref).max() / ref.max() < 1e-9
+    s.close()
+
+
+# --------------------------------------------------------------------------- D2Q9 (S:§8f NEXT-4; Eq. 3-4)
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_d2q9_taylor_green_decay(lbm, scheme):
+    """The paper's printed D2Q9 lattice on a single plane (nz = 1): 2-D Taylor-Green vortex, an exact
+    Navier-Stokes solution decaying as exp(-2 nu |k|^2 t), |k|^2 = 2 (2 pi / n)^2; parity with the oracle
+    over the whole run and the decay rate from the GPU's own energy history."""
+    n, tau, u0, steps = 64, 0.8, 0.02, 300
+    rho, u = inputs.taylor_green_2d(n, n, 1, u0)
+    o = Oracle(n, n, 1, 9, tau)
+    s = lbm.Solver(n, n, 1, 9, tau, scheme=dict(schemes(lbm))[scheme])
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    E = [s.diagnostics()[4]]
+    for _ in range(steps // 10):
+        s.step(10)
+        E.append(s.diagnostics()[4])
+    o.step(steps)
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    nu, k2 = (tau - 0.5) / 3, 2 * (2 * np.pi / n) ** 2
+    slope = np.polyfit(10 * np.arange(len(E)), np.log(E), 1)[0]
+    assert abs(slope / (-2 * nu * k2) - 1) < 2e-3
+    s.close()
+
+
+def test_d2q9_planes_are_independent(lbm):
+    """LBM_D2Q9 with nz > 1: every z-plane is an independent 2-D domain (include/lbm.h)."""
+    nx, ny, nz = 40, 24, 3
+    f0 = random_f(9, nx * ny * nz, seed=3)
+    fk = [B, B, P, P, P, P]
+    o, s = make_pair(lbm, (nx, ny, nz), 9, 0.7, face_kind=fk, force=(1e-4, 2e-4, 0))
+    o.set_f(f0)
+    s.set_populations(dev(f0))
+    o.step(6)
+    s.step(6)
+    got = s.get_populations().cpu().numpy()
+    assert np.abs(got - o.get_f()).max() <= TOL
+    one = lbm.Solver(nx, ny, 1, 9, 0.7, face_kind=fk, force=(1e-4, 2e-4, 0))
+    one.set_populations(dev(f0.reshape(9, nz, ny * nx)[:, 1].copy()))
+    one.step(6)
+    assert (one.get_populations().cpu().numpy() == got.reshape(9, nz, ny * nx)[:, 1]).all()
+    one.close()
     s.close()
 
 
