@@ -117,19 +117,22 @@ def ncu_traffic(workload_name: str, scheme: str):
     return None
 
 
-def pick_sample_grid(w, target_cells):
-    n = w.nx
-    while n ** 3 > target_cells and n > 32:
-        n //= 2
-    return n
+def pick_sample(w, target_cells):
+    """A reduced copy of workload w (same tau, fields recipe, walls, force, geometry) with at most target_cells
+    cells: every length halved until it fits."""
+    k = 1
+    while (w.nx // k) * (w.ny // k) * (w.nz // k) > target_cells and min(w.nx, w.ny, w.nz) // k > 32:
+        k *= 2
+    return w.shrunk(k) if k > 1 else w
 
 
-def oracle_mlups(w, n, steps, warmup=1):
-    """Time the oracle as it stands on an n^3 sample of workload w (same tau / walls / force / fields recipe)."""
+def oracle_mlups(ws, steps, warmup=1):
+    """Time the oracle as it stands on the sample workload ws."""
     from oracle import Oracle, num_threads
-    ws = w.scaled(n)
     rho, u = ws.fields()
-    o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force)
+    o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, eq=ws.eq, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force)
+    if ws.has_geometry:
+        o.set_geometry(ws.geo(), ws.wall_model)
     o.init_equilibrium(rho, u)
     o.step(warmup)
     t0 = time.perf_counter()
@@ -145,10 +148,11 @@ def run_reference(args, w):
     rank, _, world = replicas.env_world()
     if rank != 0:
         return 0
-    n = pick_sample_grid(w, 128 ** 3)
+    ws = pick_sample(w, 128 ** 3)
     t_all = time.perf_counter()
-    value, dt, cores = oracle_mlups(w, n, args.steps, max(args.warmup, 1))
-    sample = f"{n}^3 sub-grid of {w.name} (same tau, fields recipe, walls, force), {args.steps} oracle steps, {dt:.1f} s"
+    value, dt, cores = oracle_mlups(ws, args.steps, max(args.warmup, 1))
+    sample = (f"{ws.nx}x{ws.ny}x{ws.nz} reduced copy of {w.name} (same tau, fields recipe, walls, force, geometry), "
+              f"{args.steps} oracle steps, {dt:.1f} s")
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
@@ -234,7 +238,9 @@ def run_gpu(args, w):
         replicas.finalize()
         return 0
 
-    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8)  # S:§8d algorithmic bytes per lattice update
+    # S:§8d algorithmic bytes per lattice update: every population read once and written once (+ the 4-byte
+    # link mask of the geometry variant)
+    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8) + (4 if w.has_geometry else 0)
     ms_per_launch = secs / launches * 1e3
     achieved = bytes_per_cell * w.N / (secs / launches) / 1e9
     peak, peak_src = measured_peak()
@@ -244,6 +250,8 @@ def run_gpu(args, w):
         "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "collision": "BGK", "tau": w.tau,
+                   "equilibrium": "Eq. 5" if w.eq else "Eq. 2", "geometry": ("none" if not w.has_geometry else
+                                                                              ("nodal" if w.wall_model else "halfway") + " walls, solid mask"),
                    "scheme": args.scheme, "storage": args.store, "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
                    "l2": f"inputs larger than L2: {bytes_per_cell * w.N / 1e9:.2f} GB touched per step vs 126 MB L2"},
         "clocks": clocks,
@@ -259,11 +267,11 @@ def run_gpu(args, w):
     }
     # ---- the oracle on this box's host cores, on a bounded sample (reported baseline, not the target) ----
     if world == 1 and not args.no_cpu_baseline:
-        n = pick_sample_grid(w, 256 ** 3)
-        t0 = time.perf_counter()
-        v, dt, cores = oracle_mlups(w, n, 8, 1)
+        ws = pick_sample(w, 256 ** 3)
+        v, dt, cores = oracle_mlups(ws, 8, 1)
         out["cpu_baseline"] = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle",
-                               "sample": f"{n}^3 sub-grid of {w.name} (same tau, fields recipe, walls, force), 8 oracle steps, {dt:.1f} s"}
+                               "sample": f"{ws.nx}x{ws.ny}x{ws.nz} reduced copy of {w.name} (same tau, fields recipe, walls, force, "
+                                         f"geometry), 8 oracle steps, {dt:.1f} s"}
     else:
         out["cpu_baseline"] = None
     print(json.dumps(out), flush=True)
@@ -277,7 +285,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = 512^3 headline)")
+    ap.add_argument("--config", type=int, default=3,
+                    help="index into BASELINE.json configs (default 3 = 512^3 headline); 5 = the paper's sphere case")
     ap.add_argument("--scheme", default="ab", choices=["ab", "aa"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", default="", help="bx,by block shape override")

@@ -23,6 +23,8 @@
 //   indexing .................. pinned: independent brute-force gather on 4^3 (long double)
 //   D3Q27 ..................... pinned only through the same invariants and closed forms;
 //                               no D3Q27-specific printed value exists in the paper.
+//   D2Q9 ...................... pinned: the table is Eq. 3-4 as printed; dynamics by 2-D isotropy, brute-force
+//                               gather, exact 2-D Taylor-Green decay, Poiseuille closed form (tests/test_oracle_d2q9_pins.py)
 //   solid mask `geo` .......... pinned: brute-force gather with a mask; staircase channel built from
 //                               the mask equals the face-built channel bit for bit
 //   nodal bounce-back (Eq. 10)  pinned: second-order convergence of the channel profile (the
