@@ -63,11 +63,11 @@ __device__ __forceinline__ void static_for(F&& f) {
 }
 
 // Resident 256-thread blocks per SM the fused kernels are compiled for (register cap 80 / 128).
-// Measured on B200: the A/B D3Q19 kernels fit 80 registers without spilling and need the third block
-// (the fp32-storage variant loses 15 % of its bandwidth at two); the forced and in-place variants
-// and D3Q27 spill below 128.
-template <int Q, bool FORCE, bool INPLACE>
-constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
+// Measured on B200: the A/B D3Q19 kernels fit 80 registers without spilling and need the third block;
+// the fp32-storage A/B kernel keeps its populations packed (collide_shifted) and fits 64 registers, which
+// buys the fourth block its half-size loads need; the forced and in-place variants and D3Q27 spill below 128.
+template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
+constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 27 && STBYTES == 4 && !INPLACE) ? 3 : (Q == 19 && STBYTES == 4 && !INPLACE) ? (FORCE ? 3 : 4) : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
 
 // ---------------------------------------------------------------------------------------
 // How a cell finds out that a link has no upstream node (template parameter BC):
@@ -335,12 +335,106 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
   }
 }
 
+// The same collision for the fp32-storage variant, written in the stored variable g_a = f_a - t_a (S:§8f NEXT-1):
+//   rho = 1 + sum g,  sum e f = sum e g  (sum t = 1, sum t e = 0),
+//   g*_a = (1 - omega) g_a + omega t_a [ (rho - 1) + A (3 e.u + 4.5 (e.u)^2 - 1.5 u.u) ]  (+ source, Ladd term)
+// so the populations stay packed as floats in registers until they are used, no t_a is added or subtracted and
+// the small deviations are not rounded against O(t_a).  `store(IC<a>, g*_a)` writes one result.
+template <int Q, int EQ, int BC, bool FORCE, typename StoreF>
+__device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Params& p, const CellFlags<BC>& c, StoreF&& store) {
+  double dr = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
+  static_for<0, Q>([&](auto AA) {
+    constexpr int a = decltype(AA)::value;
+    using D = Dir<Q, a>;
+    const double v = (double)g[a];
+    dr += v;
+    if constexpr (D::ex == 1) mx += v;
+    if constexpr (D::ex == -1) mx -= v;
+    if constexpr (D::ey == 1) my += v;
+    if constexpr (D::ey == -1) my -= v;
+    if constexpr (D::ez == 1) mz += v;
+    if constexpr (D::ez == -1) mz -= v;
+  });
+  if constexpr (FORCE) {
+    mx += 0.5 * p.F[0];
+    my += 0.5 * p.F[1];
+    mz += 0.5 * p.F[2];
+  }
+  const double rho = 1.0 + dr;
+  double ux = mx, uy = my, uz = mz;
+  if constexpr (EQ == EQ_STANDARD) {
+    const double inv = 1.0 / rho;
+    ux *= inv; uy *= inv; uz *= inv;
+  }
+  const double om = p.omega, om1 = 1.0 - p.omega;
+  const double usq15 = 1.5 * (ux * ux + uy * uy + uz * uz);
+  const double A = (EQ == EQ_STANDARD) ? rho : 1.0;
+  const double base = dr - A * usq15;  // feq_a - t_a = t_a (base + A (3 e.u + 4.5 (e.u)^2))
+  double k = 0.0, uF3 = 0.0;
+  if constexpr (FORCE) {
+    k = 1.0 - 0.5 * om;
+    uF3 = 3.0 * (ux * p.F[0] + uy * p.F[1] + uz * p.F[2]);
+  }
+  // Ladd term of an outgoing wall link b through a MOVING face (D:R6), 0 elsewhere; `touch` keeps the
+  // per-direction tests off every cell that is not next to a MOVING face
+  bool touch = false;
+  if constexpr (BC != BC_PERIODIC) {
+    if (p.any_moving)
+      touch = (c.lo[0] && p.moving[0]) || (c.hi[0] && p.moving[1]) || (c.lo[1] && p.moving[2]) || (c.hi[1] && p.moving[3]) ||
+              (c.lo[2] && p.moving[4]) || (c.hi[2] && p.moving[5]);
+  }
+  auto ladd = [&](auto BB) -> double {
+    constexpr int b = decltype(BB)::value;
+    using D = Dir<Q, b>;
+    double corr = 0.0;
+    if constexpr (BC != BC_PERIODIC && D::s > 0) {
+      if (touch) {
+        int face = -1;
+        if constexpr (D::ex != 0) {
+          constexpr int fx = (D::ex == 1) ? 1 : 0;
+          if ((D::ex == 1 ? c.hi[0] : c.lo[0]) && p.moving[fx]) face = fx;
+        }
+        if constexpr (D::ey != 0) {
+          constexpr int fy = (D::ey == 1) ? 3 : 2;
+          if ((D::ey == 1 ? c.hi[1] : c.lo[1]) && p.moving[fy]) face = fy;
+        }
+        if constexpr (D::ez != 0) {
+          constexpr int fz = (D::ez == 1) ? 5 : 4;
+          if ((D::ez == 1 ? c.hi[2] : c.lo[2]) && p.moving[fz]) face = fz;
+        }
+        if (face >= 0) corr = (6.0 * D::t) * A * edot<Q, b>(p.face_u[face][0], p.face_u[face][1], p.face_u[face][2]);
+      }
+    }
+    return corr;
+  };
+  static_for<0, (Q + 1) / 2>([&](auto AA) {
+    constexpr int a = decltype(AA)::value;
+    using D = Dir<Q, a>;
+    if constexpr (a == D::opp) {
+      double gq = (om * D::t) * base;
+      if constexpr (FORCE) gq -= (k * D::t) * uF3;
+      store(IC<a>{}, fma(om1, (double)g[a], gq));
+    } else {
+      const double eu = edot<Q, a>(ux, uy, uz);
+      double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
+      double d = (3.0 * om * D::t) * (A * eu);
+      if constexpr (FORCE) {
+        const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
+        s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
+        d = fma(3.0 * k * D::t, eF, d);
+      }
+      store(IC<a>{}, fma(om1, (double)g[a], s + d) - ladd(IC<a>{}));
+      store(IC<D::opp>{}, fma(om1, (double)g[D::opp], s - d) - ladd(IC<D::opp>{}));
+    }
+  });
+}
+
 // Eq. 10 of the paper's modified nodal bounce-back (D:R17), applied to the populations a
 // wall node has just gathered: a direction a nothing streamed in along (link bit a set) takes the
 // value that arrived along its opposite, f_a = f_abar, if abar did arrive from an active node (bit
 // abar clear).  When neither end of the link is active the halfway value already in f[a] stays.
-template <int Q, int BC>
-__device__ __forceinline__ void nodal_replicate(double (&f)[Q], const Params& p, const CellFlags<BC>& c) {
+template <int Q, int BC, typename T>
+__device__ __forceinline__ void nodal_replicate(T (&f)[Q], const Params& p, const CellFlags<BC>& c) {
   if constexpr (BC == BC_GEO) {
     if (p.nodal && (c.m != 0u)) {
       static_for<0, Q>([&](auto A) {
@@ -355,35 +449,71 @@ __device__ __forceinline__ void nodal_replicate(double (&f)[Q], const Params& p,
   }
 }
 
+// Gather of the Q populations of one cell.  link(IC<a>) is the address f_a comes from when the link has an
+// upstream node, wall(IC<a>) the one it comes from otherwise (both always point into the buffer: the upstream
+// index is wrapped even across a wall face).  BC_WALLS selects the address (flags cost no memory access);
+// BC_GEO issues every regular load at once, WITHOUT waiting for the link mask, and re-reads only the wall links
+// afterwards: with address selection all Q loads would queue behind the mask load and the latency to cover
+// would double.  A regular load of a wall link reads a slot nobody writes; the value is discarded.  The price
+// is Q wasted loads on an inactive node, which is right for the paper's workloads (an obstacle in a channel:
+// a fraction of a percent of the nodes are solid).  Returns false for an inactive node.
+template <int Q, int BC, typename T, typename LinkF, typename WallF, typename LoadF>
+__device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&& link, WallF&& wall, LoadF&& load) {
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    auto q = link(A);
+    if constexpr (BC == BC_WALLS) {
+      if (c.template leaves<Q, a, -1>()) q = wall(A);  // a select, not a branch
+    }
+    f[a] = load(A, q);
+  });
+  if constexpr (BC == BC_GEO) {
+    if (!c.template active<Q>()) return false;
+    if (c.m != 0u) {
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        if constexpr (Dir<Q, a>::s > 0) {
+          if (c.template leaves<Q, a, -1>()) f[a] = load(A, wall(A));
+        }
+      });
+    }
+  }
+  return true;
+}
+
 // ---------------------------------------------------------------------------------------
 // A/B scheme ("stream on read").  The buffer holds the post-collision populations aligned at their
 // own cell, B = S^-1 f, S the slot permutation of one propagation (Eq. 7 with wall links, Eq. 10):
 // f_a(x) = B_a(x - e_a)  inside,  = B_abar(x)  at a wall link.  One step = pull (gives the canonical
 // pre-collision f of this time level), collide, store aligned at the own cell into the other buffer.
 template <int Q, int EQ, int BC, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
   const CellFlags<BC> c(p, x, y, z, nb.ic);
-  if (!c.template active<Q>()) return;  // solid interior: no traffic at all
-  double f[Q];
-  static_for<0, Q>([&](auto A) {
-    constexpr int a = decltype(A)::value;
-    const ST* q = plane<a>(src, p.N) + nb.template at<Q, a, -1>();
-    if constexpr (BC != BC_PERIODIC) {
-      if (c.template leaves<Q, a, -1>()) q = plane<Dir<Q, a>::opp>(src, p.N) + nb.ic;  // a select, not a branch
-    }
-    f[a] = ld_pop<ST, Q, a>(q, 0);  // t_a == t_abar: one load serves both cases
-  });
-  nodal_replicate<Q, BC>(f, p, c);
-  collide<Q, EQ, BC, FORCE>(f, p, c);
-  static_for<0, Q>([&](auto A) {
-    constexpr int a = decltype(A)::value;
-    st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
-  });
+  auto link = [&](auto A) { return plane<decltype(A)::value>(src, p.N) + nb.template at<Q, decltype(A)::value, -1>(); };
+  auto wall = [&](auto A) { return plane<Dir<Q, decltype(A)::value>::opp>(src, p.N) + nb.ic; };  // t_a == t_abar: same shift
+  if constexpr (sizeof(ST) == 4) {
+    float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
+    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
+    nodal_replicate<Q, BC>(g, p, c);
+    collide_shifted<Q, EQ, BC, FORCE>(g, p, c, [&](auto A, double v) {
+      constexpr int a = decltype(A)::value;
+      plane<a>(dst, p.N)[nb.ic] = (float)v;
+    });
+  } else {
+    double f[Q];
+    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
+    nodal_replicate<Q, BC>(f, p, c);
+    collide<Q, EQ, BC, FORCE>(f, p, c);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
+    });
+  }
 }
 
 // AA pattern (one buffer, in place).  Even phase: slot (x,a) holds f_a(x); read local, collide,
@@ -400,12 +530,12 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   if (x >= p.nx || y >= p.ny) return;
   const int ic = x + p.nx * (y + p.ny * z);
   const CellFlags<BC> c(p, x, y, z, ic);
-  if (!c.template active<Q>()) return;
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), ic);
   });
+  if (!c.template active<Q>()) return;  // after the loads: they do not wait for the link mask (see gather)
   nodal_replicate<Q, BC>(f, p, c);
   collide<Q, EQ, BC, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
@@ -422,18 +552,11 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
   const CellFlags<BC> c(p, x, y, z, nb.ic);
-  if (!c.template active<Q>()) return;
   double f[Q];
   // f_a(x) comes from the slot that f*_abar(x) goes to (link x <-> x - e_a traversed both ways)
-  static_for<0, Q>([&](auto A) {
-    constexpr int a = decltype(A)::value;
-    constexpr int o = Dir<Q, a>::opp;
-    const ST* q = plane<o>(buf, p.N) + nb.template at<Q, a, -1>();
-    if constexpr (BC != BC_PERIODIC) {
-      if (c.template leaves<Q, a, -1>()) q = plane<a>(buf, p.N) + nb.ic;
-    }
-    f[a] = ld_pop_rw<ST, Q, a>(q, 0);
-  });
+  auto link = [&](auto A) { return (const ST*)plane<Dir<Q, decltype(A)::value>::opp>(buf, p.N) + nb.template at<Q, decltype(A)::value, -1>(); };
+  auto wall = [&](auto A) { return (const ST*)plane<decltype(A)::value>(buf, p.N) + nb.ic; };
+  if (!gather<Q, BC>(f, c, link, wall, [](auto A, const ST* q) { return ld_pop_rw<ST, Q, decltype(A)::value>(q, 0); })) return;
   nodal_replicate<Q, BC>(f, p, c);
   collide<Q, EQ, BC, FORCE>(f, p, c);
   static_for<0, Q>([&](auto A) {
