@@ -126,20 +126,25 @@ def pick_sample(w, target_cells):
     return w.shrunk(k) if k > 1 else w
 
 
-def oracle_mlups(ws, steps, warmup=1):
-    """Time the oracle as it stands on the sample workload ws."""
+def oracle_mlups(ws, steps, warmup=1, budget_s=None):
+    """Time the oracle as it stands on the sample workload ws.  With budget_s, `steps` is replaced by the
+    number of steps that fills about budget_s seconds, estimated from the warm-up step(s)."""
     from oracle import Oracle, num_threads
     rho, u = ws.fields()
     o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, eq=ws.eq, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force)
     if ws.has_geometry:
         o.set_geometry(ws.geo(), ws.wall_model)
     o.init_equilibrium(rho, u)
+    t0 = time.perf_counter()
     o.step(warmup)
+    if budget_s is not None:
+        per_step = (time.perf_counter() - t0) / max(warmup, 1)
+        steps = max(steps, min(2000, int(budget_s / max(per_step, 1e-6))))
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
     o.close()
-    return ws.N * steps / dt / 1e6, dt, num_threads()
+    return ws.N * steps / dt / 1e6, dt, num_threads(), steps
 
 
 # ------------------------------------------------------------------------------------------ reference arm
@@ -148,9 +153,9 @@ def run_reference(args, w):
     rank, _, world = replicas.env_world()
     if rank != 0:
         return 0
-    ws = pick_sample(w, 128 ** 3)
+    ws = pick_sample(w, 256 ** 3)
     t_all = time.perf_counter()
-    value, dt, cores = oracle_mlups(ws, args.steps, max(args.warmup, 1))
+    value, dt, cores, _ = oracle_mlups(ws, args.steps, max(args.warmup, 1))
     sample = (f"{ws.nx}x{ws.ny}x{ws.nz} reduced copy of {w.name} (same tau, fields recipe, walls, force, geometry), "
               f"{args.steps} oracle steps, {dt:.1f} s")
     out = {
@@ -268,10 +273,10 @@ def run_gpu(args, w):
     # ---- the oracle on this box's host cores, on a bounded sample (reported baseline, not the target) ----
     if world == 1 and not args.no_cpu_baseline:
         ws = pick_sample(w, 256 ** 3)
-        v, dt, cores = oracle_mlups(ws, 8, 1)
+        v, dt, cores, osteps = oracle_mlups(ws, 8, 2, budget_s=15.0)
         out["cpu_baseline"] = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle",
                                "sample": f"{ws.nx}x{ws.ny}x{ws.nz} reduced copy of {w.name} (same tau, fields recipe, walls, force, "
-                                         f"geometry), 8 oracle steps, {dt:.1f} s"}
+                                         f"geometry), {osteps} oracle steps, {dt:.1f} s"}
     else:
         out["cpu_baseline"] = None
     print(json.dumps(out), flush=True)
