@@ -159,6 +159,56 @@ int64_t lbm_launch_count(lbm_handle h);
  * stream-collide kernel; 0,0 restores the default.  bx*by must be <= 256 and a multiple of 32. */
 int lbm_set_block(lbm_handle h, int bx, int by);
 
+/* ---------------------------------------------------------------------------------------------
+ * z-slab decomposition over several GPUs (Cartesian blocks, one process per device;
+ * the populations that cross a cut are exchanged once per step, `PassF`).
+ * D:R21.  The box nx*ny*nz_global is cut into slabs of whole z-planes; one handle per slab, one
+ * slab per GPU (several slabs on one device also work).  A slab handle is a box of
+ *     nz_local + 2  planes: plane 0 and plane nz_local+1 are HALO planes that stand for the last
+ *     plane of the slab below and the first plane of the slab above,
+ * so every array at this interface (rho, u, f, outputs) has N = nx*ny*(nz_local+2) cells per
+ * component, plane index 1 + (z_global - z0).  Inputs (lbm_init_equilibrium, lbm_set_populations)
+ * must carry the neighbouring slabs' values in the halo planes (periodic wrap included; ignored
+ * beyond a non-periodic z face); outputs are written on the nz_local own planes only and the
+ * diagnostics cover only them (sum / max / min them over the slabs).
+ * Per step the fused kernel also stores the 5 (D3Q19) / 9 (D3Q27) / 0 (D2Q9) populations per cell of
+ * its first and last plane that cross the cut directly into the neighbouring slab's halo plane (peer
+ * memory: NVLink between GPUs); there is no separate exchange pass and no host staging.  Ordering between
+ * slabs is on the device: step t of a slab starts when both neighbours have finished step t-1 (a 64-bit
+ * counter per side in the slab's own memory, written by the neighbour, waited for by the stream).
+ * Restrictions: LBM_SCHEME_AB only; no lbm_set_geometry; every slab must be advanced by the same
+ * number of steps; lbm_init_equilibrium / lbm_set_populations need all connected slabs idle. */
+
+/* What a neighbour needs to know about a slab.  Plain data: pass it to another process as bytes. */
+typedef struct {
+  uint64_t buf[2];        /* device addresses of the two population buffers (valid in the owner process) */
+  uint64_t flags;         /* device address of the two step counters {written by lower, by upper neighbour} */
+  int64_t plane_stride;   /* cells per direction plane = nx*ny*(nz_local+2)                              */
+  int32_t nz_local;
+  int32_t device;         /* CUDA device ordinal of the owner                                           */
+  int64_t pid;            /* owner process                                                              */
+  uint8_t ipc_buf[2][64]; /* cudaIpcMemHandle_t of buf[0], buf[1]                                        */
+  uint8_t ipc_flags[64];  /* cudaIpcMemHandle_t of flags                                                 */
+} lbm_slab_peer_t;
+
+/* Create the slab that owns global planes z0 .. z0+nz_local-1 of an nx*ny*nz_global box.  bc describes the
+ * WHOLE box: its z- / z+ faces act on the slab that owns plane 0 / nz_global-1.  lattice: as lbm_create,
+ * LBM_SCHEME_AA is refused (LBM_EUNSUPPORTED). */
+lbm_handle lbm_create_slab(int nx, int ny, int nz_local, int z0, int nz_global, int lattice, double tau, const lbm_bc_t* bc);
+
+/* Fill *out with this slab's addresses and IPC handles. */
+int lbm_slab_export(lbm_handle h, lbm_slab_peer_t* out);
+
+/* Connect the slab to its lower (z0-1) and upper (z0+nz_local) neighbours; NULL = none (a non-periodic z
+ * face, or nothing to exchange).  A periodic box of one slab connects to itself.  Descriptors of the same
+ * process are used as plain addresses (peer access between devices is enabled if needed); descriptors of
+ * another process are opened through their IPC handles.  Call on every slab before the first lbm_step. */
+int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_peer_t* upper);
+
+/* 1 = (default) device-side ordering by step counters; 0 = none: the caller synchronises all slabs between
+ * steps (lbm_step(h,1); stream sync; barrier) — for debugging and for several processes on ONE device. */
+int lbm_slab_set_sync(lbm_handle h, int device_sync);
+
 /* Message of the calling thread's last failed call ("" if none).  Static storage. */
 const char* lbm_last_error(void);
 

@@ -5,6 +5,9 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <unistd.h>
+
+#include <cuda.h>  // types of the stream memory operations only; entry points come from cudaGetDriverEntryPoint
 
 #include "../../include/lbm.h"
 #include "lbm_launch.cuh"
@@ -55,6 +58,20 @@ struct lbm_handle_s {
   double* diag_pinned;  // 8, host
   void* scratch;
   size_t scratch_bytes;
+  // z-slab of a decomposed box (D:R21)
+  bool slab;
+  int z0, nz_global, nz_local;
+  uint32_t* flags;        // device, 2 counters: steps finished by the lower / by the upper neighbour (they write, we wait)
+  uint32_t sync_count;    // steps this slab has finished since it was created (never reset)
+  int device_sync;
+  void* peer_lo[2];       // lower / upper neighbour's population buffers as seen from this process
+  void* peer_hi[2];
+  long long peer_lo_N, peer_hi_N;
+  int peer_lo_off, peer_hi_off;
+  uint32_t* peer_lo_flag;  // the counter we write in the lower neighbour (its "upper" one) / in the upper neighbour
+  uint32_t* peer_hi_flag;
+  void* ipc_opened[6];
+  int n_ipc_opened;
   int bx, by;         // block shape of the fused kernel (lbm_set_block)
   int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
   size_t elem() const { return f32 ? 4 : 8; }
@@ -87,7 +104,7 @@ Ctx make_ctx(const lbm_handle_s* h) {
   c.forced = h->forced;
   c.f32 = h->f32;
   c.block = dim3(h->bx, h->by, 1);
-  c.grid = dim3((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->nz);
+  c.grid = dim3((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->p.z_hi - h->p.z_lo);
   c.flat_grid = flat_grid(h);
   c.fbx = h->fbx;
   c.stream = h->stream;
@@ -99,6 +116,63 @@ Ctx make_ctx(const lbm_handle_s* h) {
 int read_mode(const lbm_handle_s* h) {
   if (h->scheme == LBM_SCHEME_AB) return MODE_PULL;
   return h->phase ? MODE_PULL_SWAP : MODE_NATURAL;
+}
+
+// Stream memory operation "wait until *addr >= value" (cyclic 32-bit compare), resolved once at run time so that
+// the library has no link-time dependency on libcuda.
+typedef CUresult (*wait_value32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+wait_value32_fn wait_value32() {
+  static wait_value32_fn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) f = nullptr;
+    cudaGetLastError();
+    return (wait_value32_fn)f;
+  }();
+  return fn;
+}
+
+// "this slab has finished `count` steps", written into the neighbours' counters after everything the step
+// kernel stored (their halo planes included) is visible system-wide
+__global__ void slab_signal_kernel(uint32_t* lo, uint32_t* hi, uint32_t count) {
+  __threadfence_system();
+  if (lo) *(volatile uint32_t*)lo = count;
+  if (hi) *(volatile uint32_t*)hi = count;
+}
+
+// One step of a z-slab: wait for both neighbours' previous step, run the fused kernel (which also fills the
+// neighbours' halo planes of the buffer it writes), tell the neighbours.
+// Make the stream wait until both neighbours have finished as many steps as this slab has: their stores into
+// this slab's halo planes are then complete, and they no longer read what the next step overwrites.
+int slab_wait_neighbours(lbm_handle_s* h) {
+  if (!h->slab || !h->device_sync) return LBM_OK;
+  wait_value32_fn wait = wait_value32();
+  if (!wait) return fail(LBM_ECUDA, "cuStreamWaitValue32 is not available on this driver");
+  for (int side = 0; side < 2; ++side) {
+    if (!(side ? h->peer_hi[0] : h->peer_lo[0])) continue;
+    CUresult r = wait((CUstream)h->stream, (CUdeviceptr)(h->flags + side), h->sync_count, CU_STREAM_WAIT_VALUE_GEQ);
+    if (r != CUDA_SUCCESS) return fail(LBM_ECUDA, "cuStreamWaitValue32 failed");
+  }
+  return LBM_OK;
+}
+
+int launch_step_slab(lbm_handle_s* h, Ctx& c) {
+  const int dst = h->cur ^ 1;
+  {
+    int rc = slab_wait_neighbours(h);
+    if (rc) return rc;
+  }
+  c.p.push_lo = h->peer_lo[dst];
+  c.p.push_hi = h->peer_hi[dst];
+  LBM_Q_CALL(h, launch_step_ab_slab, c, h->buf[h->cur], h->buf[dst]);
+  h->cur = dst;
+  ++h->launches;
+  ++h->sync_count;
+  if (h->device_sync && (h->peer_lo_flag || h->peer_hi_flag)) {
+    slab_signal_kernel<<<1, 1, 0, h->stream>>>(h->peer_lo_flag, h->peer_hi_flag, h->sync_count);
+    ++h->launches;
+  }
+  return LBM_OK;
 }
 
 void launch_step(lbm_handle_s* h, const Ctx& c) {
@@ -157,6 +231,7 @@ int check_launch(const char* what) {
 }
 
 int do_init(lbm_handle_s* h, const double* rho, const double* u) {
+  if (h->slab) h->cur = 0;  // connected slabs must agree on which buffer is current
   double* nat = nullptr;
   int rc = canonical_staging(h, &nat);
   if (rc) return rc;
@@ -172,6 +247,10 @@ int do_init(lbm_handle_s* h, const double* rho, const double* u) {
 }
 
 int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
+  {
+    int rc = slab_wait_neighbours(h);  // the pull reads the halo planes
+    if (rc) return rc;
+  }
   const Ctx c = make_ctx(h);
   double* partials = diagnostics ? h->partials : nullptr;
   LBM_Q_CALL(h, launch_moments, c, read_mode(h), h->buf[h->cur], rho, u, partials);
@@ -217,6 +296,7 @@ int alloc_geometry(lbm_handle_s* h) {
 
 // geo_dev: device pointer to N bytes (must not alias h->geo or h->active), or NULL (all fluid)
 int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
+  if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
   if (wall_model == LBM_WALL_NODAL && h->p.any_moving)
@@ -270,7 +350,8 @@ int lbm_lattice(int lattice, int32_t* e, double* t) {
   return LBM_OK;
 }
 
-lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm_bc_t* bc) {
+// slab: nz = nz_local + 2 planes are allocated (halo below and above), z0 / nz_global place the slab in the box
+static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, const lbm_bc_t* bc, bool slab, int z0, int nz_global) {
   const int Q = lattice & 0xff;
   if (Q != 9 && Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D2Q9, LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
   if (nx < 1 || ny < 1 || nz < 1) { fail(LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1"); return nullptr; }
@@ -315,7 +396,24 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
     }
     h->stream = (cudaStream_t)bc->stream;
   }
-  h->walls = p.wall[0] || p.wall[2] || p.wall[4];
+  p.z_lo = 0;
+  p.z_hi = nz;
+  if (slab) {
+    h->slab = true;
+    h->z0 = z0; h->nz_global = nz_global; h->nz_local = nz - 2;
+    h->device_sync = 1;
+    p.slab = 1;
+    p.z_lo = 1;
+    p.z_hi = nz - 1;
+    // the z faces of the box act only on the slab that owns them; elsewhere the cut is an ordinary interior plane
+    const bool owns_lo = z0 == 0, owns_hi = z0 + h->nz_local == nz_global;
+    if (!owns_lo) { p.wall[4] = 0; p.moving[4] = 0; }
+    if (!owns_hi) { p.wall[5] = 0; p.moving[5] = 0; }
+    p.any_moving = 0;
+    for (int k = 0; k < 6; ++k) p.any_moving |= p.moving[k];
+  }
+  // (walls: the coordinate-test kernels are needed if ANY face of this handle is a wall)
+  h->walls = p.wall[0] || p.wall[1] || p.wall[2] || p.wall[3] || p.wall[4] || p.wall[5];
   h->forced = p.F[0] != 0.0 || p.F[1] != 0.0 || p.F[2] != 0.0;
   // default block: as long along x as the row allows (coalesced, vector-friendly), 256 threads
   int bx = 32;
@@ -329,6 +427,10 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
   if (e == cudaSuccess) e = cudaMalloc((void**)&h->partials, (size_t)kReduceBlocks * kDiag * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc((void**)&h->diag_dev, kDiag * sizeof(double));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&h->diag_pinned, kDiag * sizeof(double));
+  if (e == cudaSuccess && slab) {
+    e = cudaMalloc((void**)&h->flags, 2 * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemset(h->flags, 0, 2 * sizeof(uint32_t));
+  }
   if (e != cudaSuccess) {
     const bool oom = (e == cudaErrorMemoryAllocation);
     std::string msg = std::string("lbm_create: ") + cudaGetErrorString(e);
@@ -340,9 +442,127 @@ lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm
   return h;
 }
 
+lbm_handle lbm_create(int nx, int ny, int nz, int lattice, double tau, const lbm_bc_t* bc) {
+  return create_impl(nx, ny, nz, lattice, tau, bc, false, 0, nz);
+}
+
+lbm_handle lbm_create_slab(int nx, int ny, int nz_local, int z0, int nz_global, int lattice, double tau, const lbm_bc_t* bc) {
+  if (nz_local < 1 || z0 < 0 || nz_global < 1 || (long long)z0 + nz_local > nz_global) {
+    fail(LBM_EINVAL, "lbm_create_slab: need nz_local >= 1, z0 >= 0 and z0 + nz_local <= nz_global");
+    return nullptr;
+  }
+  int scheme = lattice & (3 << 12);
+  if (scheme == LBM_SCHEME_AA) { fail(LBM_EUNSUPPORTED, "lbm_create_slab: z-slabs need LBM_SCHEME_AB"); return nullptr; }
+  if (nz_local > 65533) { fail(LBM_EINVAL, "lbm_create_slab: nz_local exceeds the launch grid limits"); return nullptr; }
+  return create_impl(nx, ny, nz_local + 2, lattice, tau, bc, true, z0, nz_global);
+}
+
+int lbm_slab_export(lbm_handle h, lbm_slab_peer_t* out) {
+  if (!h || !out) return fail(LBM_EINVAL, "lbm_slab_export: NULL argument");
+  if (!h->slab) return fail(LBM_EINVAL, "lbm_slab_export: not a slab handle (lbm_create_slab)");
+  std::memset(out, 0, sizeof(*out));
+  out->buf[0] = (uint64_t)h->buf[0];
+  out->buf[1] = (uint64_t)h->buf[1];
+  out->flags = (uint64_t)h->flags;
+  out->plane_stride = h->N;
+  out->nz_local = h->nz_local;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  out->device = dev;
+  out->pid = (int64_t)getpid();
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "lbm_slab_peer_t reserves 64 bytes per IPC handle");
+  cudaIpcMemHandle_t ih;
+  void* ptrs[3] = {h->buf[0], h->buf[1], (void*)h->flags};
+  uint8_t* dsts[3] = {out->ipc_buf[0], out->ipc_buf[1], out->ipc_flags};
+  for (int k = 0; k < 3; ++k) {
+    // without IPC support the descriptor still serves slabs of the same process
+    if (cudaIpcGetMemHandle(&ih, ptrs[k]) == cudaSuccess) std::memcpy(dsts[k], &ih, sizeof(ih));
+    else cudaGetLastError();
+  }
+  return LBM_OK;
+}
+
+namespace {
+// Address of a neighbour's allocation as this process / device may use it.
+int map_peer(lbm_handle_s* h, const lbm_slab_peer_t* d, uint64_t addr, const uint8_t* ipc, void** out) {
+  if (d->pid == (int64_t)getpid()) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (d->device != dev) {
+      int can = 0;
+      CUDA_TRY(cudaDeviceCanAccessPeer(&can, dev, d->device));
+      if (!can) return fail(LBM_EUNSUPPORTED, "lbm_slab_connect: no peer access between the two devices");
+      cudaError_t e = cudaDeviceEnablePeerAccess(d->device, 0);
+      if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail(e, "cudaDeviceEnablePeerAccess");
+      cudaGetLastError();
+    }
+    *out = (void*)addr;
+    return LBM_OK;
+  }
+  cudaIpcMemHandle_t ih;
+  std::memcpy(&ih, ipc, sizeof(ih));
+  void* ptr = nullptr;
+  cudaError_t e = cudaIpcOpenMemHandle(&ptr, ih, cudaIpcMemLazyEnablePeerAccess);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaIpcOpenMemHandle");
+  if (h->n_ipc_opened < 6) h->ipc_opened[h->n_ipc_opened++] = ptr;
+  *out = ptr;
+  return LBM_OK;
+}
+
+void close_peers(lbm_handle_s* h) {
+  for (int k = 0; k < h->n_ipc_opened; ++k) cudaIpcCloseMemHandle(h->ipc_opened[k]);
+  h->n_ipc_opened = 0;
+  h->peer_lo[0] = h->peer_lo[1] = h->peer_hi[0] = h->peer_hi[1] = nullptr;
+  h->peer_lo_flag = h->peer_hi_flag = nullptr;
+  cudaGetLastError();
+}
+}  // namespace
+
+int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_peer_t* upper) {
+  if (!h) return fail(LBM_EINVAL, "lbm_slab_connect: NULL handle");
+  if (!h->slab) return fail(LBM_EINVAL, "lbm_slab_connect: not a slab handle (lbm_create_slab)");
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  close_peers(h);
+  const long long plane = (long long)h->nx * h->ny;
+  for (int side = 0; side < 2; ++side) {
+    const lbm_slab_peer_t* d = side ? upper : lower;
+    if (!d) continue;
+    if (d->plane_stride != plane * (d->nz_local + 2) || d->nz_local < 1)
+      { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: neighbour descriptor does not match this slab's nx, ny"); }
+    void* b[2] = {nullptr, nullptr};
+    void* fl = nullptr;
+    int rc = map_peer(h, d, d->buf[0], d->ipc_buf[0], &b[0]);
+    if (!rc) rc = map_peer(h, d, d->buf[1], d->ipc_buf[1], &b[1]);
+    if (!rc) rc = map_peer(h, d, d->flags, d->ipc_flags, &fl);
+    if (rc) { close_peers(h); return rc; }
+    if (side == 0) {  // lower neighbour: we fill its UPPER halo plane and write its "upper neighbour" counter
+      h->peer_lo[0] = b[0]; h->peer_lo[1] = b[1];
+      h->peer_lo_N = d->plane_stride;
+      h->peer_lo_off = (int)(plane * (d->nz_local + 1));
+      h->peer_lo_flag = (uint32_t*)fl + 1;
+    } else {          // upper neighbour: its LOWER halo plane, its "lower neighbour" counter
+      h->peer_hi[0] = b[0]; h->peer_hi[1] = b[1];
+      h->peer_hi_N = d->plane_stride;
+      h->peer_hi_off = 0;
+      h->peer_hi_flag = (uint32_t*)fl;
+    }
+  }
+  h->p.push_lo_N = h->peer_lo_N; h->p.push_lo_off = h->peer_lo_off;
+  h->p.push_hi_N = h->peer_hi_N; h->p.push_hi_off = h->peer_hi_off;
+  return LBM_OK;
+}
+
+int lbm_slab_set_sync(lbm_handle h, int device_sync) {
+  if (!h || !h->slab) return fail(LBM_EINVAL, "lbm_slab_set_sync: not a slab handle");
+  h->device_sync = device_sync ? 1 : 0;
+  return LBM_OK;
+}
+
 void lbm_destroy(lbm_handle h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
+  if (h->slab) close_peers(h);
+  if (h->flags) cudaFree(h->flags);
   for (int b = 0; b < 2; ++b)
     if (h->buf[b]) cudaFree(h->buf[b]);
   if (h->partials) cudaFree(h->partials);
@@ -361,6 +581,7 @@ int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model) {
 
 int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model) {
   if (!h) return fail(LBM_EINVAL, "lbm_set_geometry_host: NULL handle");
+  if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (!geo_host) return do_set_geometry(h, nullptr, wall_model);
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
@@ -400,6 +621,7 @@ int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u) {
 
 int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host) {
   if (!h) return fail(LBM_EINVAL, "lbm_init_equilibrium_host: NULL handle");
+  if (h->slab) h->cur = 0;  // as do_init will (the staging below depends on it)
   // Stage the 4N doubles in device memory that do_init does not write before it has read them:
   // the CURRENT storage buffer for fp64 A/B (do_init writes the idle one first), else scratch.
   double* stage = nullptr;
@@ -429,9 +651,14 @@ int lbm_step(lbm_handle h, int nsteps) {
   if (!h) return fail(LBM_EINVAL, "lbm_step: NULL handle");
   if (nsteps < 0) return fail(LBM_EINVAL, "lbm_step: nsteps must be >= 0");
   if (nsteps == 0) return LBM_OK;
-  const Ctx c = make_ctx(h);
+  Ctx c = make_ctx(h);
   for (int s = 0; s < nsteps; ++s) {
-    launch_step(h, c);
+    if (h->slab) {
+      int rc = launch_step_slab(h, c);
+      if (rc) return rc;
+    } else {
+      launch_step(h, c);
+    }
     ++h->time;
   }
   h->stepped = true;
@@ -469,6 +696,10 @@ int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* dia
 
 int lbm_get_populations(lbm_handle h, double* f) {
   if (!h || !f) return fail(LBM_EINVAL, "lbm_get_populations: NULL argument");
+  {
+    int rc = slab_wait_neighbours(h);
+    if (rc) return rc;
+  }
   const Ctx c = make_ctx(h);
   LBM_Q_CALL(h, launch_export, c, read_mode(h), h->buf[h->cur], f);
   ++h->launches;
@@ -477,7 +708,7 @@ int lbm_get_populations(lbm_handle h, double* f) {
 
 int lbm_set_populations(lbm_handle h, const double* f) {
   if (!h || !f) return fail(LBM_EINVAL, "lbm_set_populations: NULL argument");
-  if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
+  if (h->scheme != LBM_SCHEME_AB || h->slab) h->cur = 0;
   do_import(h, f, h->cur);
   h->phase = 0;
   h->stepped = false;

@@ -1,11 +1,12 @@
 // lbm_inst.cu — kernel instantiations.  Compiled once per (LBM_Q, LBM_PART) by build.py, in parallel:
 //   LBM_Q    9 | 19 | 27
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
+//            5 A/B step of a z-slab (fused halo push)
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..4"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..5"
 #endif
 
 namespace lbm {
@@ -63,6 +64,24 @@ void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
     using ST = decltype(st);
     stream_collide_ab<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
         <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+  });
+}
+#elif LBM_PART == 5
+template <>
+void launch_step_ab_slab<Q_>(const Ctx& c, const void* src, void* dst) {
+  // z-slabs exist for the analytic box only (BC_PERIODIC / BC_WALLS): lbm_set_geometry refuses a slab handle
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_force(c, [&](auto force) {
+      dispatch_storage(c, [&](auto st) {
+        using ST = decltype(st);
+        if (c.bc == BC_PERIODIC)
+          stream_collide_ab<Q_, decltype(eq)::value, BC_PERIODIC, decltype(force)::value != 0, ST, true>
+              <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+        else
+          stream_collide_ab<Q_, decltype(eq)::value, BC_WALLS, decltype(force)::value != 0, ST, true>
+              <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+      });
+    });
   });
 }
 #elif LBM_PART == 1
@@ -143,7 +162,7 @@ void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const ui
   });
 }
 #else
-#error "LBM_PART must be 0..4"
+#error "LBM_PART must be 0..5"
 #endif
 
 }  // namespace lbm

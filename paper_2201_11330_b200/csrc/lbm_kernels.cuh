@@ -90,6 +90,19 @@ struct Params {
   // or beyond a non-periodic face); bit `rest`: node i itself is inactive.
   const uint32_t* links;
   int nodal;            // D:R3/R17: the paper's modified nodal bounce-back (Eq. 10) instead of halfway
+  // Planes [z_lo, z_hi) are the ones this handle updates and the z faces of the box lie at z_lo and z_hi-1.
+  // Whole box: 0, nz.  z-slab of a decomposed box (D:R21): 1, nz-1 — planes 0 and nz-1 are halo
+  // planes that hold the neighbouring slab's values; wall[4] / wall[5] are set only on the slab that owns the face.
+  int z_lo, z_hi;
+  int slab;
+  // slab only, A/B scheme: where the fused kernel ALSO stores the populations the neighbouring slab will pull
+  // across the cut (the paper's PassF, done by peer stores instead of a host-staged MPI exchange):
+  // direction plane a of the lower / upper neighbour's destination buffer starts at push_lo + a*push_lo_N;
+  // push_lo_off / push_hi_off = in-plane offset of that neighbour's receiving halo plane.  NULL = nothing to push.
+  void* push_lo;
+  void* push_hi;
+  long long push_lo_N, push_hi_N;
+  int push_lo_off, push_hi_off;
 };
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
@@ -105,8 +118,8 @@ struct CellFlags {
       hi[0] = (x == p.nx - 1) & (p.wall[1] != 0);
       lo[1] = (y == 0) & (p.wall[2] != 0);
       hi[1] = (y == p.ny - 1) & (p.wall[3] != 0);
-      lo[2] = (z == 0) & (p.wall[4] != 0);
-      hi[2] = (z == p.nz - 1) & (p.wall[5] != 0);
+      lo[2] = (z == p.z_lo) & (p.wall[4] != 0);
+      hi[2] = (z == p.z_hi - 1) & (p.wall[5] != 0);
     } else {
       lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
     }
@@ -486,11 +499,27 @@ __device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&
 // own cell, B = S^-1 f, S the slot permutation of one propagation (Eq. 7 with wall links, Eq. 10):
 // f_a(x) = B_a(x - e_a)  inside,  = B_abar(x)  at a wall link.  One step = pull (gives the canonical
 // pre-collision f of this time level), collide, store aligned at the own cell into the other buffer.
-template <int Q, int EQ, int BC, bool FORCE, typename ST>
+// SLAB (D:R21): the handle is one z-slab of a decomposed box.  Cells of the first / last updated plane store the
+// populations that cross the cut a second time, straight into the neighbouring slab's halo plane (peer memory over
+// NVLink, or the same device): e_z = -1 directions from plane z_lo, e_z = +1 directions from plane z_hi-1.  The
+// neighbour then pulls them like any other upstream value.  Compute and exchange are one kernel; the ordering
+// between slabs is stream-level (lbm_abi.cu: wait on the neighbours' step counters, launch, signal).
+template <int Q, int A, typename ST>
+__device__ __forceinline__ void push_one(const Params& p, int z, int ixy, ST v) {
+  if constexpr (Dir<Q, A>::ez == -1) {
+    if (z == p.z_lo && p.push_lo) ((ST*)p.push_lo + (long long)A * p.push_lo_N)[p.push_lo_off + ixy] = v;
+  }
+  if constexpr (Dir<Q, A>::ez == 1) {
+    if (z == p.z_hi - 1 && p.push_hi) ((ST*)p.push_hi + (long long)A * p.push_hi_N)[p.push_hi_off + ixy] = v;
+  }
+}
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB = false>
 __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
+  int z = blockIdx.z;
+  if constexpr (SLAB) z += p.z_lo;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
   const CellFlags<BC> c(p, x, y, z, nb.ic);
@@ -502,7 +531,9 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     nodal_replicate<Q, BC>(g, p, c);
     collide_shifted<Q, EQ, BC, FORCE>(g, p, c, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
-      plane<a>(dst, p.N)[nb.ic] = (float)v;
+      const float s = (float)v;
+      plane<a>(dst, p.N)[nb.ic] = s;
+      if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], s);
     });
   } else {
     double f[Q];
@@ -512,6 +543,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
+      if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], f[a]);
     });
   }
 }
@@ -601,11 +633,12 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
 // Row-wise grid-stride loop of the sweeps off the per-step path: a 256-thread block is bx x (256/bx)
 // with bx a power of two covering the row (or 256); rows (y,z) are dealt to the blocks round-robin.
 // One 32-bit division per row, none per cell; x stays the coalesced direction.
+// The rows are those of the updated planes [z_lo, z_hi), or of every plane (the halo planes of a slab too).
 template <typename F>
-__device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body) {
+__device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body, bool with_halo = false) {
   const int tx = threadIdx.x & (bx - 1), ty = threadIdx.x / bx, by = blockDim.x / bx;
-  const int rows = p.ny * p.nz;
-  for (int r = blockIdx.x * by + ty; r < rows; r += gridDim.x * by) {
+  const int r0 = with_halo ? 0 : p.ny * p.z_lo, rows = with_halo ? p.ny * p.nz : p.ny * p.z_hi;
+  for (int r = r0 + blockIdx.x * by + ty; r < rows; r += gridDim.x * by) {
     const int z = r / p.ny, y = r - z * p.ny;
     for (int x = tx; x < p.nx; x += bx) body(x, y, z, x + p.nx * r);
   }
@@ -648,10 +681,16 @@ __global__ void __launch_bounds__(256) import_canonical(const double* __restrict
         if constexpr (BC != BC_PERIODIC) {
           if (c.template leaves<Q, a, 1>()) q = plane<o>(in, p.N) + i;
         }
+        // slab: the halo planes are filled here too (the canonical arrays of a slab carry the neighbour's
+        // planes); a slot whose downstream node would lie beyond a halo plane is never read: leave it.
+        if constexpr (Dir<Q, a>::ez != 0) {
+          const int zd = z + Dir<Q, a>::ez;
+          if (p.slab && (zd < 0 || zd >= p.nz) && !c.template leaves<Q, a, 1>()) return;
+        }
       }
       st_pop<ST, Q, a>(plane<a>(buf, p.N), i, __ldg(q));
     });
-  });
+  }, p.slab != 0);
 }
 
 // InitPDF: canonical f_a(x) = feq_a(rho(x), u(x)), natural fp64 layout.
@@ -666,7 +705,7 @@ __global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __r
       constexpr int a = decltype(A)::value;
       plane<a>(out, p.N)[i] = feq[a];
     });
-  });
+  }, p.slab != 0);
 }
 
 // ---------------------------------------------------------------------------------------

@@ -29,6 +29,7 @@ SYMBOLS = (
     "lbm_moments", "lbm_moments_host", "lbm_get_populations", "lbm_set_populations", "lbm_lattice",
     "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_last_error",
     "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
+    "lbm_create_slab", "lbm_slab_export", "lbm_slab_connect", "lbm_slab_set_sync",
 )
 
 
@@ -38,6 +39,20 @@ class lbm_bc_t(C.Structure):
         ("face_u", (C.c_double * 3) * 6),
         ("force", C.c_double * 3),
         ("stream", C.c_void_p),
+    ]
+
+
+class lbm_slab_peer_t(C.Structure):
+    """What a neighbouring z-slab needs to know about a slab (include/lbm.h); plain bytes, picklable via bytes()."""
+    _fields_ = [
+        ("buf", C.c_uint64 * 2),
+        ("flags", C.c_uint64),
+        ("plane_stride", C.c_int64),
+        ("nz_local", C.c_int32),
+        ("device", C.c_int32),
+        ("pid", C.c_int64),
+        ("ipc_buf", (C.c_uint8 * 64) * 2),
+        ("ipc_flags", C.c_uint8 * 64),
     ]
 
 
@@ -89,6 +104,14 @@ def load():
         getattr(lib, name).argtypes = [vp, C.c_void_p, i32]
     lib.lbm_boundary_force.restype = i32
     lib.lbm_boundary_force.argtypes = [vp, C.c_void_p]
+    lib.lbm_create_slab.restype = vp
+    lib.lbm_create_slab.argtypes = [i32, i32, i32, i32, i32, i32, C.c_double, C.POINTER(lbm_bc_t)]
+    lib.lbm_slab_export.restype = i32
+    lib.lbm_slab_export.argtypes = [vp, C.POINTER(lbm_slab_peer_t)]
+    lib.lbm_slab_connect.restype = i32
+    lib.lbm_slab_connect.argtypes = [vp, C.POINTER(lbm_slab_peer_t), C.POINTER(lbm_slab_peer_t)]
+    lib.lbm_slab_set_sync.restype = i32
+    lib.lbm_slab_set_sync.argtypes = [vp, i32]
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_last_error.argtypes = []
     _lib = lib
@@ -140,6 +163,28 @@ def lbm_create(nx, ny, nz, lattice, tau, bc: lbm_bc_t | None = None):
 
 def lbm_destroy(h):
     load().lbm_destroy(h)
+
+
+def lbm_create_slab(nx, ny, nz_local, z0, nz_global, lattice, tau, bc: lbm_bc_t | None = None):
+    h = load().lbm_create_slab(int(nx), int(ny), int(nz_local), int(z0), int(nz_global), int(lattice), float(tau),
+                               None if bc is None else C.byref(bc))
+    if not h:
+        raise LBMError(LBM_EINVAL, lbm_last_error())
+    return h
+
+
+def lbm_slab_export(h) -> lbm_slab_peer_t:
+    d = lbm_slab_peer_t()
+    _check(load().lbm_slab_export(h, C.byref(d)))
+    return d
+
+
+def lbm_slab_connect(h, lower: lbm_slab_peer_t | None, upper: lbm_slab_peer_t | None):
+    _check(load().lbm_slab_connect(h, None if lower is None else C.byref(lower), None if upper is None else C.byref(upper)))
+
+
+def lbm_slab_set_sync(h, device_sync: bool):
+    _check(load().lbm_slab_set_sync(h, 1 if device_sync else 0))
 
 
 def _u8ptr(t, n, device):

@@ -1,0 +1,269 @@
+"""z-slab decomposition of one box over several GPUs (include/lbm.h "z-slab decomposition"; R21, §8).
+
+The paper splits the box into Cartesian MPI blocks, one per device, and exchanges the populations that
+cross a cut once per step through host-staged MPI.  Here the cut is along
+z only, the exchange is done by the fused step kernel itself (peer stores into the neighbour's halo plane)
+and the ordering between slabs is a device-side step counter; this module is the host-side plumbing:
+
+  partition / neighbours / halo_box / combine_diagnostics   pure functions (tested on CPU)
+  exchange_descriptors, all_reduce_diagnostics               torch.distributed (gloo on CPU, nccl on GPUs)
+  SlabSolver                                                 one slab = one rank's share (one process per GPU)
+  SlabGroup                                                  all slabs of a box in ONE process (one or more devices)
+
+No lattice-Boltzmann arithmetic happens here.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import lbm
+
+
+# ------------------------------------------------------------------------------------------ pure host logic
+def partition(nz: int, world: int):
+    """Balanced split of nz planes into `world` slabs of whole planes: [(z0, nz_local)], larger slabs first."""
+    if world < 1 or nz < world:
+        raise ValueError(f"cannot cut {nz} planes into {world} slabs of at least one plane")
+    base, extra = divmod(nz, world)
+    out, z0 = [], 0
+    for r in range(world):
+        n = base + (1 if r < extra else 0)
+        out.append((z0, n))
+        z0 += n
+    return out
+
+
+def neighbours(rank: int, world: int, periodic_z: bool):
+    """(lower, upper) rank of a slab, None where the box ends at a non-periodic z face.  A periodic box of one
+    slab is its own neighbour on both sides."""
+    lower = rank - 1 if rank > 0 else (world - 1 if periodic_z else None)
+    upper = rank + 1 if rank < world - 1 else (0 if periodic_z else None)
+    return lower, upper
+
+
+def halo_box(nx: int, ny: int, z0: int, nz_local: int):
+    """Sub-box of the global grid that a slab's arrays cover: its own planes plus one halo plane on each side
+    (inputs.Workload.fields(box=...) wraps the coordinates periodically)."""
+    return ((0, nx), (0, ny), (z0 - 1, z0 + nz_local + 1))
+
+
+def combine_diagnostics(parts):
+    """The 8 diagnostics of the whole box from those of its slabs: sums, max |u|, min rho, non-finite count."""
+    parts = np.asarray(list(parts), dtype=np.float64).reshape(-1, 8)
+    out = parts.sum(axis=0)
+    out[5] = parts[:, 5].max()
+    out[6] = parts[:, 6].min()
+    return out
+
+
+def strip_halo(a, nx: int, ny: int, nz_local: int, comps: int = 1):
+    """Own planes of a slab array laid out [comps][nz_local+2][ny][nx] -> [comps][nz_local*ny*nx]."""
+    v = a.reshape(comps, nz_local + 2, ny * nx)[:, 1:-1, :]
+    return v.reshape(comps, nz_local * ny * nx)
+
+
+# ------------------------------------------------------------------------------------------ torch.distributed
+def exchange_descriptors(desc_bytes: bytes):
+    """All ranks' slab descriptors (bytes of lbm_slab_peer_t), in rank order."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return [desc_bytes]
+    out = [None] * dist.get_world_size()
+    dist.all_gather_object(out, desc_bytes)
+    return out
+
+
+def all_reduce_diagnostics(diag, device="cpu"):
+    """combine_diagnostics across the ranks of the process group (three small all-reduces: SUM, MAX, MIN)."""
+    import torch
+    import torch.distributed as dist
+    d = np.asarray(diag, dtype=np.float64).copy()
+    if not (dist.is_available() and dist.is_initialized()):
+        return d
+    sums = torch.tensor(d, dtype=torch.float64, device=device)
+    mx = torch.tensor([d[5]], dtype=torch.float64, device=device)
+    mn = torch.tensor([d[6]], dtype=torch.float64, device=device)
+    dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+    dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+    dist.all_reduce(mn, op=dist.ReduceOp.MIN)
+    out = sums.cpu().numpy()
+    out[5] = float(mx.item())
+    out[6] = float(mn.item())
+    return out
+
+
+def _peer_from_bytes(b: bytes) -> lbm.lbm_slab_peer_t:
+    return lbm.lbm_slab_peer_t.from_buffer_copy(b)
+
+
+# ------------------------------------------------------------------------------------------ one slab
+class Slab:
+    """One z-slab handle with its placement; arrays at its interface cover nz_local + 2 planes."""
+
+    def __init__(self, w, z0, nz_local, scheme=lbm.LBM_SCHEME_AB, store=lbm.LBM_STORE_F64, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2201_11330_b200 needs a CUDA device (no CPU fallback)")
+        if getattr(w, "has_geometry", False):
+            raise lbm.LBMError(lbm.LBM_EUNSUPPORTED, "z-slabs do not support lbm_set_geometry")
+        self.w, self.z0, self.nz_local = w, int(z0), int(nz_local)
+        self.nx, self.ny, self.Q = w.nx, w.ny, w.Q
+        self.N = self.nx * self.ny * (self.nz_local + 2)
+        self.N_own = self.nx * self.ny * self.nz_local
+        self.device = torch.cuda.current_device()
+        self.torch_stream = stream
+        eq = lbm.LBM_EQ_INCOMP if getattr(w, "eq", 0) else lbm.LBM_EQ_STANDARD
+        self.bc = lbm.make_bc(w.face_kind, w.face_u, w.force, None if stream is None else stream.cuda_stream)
+        self.h = lbm.lbm_create_slab(self.nx, self.ny, self.nz_local, self.z0, w.nz, int(w.Q) | eq | scheme | store, w.tau, self.bc)
+
+    def descriptor(self) -> bytes:
+        return bytes(lbm.lbm_slab_export(self.h))
+
+    def connect(self, lower: bytes | None, upper: bytes | None):
+        lbm.lbm_slab_connect(self.h, None if lower is None else _peer_from_bytes(lower),
+                             None if upper is None else _peer_from_bytes(upper))
+
+    def fields(self):
+        """(rho, u) of the workload on this slab's planes + halo planes (numpy; seeded, point-wise recipe)."""
+        return self.w.fields(box=halo_box(self.nx, self.ny, self.z0, self.nz_local))
+
+    def init_equilibrium(self, rho=None, u=None):
+        """rho[N], u[3N] device tensors WITH halo planes; default: the workload's own fields."""
+        import torch
+        if rho is None and u is None:
+            r, v = self.fields()
+            rho = torch.from_numpy(r).cuda()
+            u = torch.from_numpy(np.ascontiguousarray(v.reshape(-1))).cuda()
+        lbm.lbm_init_equilibrium(self.h, rho, u)
+
+    def step(self, n=1):
+        lbm.lbm_step(self.h, n)
+
+    def diagnostics(self):
+        return lbm.lbm_moments(self.h, None, None, True)
+
+    def moments(self):
+        """(rho[N_own], u[3, N_own]) of the own planes (device tensors), diagnostics of the own planes."""
+        import torch
+        rho = torch.zeros(self.N, dtype=torch.float64, device="cuda")
+        u = torch.zeros(3 * self.N, dtype=torch.float64, device="cuda")
+        d = lbm.lbm_moments(self.h, rho, u, True)
+        return (strip_halo(rho, self.nx, self.ny, self.nz_local)[0], strip_halo(u, self.nx, self.ny, self.nz_local, 3), d)
+
+    def get_populations(self):
+        """Canonical populations of the own planes, [Q, N_own] (device tensor)."""
+        import torch
+        f = torch.zeros(self.Q * self.N, dtype=torch.float64, device="cuda")
+        lbm.lbm_get_populations(self.h, f)
+        return strip_halo(f, self.nx, self.ny, self.nz_local, self.Q)
+
+    def set_populations(self, f_with_halo):
+        lbm.lbm_set_populations(self.h, f_with_halo.contiguous().view(-1))
+
+    @property
+    def launches(self):
+        return lbm.lbm_launch_count(self.h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            lbm.lbm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class SlabSolver(Slab):
+    """This rank's slab of workload w under torch.distributed (one process per GPU): creates the slab, exchanges
+    the descriptors, connects to the neighbours' memory (CUDA IPC -> NVLink peer stores)."""
+
+    def __init__(self, w, rank, world, device_sync=True, **kw):
+        self.rank, self.world = rank, world
+        z0, nzl = partition(w.nz, world)[rank]
+        super().__init__(w, z0, nzl, **kw)
+        descs = exchange_descriptors(self.descriptor())
+        lo, up = neighbours(rank, world, w.face_kind[4] == 0)
+        self.connect(None if lo is None else descs[lo], None if up is None else descs[up])
+        if not device_sync:
+            lbm.lbm_slab_set_sync(self.h, False)
+
+    def global_diagnostics(self, device="cuda"):
+        return all_reduce_diagnostics(self.diagnostics(), device)
+
+
+class SlabGroup:
+    """All slabs of a box in one process: slab r on devices[r % len(devices)], each on its own stream.
+    Used to test the slab path on one GPU and to drive several GPUs from one process."""
+
+    def __init__(self, w, nslabs, devices=None, **kw):
+        import torch
+        self.w = w
+        self.devices = list(devices) if devices else [torch.cuda.current_device()]
+        self.slabs = []
+        self.parts = partition(w.nz, nslabs)
+        for r, (z0, nzl) in enumerate(self.parts):
+            with torch.cuda.device(self._dev(r)):
+                self.slabs.append(Slab(w, z0, nzl, stream=torch.cuda.Stream(), **kw))
+        descs = [s.descriptor() for s in self.slabs]
+        for r, s in enumerate(self.slabs):
+            lo, up = neighbours(r, nslabs, w.face_kind[4] == 0)
+            with torch.cuda.device(self._dev(r)):
+                s.connect(None if lo is None else descs[lo], None if up is None else descs[up])
+
+    def _dev(self, r):
+        return self.devices[r % len(self.devices)]
+
+    def _each(self, fn):
+        import torch
+        out = []
+        for r, s in enumerate(self.slabs):
+            with torch.cuda.device(self._dev(r)), torch.cuda.stream(s.torch_stream):
+                out.append(fn(s))
+        return out
+
+    def synchronize(self):
+        for s in self.slabs:
+            s.torch_stream.synchronize()
+
+    def init_equilibrium(self):
+        self.synchronize()
+        self._each(lambda s: s.init_equilibrium())
+        self.synchronize()
+
+    def step(self, n=1):
+        # one step per slab in turn: no stream ever queues far ahead of the neighbours it waits for
+        for _ in range(n):
+            for s in self.slabs:
+                s.step(1)
+
+    def diagnostics(self):
+        return combine_diagnostics(self._each(lambda s: s.diagnostics()))
+
+    def get_populations(self):
+        """Canonical populations of the whole box, [Q, N] (on the first device)."""
+        import torch
+        parts = self._each(lambda s: s.get_populations().view(s.Q, s.nz_local, -1))
+        self.synchronize()
+        dev = parts[0].device
+        return torch.cat([p.to(dev) for p in parts], dim=1).reshape(self.w.Q, -1)
+
+    def moments(self):
+        import torch
+        parts = self._each(lambda s: s.moments())
+        self.synchronize()
+        dev = parts[0][0].device
+        rho = torch.cat([p[0].to(dev) for p in parts])
+        u = torch.cat([p[1].view(3, s.nz_local, -1).to(dev) for p, s in zip(parts, self.slabs)], dim=1).reshape(3, -1)
+        return rho, u, combine_diagnostics([p[2] for p in parts])
+
+    @property
+    def launches(self):
+        return sum(s.launches for s in self.slabs)
+
+    def close(self):
+        self.synchronize()
+        for s in self.slabs:
+            s.close()

@@ -1,0 +1,203 @@
+"""GPU parity of the z-slab decomposition (include/lbm.h "z-slab decomposition", R21): a box cut into
+slabs whose fused step kernels fill each other's halo planes must give, cell for cell, the populations of the
+undivided box — bit for bit against the single-handle CUDA run (same arithmetic per cell), and within 1e-12 of
+the CPU oracle.  All slabs live on ONE device here (separate streams, device-side step counters); nothing in
+these tests makes a kernel wait for another kernel.
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from oracle.binding import EQ_INCOMP, EQ_STANDARD
+from paper_2201_11330_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+TOL = 1e-12
+B, M, P = inputs.FACE_BOUNCE, inputs.FACE_MOVING, inputs.FACE_PERIODIC
+
+
+@pytest.fixture(scope="module")
+def mods():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2201_11330_b200 import lbm, slabs
+    lbm.load()
+    return lbm, slabs
+
+
+def workload(dims, Q, tau, faces=None, face_u=None, force=(0.0, 0.0, 0.0), eq=EQ_STANDARD, kind="tgv", steps=8):
+    fu = np.zeros((6, 3))
+    for k, v in (face_u or {}).items():
+        fu[k] = v
+    return inputs.Workload(f"slabtest_{Q}_{dims}", dims[0], dims[1], dims[2], Q, tau, steps,
+                           face_kind=tuple(faces or [P] * 6), face_u=tuple(map(tuple, fu)), force=tuple(force),
+                           u0=0.05, noise=1e-3, seed=inputs.SEED_BASE + 77, kind=kind, eq=eq)
+
+
+def oracle_run(w, steps):
+    rho, u = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, eq=w.eq, face_kind=w.face_kind, face_u=w.face_u, force=w.force)
+    o.init_equilibrium(rho, u)
+    o.step(steps)
+    f = o.get_f()
+    d = o.moments(False)[2]
+    o.close()
+    return f, d
+
+
+def single_run(lbm, w, steps, store=0):
+    rho, u = w.fields()
+    s = lbm.Solver.from_workload(w, scheme=lbm.LBM_SCHEME_AB, store=store)
+    s.init_equilibrium(torch.from_numpy(rho).cuda(), torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).cuda())
+    s.step(steps)
+    f = s.get_populations().clone()
+    d = s.diagnostics()
+    s.close()
+    return f, d
+
+
+CASES = {
+    "tgv_periodic_q19": dict(dims=(24, 20, 22), Q=19, tau=0.8),
+    "channel_zwalls_q27_forced": dict(dims=(20, 12, 13), Q=27, tau=0.9, faces=[P, P, P, P, B, B], force=(1e-5, 2e-6, 0.0), kind="rest"),
+    "cavity_lid_q19": dict(dims=(16, 14, 12), Q=19, tau=0.55, faces=[B, B, B, B, B, M], face_u={5: (0.1, 0.0, 0.0)}, kind="rest"),
+    "moving_zlo_and_x_q27": dict(dims=(12, 10, 9), Q=27, tau=0.7, faces=[B, M, P, P, M, B],
+                                 face_u={1: (0.0, 0.03, -0.02), 4: (0.05, 0.01, 0.0)}, kind="rest"),
+    "incomp_forced_q19": dict(dims=(40, 6, 10), Q=19, tau=0.62, eq=EQ_INCOMP, force=(0.0, 1e-5, -3e-6)),
+    "d2q9_planes": dict(dims=(33, 17, 5), Q=9, tau=0.7),
+}
+
+
+@pytest.mark.parametrize("nslabs", [1, 2, 3])
+@pytest.mark.parametrize("case", list(CASES))
+def test_slabs_equal_the_undivided_box(mods, case, nslabs):
+    lbm, slabs = mods
+    w = workload(**CASES[case])
+    ref, dref = oracle_run(w, w.steps)
+    one, d1 = single_run(lbm, w, w.steps)
+    g = slabs.SlabGroup(w, nslabs)
+    g.init_equilibrium()
+    g.step(w.steps)
+    f = g.get_populations()
+    d = g.diagnostics()
+    launches = g.launches
+    g.close()
+    assert launches >= nslabs * w.steps
+    assert torch.equal(f, one), f"{case}: slabs differ from the undivided CUDA run by {float((f - one).abs().max())}"
+    assert float(np.abs(f.cpu().numpy() - ref).max()) <= TOL
+    # sums are order dependent (R14): relative 1e-12; max / min exact
+    for k in (0, 4):
+        assert abs(d[k] - dref[k]) <= 1e-12 * max(1.0, abs(dref[k]))
+    assert d[5] == d1[5] and d[6] == d1[6] and d[7] == 0
+
+
+def test_one_plane_slabs_and_ragged_split(mods):
+    """nz = 7 cut into 7 slabs of one plane (both pushes come from the same plane) and into 4 ragged slabs."""
+    lbm, slabs = mods
+    w = workload((18, 9, 7), 19, 0.6, steps=10)
+    one, _ = single_run(lbm, w, w.steps)
+    for n in (7, 4):
+        g = slabs.SlabGroup(w, n)
+        assert [p[1] for p in g.parts] == ([1] * 7 if n == 7 else [2, 2, 2, 1])
+        g.init_equilibrium()
+        g.step(w.steps)
+        f = g.get_populations()
+        g.close()
+        assert torch.equal(f, one)
+
+
+def test_random_populations_through_set_populations(mods):
+    """Non-equilibrium state handed over WITH halo planes (the interface contract of a slab)."""
+    lbm, slabs = mods
+    w = workload((10, 12, 9), 27, 0.75, faces=[P, P, B, B, P, P], kind="rest")
+    rng = np.random.default_rng(5)
+    f0 = (1.0 / 27) * (1.0 + 0.2 * rng.uniform(-1, 1, (27, w.nz, w.ny * w.nx)))
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind)
+    o.set_f(f0.reshape(27, -1))
+    o.step(5)
+    ref = o.get_f()
+    o.close()
+    g = slabs.SlabGroup(w, 3)
+    for s in g.slabs:
+        zs = [(s.z0 - 1 + k) % w.nz for k in range(s.nz_local + 2)]
+        s.set_populations(torch.from_numpy(np.ascontiguousarray(f0[:, zs, :])).cuda())
+    torch.cuda.synchronize()
+    g.step(5)
+    f = g.get_populations()
+    g.close()
+    assert float(np.abs(f.cpu().numpy() - ref).max()) <= TOL
+
+
+def test_fp32_storage_slabs_equal_the_undivided_fp32_run(mods):
+    lbm, slabs = mods
+    w = workload((32, 8, 12), 19, 0.8, steps=12)
+    one, _ = single_run(lbm, w, w.steps, store=lbm.LBM_STORE_F32)
+    g = slabs.SlabGroup(w, 3, store=lbm.LBM_STORE_F32)
+    g.init_equilibrium()
+    g.step(w.steps)
+    f = g.get_populations()
+    g.close()
+    assert torch.equal(f, one)
+
+
+def test_host_synchronised_mode(mods):
+    """lbm_slab_set_sync(0): no device-side counters, the caller synchronises all slabs between steps."""
+    lbm, slabs = mods
+    w = workload((16, 8, 10), 19, 0.7, steps=6)
+    one, _ = single_run(lbm, w, w.steps)
+    g = slabs.SlabGroup(w, 2)
+    for s in g.slabs:
+        lbm.lbm_slab_set_sync(s.h, False)
+    g.init_equilibrium()
+    for _ in range(w.steps):
+        g.step(1)
+        g.synchronize()
+    f = g.get_populations()
+    g.close()
+    assert torch.equal(f, one)
+
+
+def test_moments_fields_of_the_slabs(mods):
+    lbm, slabs = mods
+    w = workload((12, 10, 8), 19, 0.9, faces=[P, P, P, P, B, B], force=(2e-5, 0.0, 0.0), kind="rest", steps=7)
+    rho0, u0 = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, force=w.force)
+    o.init_equilibrium(rho0, u0)
+    o.step(w.steps)
+    rr, ur, dr = o.moments(True)
+    o.close()
+    g = slabs.SlabGroup(w, 3)
+    g.init_equilibrium()
+    g.step(w.steps)
+    rho, u, d = g.moments()
+    g.close()
+    assert float(np.abs(rho.cpu().numpy() - rr).max()) <= 1e-13
+    assert float(np.abs(u.cpu().numpy() - ur.reshape(3, -1)).max()) <= 1e-13
+    assert abs(d[1] - dr[1]) <= 1e-12 * max(1.0, abs(dr[1]))
+
+
+def test_slab_argument_errors(mods):
+    lbm, slabs = mods
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create_slab(8, 8, 4, 6, 8, 19, 0.8)  # z0 + nz_local > nz_global
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_create_slab(8, 8, 0, 0, 8, 19, 0.8)
+    with pytest.raises(lbm.LBMError) as ei:
+        lbm.lbm_create_slab(8, 8, 4, 0, 8, 19 | lbm.LBM_SCHEME_AA, 0.8)
+    assert ei.value.code == lbm.LBM_EINVAL or "LBM_SCHEME_AB" in str(ei.value)
+    h = lbm.lbm_create_slab(8, 8, 4, 0, 8, 19, 0.8)
+    other = lbm.lbm_create_slab(6, 8, 4, 4, 8, 19, 0.8)  # different nx
+    try:
+        with pytest.raises(lbm.LBMError):
+            lbm.lbm_slab_connect(h, lbm.lbm_slab_export(other), None)
+        with pytest.raises(lbm.LBMError):
+            lbm.lbm_set_geometry(h, None, lbm.LBM_WALL_NODAL, 8 * 8 * 6)
+        plain = lbm.lbm_create(8, 8, 8, 19, 0.8)
+        assert lbm.load().lbm_slab_export(plain, None) == lbm.LBM_EINVAL
+        with pytest.raises(lbm.LBMError):
+            lbm.lbm_slab_export(plain)
+        lbm.lbm_destroy(plain)
+    finally:
+        lbm.lbm_destroy(h)
+        lbm.lbm_destroy(other)
