@@ -284,6 +284,112 @@ def run_gpu(args, w):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ z-slab arm
+def run_gpu_slabs(args, w):
+    """--decomp zslab: ONE box cut into z-slabs.  Under torchrun: one slab per rank / GPU,
+    halo planes filled by the neighbours' fused kernels over NVLink peer memory (strong scaling: the box is fixed).
+    In a single process: --slabs R slabs on this GPU (measures what the slab path costs against the undivided box)."""
+    import numpy as np
+    import torch
+
+    from paper_2201_11330_b200 import lbm, replicas, slabs
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CUDA library is the only implementation")
+    lbm.load()
+    rank, local_rank, world = replicas.init()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    store = {"f64": lbm.LBM_STORE_F64, "f32": lbm.LBM_STORE_F32}[args.store]
+    K, W = args.steps, max(args.warmup, 3)
+    if world > 1:
+        stream = torch.cuda.Stream(device=dev)
+        g = slabs.SlabSolver(w, rank, world, store=store, stream=stream)
+        own_cells, nslabs = g.N_own, world
+        sync = stream.synchronize
+        with torch.cuda.stream(stream):
+            g.init_equilibrium()
+        diag = lambda: g.global_diagnostics(dev)
+        rec = lambda ev: ev.record(stream)
+    else:
+        g = slabs.SlabGroup(w, args.slabs, store=store)
+        own_cells, nslabs = w.N, args.slabs
+        sync = g.synchronize
+        g.init_equilibrium()
+        diag = g.diagnostics
+        rec = None
+    sync()
+    replicas.barrier()
+    d_init = diag()
+    g.step(W)
+    sync()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    replicas.barrier()
+    torch.cuda.synchronize()
+    l0 = g.launches
+    if rec is not None:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        rec(ev0)
+        g.step(K)
+        rec(ev1)
+        sync()
+        secs = ev0.elapsed_time(ev1) / 1e3
+    else:
+        # several streams: an event pair on every slab's stream, the job time is first start -> last end
+        evs = []
+        for s in g.slabs:
+            e0 = torch.cuda.Event(enable_timing=True)
+            e0.record(s.torch_stream)
+            evs.append([e0, None])
+        g.step(K)
+        for s, pair in zip(g.slabs, evs):
+            pair[1] = torch.cuda.Event(enable_timing=True)
+            pair[1].record(s.torch_stream)
+        sync()
+        first = evs[0][0]
+        secs = max(first.elapsed_time(p[1]) for p in evs) / 1e3
+    replicas.barrier()
+    launches = g.launches - l0
+    clocks = sampler.stop() if rank == 0 else None
+    d_end = diag()
+    units, secs_max, ups = replicas.aggregate_throughput(own_cells * K, secs, dev)
+    g.close()
+    if rank != 0:
+        replicas.finalize()
+        return 0
+    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8)
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_cell * units / secs_max / 1e9 / world  # per GPU
+    halo_dirs = sum(1 for ez in _EZ[w.Q] if ez == 1)
+    out = {
+        "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "collision": "BGK", "tau": w.tau,
+                   "scheme": "ab", "storage": args.store,
+                   "parallelism": f"z-slabs: {nslabs} slab(s) on {world} GPU(s), fused halo push over peer memory",
+                   "halo_bytes_per_step_per_cut": 2 * halo_dirs * w.nx * w.ny * (4 if args.store == "f32" else 8),
+                   "l2": f"inputs larger than L2: {bytes_per_cell * w.N / 1e9:.2f} GB touched per step vs 126 MB L2"},
+        "clocks": clocks, "e2e": None, "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "kernel": "stream_collide_ab<..., SLAB>", "bytes_per_cell_update": bytes_per_cell, "peak_source": peak_src,
+                     "note": "per GPU: algorithmic bytes of all slabs / job time / GPUs"},
+        "checks": {"mass_drift_rel": abs(d_end[0] - d_init[0]) / d_init[0], "nonfinite_cells": d_end[7]},
+        "cpu_baseline": None,
+    }
+    print(json.dumps(out), flush=True)
+    replicas.finalize()
+    return 0
+
+
+# e_z of every direction in the library's order (DESIGN.md R4), only to count the populations that cross a z cut
+_EZ = {9: [0] * 9,
+       19: [0, -1, 0, 1, 0, -1, 0, 1, -1, 0, 1, -1, 0, 1, 0, -1, 0, 1, 0],
+       27: [-1, 0, 1] * 9}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -296,11 +402,16 @@ def main():
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", default="", help="bx,by block shape override")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "zslab"],
+                    help="--gpus N > 1: N independent replicas (default; BASELINE.json: no sharding) or ONE box cut into z-slabs")
+    ap.add_argument("--slabs", type=int, default=2, help="--decomp zslab in a single process: slabs on this one GPU")
     args = ap.parse_args()
     from paper_2201_11330_b200 import inputs
     w = inputs.config(args.config)
     if args.impl == "reference":
         return run_reference(args, w)
+    if args.decomp == "zslab":
+        return run_gpu_slabs(args, w)
     return run_gpu(args, w)
 
 

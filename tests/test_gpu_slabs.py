@@ -201,3 +201,67 @@ def test_slab_argument_errors(mods):
     finally:
         lbm.lbm_destroy(h)
         lbm.lbm_destroy(other)
+
+
+# --------------------------------------------------------------------------- two processes, CUDA IPC
+IPC_WORKER = r"""
+import os, sys, json
+import numpy as np
+import torch
+import torch.distributed as dist
+sys.path.insert(0, os.environ["LBM_ROOT"])
+from paper_2201_11330_b200 import inputs, lbm, replicas, slabs
+rank, local_rank, world = replicas.init(backend="gloo")
+torch.cuda.set_device(0)  # both ranks share the one GPU: host-synchronised mode, no rank ever waits on the device
+lbm.load()
+w = inputs.Workload("ipc", 20, 12, 11, 19, 0.7, 6, face_kind=(0, 0, 1, 1, 0, 0), u0=0.04, noise=1e-3, seed=inputs.SEED_BASE + 9)
+g = slabs.SlabSolver(w, rank, world, device_sync=False)
+g.init_equilibrium()
+torch.cuda.synchronize(); replicas.barrier()
+for _ in range(w.steps):
+    g.step(1)
+    torch.cuda.synchronize(); replicas.barrier()
+own = g.get_populations().cpu().view(w.Q, g.nz_local, -1)
+tot = slabs.all_reduce_diagnostics(g.diagnostics())
+parts = [None] * world
+dist.all_gather_object(parts, own.numpy())
+if rank == 0:
+    f = np.concatenate(parts, axis=1).reshape(w.Q, -1)
+    rho, u = w.fields()
+    s = lbm.Solver.from_workload(w)
+    s.init_equilibrium(torch.from_numpy(rho).cuda(), torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).cuda())
+    s.step(w.steps)
+    one = s.get_populations().cpu().numpy()
+    d1 = s.diagnostics()
+    s.close()
+    print("OUT" + json.dumps({"equal": bool(np.array_equal(f, one)), "maxdiff": float(np.abs(f - one).max()),
+                              "mass_rel": float(abs(tot[0] - d1[0]) / d1[0]), "umax_equal": bool(tot[5] == d1[5])}), flush=True)
+replicas.barrier()
+g.close()
+replicas.finalize()
+"""
+
+
+def test_two_processes_connected_through_cuda_ipc(mods, tmp_path):
+    """One process per slab as under torchrun (descriptors exchanged as bytes, neighbour memory opened with CUDA IPC,
+    halo planes filled by the other process's kernel).  Both processes share this one GPU, so the run is
+    host-synchronised (lbm_slab_set_sync(0)): a step, a stream sync, a barrier."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "ipc_worker.py"
+    script.write_text(IPC_WORKER)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, LBM_ROOT=root, MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
+    r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-8000:]
+    out = [json.loads(ln[3:]) for ln in r.stdout.splitlines() if ln.startswith("OUT")][-1]
+    assert out["equal"], out
+    assert out["mass_rel"] <= 1e-13 and out["umax_equal"]
