@@ -15,7 +15,7 @@ _lib = None
 
 EQ_STANDARD, EQ_INCOMP = 0, 1
 WALL_HALFWAY, WALL_NODAL = 0, 1
-FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING = 0, 1, 2
+FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE = 0, 1, 2, 3
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -41,6 +41,8 @@ def _load():
         lib.orc_set_geometry.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         lib.orc_get_active.argtypes = [C.c_void_p, C.c_void_p]
         lib.orc_boundary_force.argtypes = [C.c_void_p, _dp]
+        lib.orc_set_face_rho.argtypes = [C.c_void_p, _dp]
+        lib.orc_set_face_velocity.argtypes = [C.c_void_p, C.c_int, _dp]
         lib.orc_num_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -82,7 +84,7 @@ def feq(Q: int, eq: int, rho: float, u) -> np.ndarray:
 
 
 class Oracle:
-    def __init__(self, nx, ny, nz, Q=19, tau=0.8, eq=EQ_STANDARD, face_kind=None, face_u=None, force=None):
+    def __init__(self, nx, ny, nz, Q=19, tau=0.8, eq=EQ_STANDARD, face_kind=None, face_u=None, force=None, face_rho=None):
         lib = _load()
         self.nx, self.ny, self.nz, self.Q = int(nx), int(ny), int(nz), int(Q)
         self.N = self.nx * self.ny * self.nz
@@ -94,6 +96,15 @@ class Oracle:
         if not self._h:
             raise ValueError("orc_create failed (bad lattice, size or tau <= 0.5)")
         self._lib = lib
+        if face_rho is not None:
+            fr = np.ascontiguousarray(face_rho, dtype=np.float64).reshape(6)
+            lib.orc_set_face_rho(self._h, _p(fr))
+
+    def set_face_velocity(self, face, u=None):
+        """Per-cell wall velocity of MOVING face `face`: u[3, n] over the face's cells (lower axis fastest); None = uniform."""
+        uu = None if u is None else np.ascontiguousarray(u, dtype=np.float64).reshape(-1)
+        if self._lib.orc_set_face_velocity(self._h, int(face), _p(uu)) != 0:
+            raise ValueError("bad face")
 
     def close(self):
         if getattr(self, "_h", None):

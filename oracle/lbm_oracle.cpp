@@ -84,7 +84,10 @@ bool make_lattice(int Q, Lattice& L) {
 }
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };              // Eq. 2 | Eq. 5
-enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2 };
+enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3 };
+// D:R22 (open boundaries; the paper names a parabolic inlet and an outflow, with no formulae):
+//   inlet  = FACE_MOVING with a per-cell wall velocity profile (velocity bounce-back, Ladd),
+//   outlet = FACE_PRESSURE: anti-bounce-back at the prescribed density face_rho.
 // D:R3 / D:R16.  HALFWAY: the wall lies half a link beyond the last fluid node (BASELINE.json
 // configs).  NODAL: the paper's "modified nodal bounce back" (Eq. 10): wall nodes lie on
 // the wall, receive f_alpha = f_abar for the directions no node streams into them, and collide.
@@ -99,10 +102,13 @@ struct Oracle {
   double rho0;       // constant density of the incompressible model, 1
   int face_kind[6];  // x-, x+, y-, y+, z-, z+
   double face_u[6][3];
+  double face_rho[6];                      // density prescribed on FACE_PRESSURE faces (D:R22)
+  std::vector<double> face_profile[6];     // optional per-cell wall velocity of a MOVING face: [c*n + j] (D:R22)
   double F[3];       // uniform body force density (D:R7, Guo forcing; not in the paper)
   std::vector<double> f;      // P:208 `f`:  pre-collision populations, AoS f[id*Q+iq]
   std::vector<double> fb;     // P:208 `fb`: "backup" = post-collision populations
   std::vector<double> rho_w;  // density seen by the collision sweep, kept for the wall term (D:R6)
+  std::vector<double> u_w;    // velocity seen by the collision sweep, [i*3+d], kept for the pressure faces (D:R22)
   std::vector<uint8_t> geo;     // P:210 `geo`: 1 = solid node, 0 = fluid node (all fluid by default)
   std::vector<uint8_t> active;  // node takes part in collision and propagation (D:R16)
   int wall_model = WALL_HALFWAY;
@@ -142,11 +148,14 @@ inline void moments_of(const Oracle& o, const double* fc, double& rho, double u[
 
 // Node x + s*e_iq with periodic wrap.  Returns false if it lies outside the box through a
 // non-periodic face; then `moving_face` is the MOVING face crossed (D:R6 tie-break: the highest
-// face index among the MOVING faces crossed) or -1.
-inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int out[3], int* moving_face) {
+// face index among the MOVING faces crossed) or -1, and `pressure_face` (D:R22) the PRESSURE face that
+// resolves the link: the highest-index PRESSURE face crossed, but only if the link crosses no MOVING
+// and no BOUNCE face (precedence MOVING > BOUNCE > PRESSURE), else -1.
+inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int out[3], int* moving_face,
+                      int* pressure_face = nullptr) {
   const int c[3] = {x, y, z}, n[3] = {o.nx, o.ny, o.nz};
-  bool inside = true;
-  if (moving_face) *moving_face = -1;
+  bool inside = true, bounce = false;
+  int mf = -1, pf = -1;
   for (int d = 0; d < 3; ++d) {
     out[d] = c[d] + sgn * o.L.e[iq][d];
     if (out[d] < 0 || out[d] >= n[d]) {
@@ -155,11 +164,30 @@ inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int
         out[d] = ((out[d] % n[d]) + n[d]) % n[d];
       } else {
         inside = false;
-        if (moving_face && o.face_kind[face] == FACE_MOVING && face > *moving_face) *moving_face = face;
+        if (o.face_kind[face] == FACE_MOVING && face > mf) mf = face;
+        if (o.face_kind[face] == FACE_BOUNCE) bounce = true;
+        if (o.face_kind[face] == FACE_PRESSURE && face > pf) pf = face;
       }
     }
   }
+  if (moving_face) *moving_face = mf;
+  if (pressure_face) *pressure_face = (mf < 0 && !bounce) ? pf : -1;
   return inside;
+}
+
+// Wall velocity of MOVING face `face` as seen by cell (x,y,z): the uniform face_u, or the cell's entry of the
+// per-cell profile (D:R22), indexed by the two in-face coordinates of the cell, lower axis fastest.
+inline void wall_velocity(const Oracle& o, int face, int x, int y, int z, double uw[3]) {
+  if (o.face_profile[face].empty()) {
+    for (int d = 0; d < 3; ++d) uw[d] = o.face_u[face][d];
+    return;
+  }
+  const int axis = face / 2;
+  int64_t j, n;
+  if (axis == 0) { j = y + (int64_t)o.ny * z; n = (int64_t)o.ny * o.nz; }
+  else if (axis == 1) { j = x + (int64_t)o.nx * z; n = (int64_t)o.nx * o.nz; }
+  else { j = x + (int64_t)o.nx * y; n = (int64_t)o.nx * o.ny; }
+  for (int d = 0; d < 3; ++d) uw[d] = o.face_profile[face][(size_t)d * n + j];
 }
 
 // D:R16.  HALFWAY: the active nodes are the fluid nodes (geo = 0).  NODAL: also every solid node
@@ -236,6 +264,7 @@ void collision(Oracle& o) {
     double rho, u[3];
     moments_of(o, fc, rho, u);
     o.rho_w[i] = (o.eq == EQ_STANDARD) ? rho : o.rho0;
+    for (int d = 0; d < 3; ++d) o.u_w[i * 3 + d] = u[d];
     for (int iq = 0; iq < Q; ++iq) {
       const double feq = feq_value(o, iq, rho, u);
       double out = fc[iq] - o.omega * (fc[iq] - feq);
@@ -277,16 +306,30 @@ void propagation(Oracle& o) {
         const int64_t i = o.cell(x, y, z);
         if (!o.active[i]) continue;
         for (int iq = 0; iq < Q; ++iq) {
-          int s[3], moving_face;
-          const bool inside = neighbour(o, x, y, z, iq, -1, s, &moving_face);
+          int s[3], moving_face, pressure_face;
+          const bool inside = neighbour(o, x, y, z, iq, -1, s, &moving_face, &pressure_face);
           if (inside && o.active[o.cell(s[0], s[1], s[2])]) {
             o.f[i * Q + iq] = o.fb[o.cell(s[0], s[1], s[2]) * Q + iq];
           } else if (o.wall_model == WALL_HALFWAY) {
             double v = o.fb[i * Q + (Q - 1 - iq)];
             if (!inside && moving_face >= 0) {
-              double eduw = 0.0;
-              for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * o.face_u[moving_face][d];
+              double uw[3], eduw = 0.0;
+              wall_velocity(o, moving_face, x, y, z, uw);
+              for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * uw[d];
               v += 6.0 * o.L.t[iq] * o.rho_w[i] * eduw;
+            } else if (!inside && pressure_face >= 0) {
+              // D:R22 anti-bounce-back: f_a = -f*_abar + 2 feq+_a(rho_face, u(x,t)), feq+ = the part of the
+              // equilibrium that is even in e (Eq. 2: t rho (1 + 4.5 (e.u)^2 - 1.5 u.u); Eq. 5: t (rho + rho0 (...)))
+              const double* uu = &o.u_w[i * 3];
+              double edu = 0.0, udu = 0.0;
+              for (int d = 0; d < 3; ++d) {
+                edu += o.L.e[iq][d] * uu[d];
+                udu += uu[d] * uu[d];
+              }
+              const double rf = o.face_rho[pressure_face];
+              const double even = (o.eq == EQ_STANDARD) ? o.L.t[iq] * rf * (1.0 + 4.5 * edu * edu - 1.5 * udu)
+                                                        : o.L.t[iq] * (rf + o.rho0 * (4.5 * edu * edu - 1.5 * udu));
+              v = -v + 2.0 * even;
             }
             o.f[i * Q + iq] = v;
           }
@@ -392,11 +435,13 @@ void* orc_create(int nx, int ny, int nz, int Q, int eq, double tau, const int* f
   for (int k = 0; k < 6; ++k) {
     o->face_kind[k] = face_kind ? face_kind[k] : FACE_PERIODIC;
     for (int d = 0; d < 3; ++d) o->face_u[k][d] = face_u ? face_u[3 * k + d] : 0.0;
+    o->face_rho[k] = 1.0;
   }
   for (int d = 0; d < 3; ++d) o->F[d] = force ? force[d] : 0.0;
   o->f.assign((size_t)o->N * Q, 0.0);
   o->fb.assign((size_t)o->N * Q, 0.0);
   o->rho_w.assign((size_t)o->N, 1.0);
+  o->u_w.assign((size_t)o->N * 3, 0.0);
   o->geo.assign((size_t)o->N, 0);
   o->active.assign((size_t)o->N, 1);
   return o;
@@ -412,6 +457,24 @@ int orc_set_geometry(void* h, const uint8_t* geo, int wall_model) {
   o.wall_model = wall_model;
   for (int64_t i = 0; i < o.N; ++i) o.geo[i] = (geo && geo[i]) ? 1 : 0;
   classify_nodes(o);
+  return 0;
+}
+
+// D:R22.  Density of the FACE_PRESSURE faces (6 values; entries of other faces are ignored).
+void orc_set_face_rho(void* h, const double* rho6) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int k = 0; k < 6; ++k) o.face_rho[k] = rho6[k];
+}
+
+// D:R22.  Per-cell wall velocity of MOVING face `face`: u[c*n + j], n = cells of the face, j over the two
+// in-face coordinates (lower axis fastest); NULL restores the uniform face_u.
+int orc_set_face_velocity(void* h, int face, const double* u) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (face < 0 || face > 5) return -1;
+  const int axis = face / 2;
+  const int64_t n = axis == 0 ? (int64_t)o.ny * o.nz : axis == 1 ? (int64_t)o.nx * o.nz : (int64_t)o.nx * o.ny;
+  if (u) o.face_profile[face].assign(u, u + 3 * n);
+  else o.face_profile[face].clear();
   return 0;
 }
 

@@ -92,5 +92,5 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
 
 if __name__ == "__main__":
     args = sys.argv[1:]
-    extra = ["-Xptxas", "-v"] if "--ptxas" in args else []
+    extra = (["-Xptxas", "-v"] if "--ptxas" in args else []) + [a for a in args if a.startswith("-D")]
     print(build(force="--force" in args or bool(extra), verbose=True, extra=extra))

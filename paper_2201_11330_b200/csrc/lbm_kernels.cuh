@@ -66,8 +66,13 @@ __device__ __forceinline__ void static_for(F&& f) {
 // Measured on B200: the A/B D3Q19 kernels fit 80 registers without spilling and need the third block;
 // the fp32-storage A/B kernel keeps its populations packed (collide_shifted) and fits 64 registers, which
 // buys the fourth block its half-size loads need; the forced and in-place variants and D3Q27 spill below 128.
+#ifdef LBM_MB_OVERRIDE  // tuning hook for occupancy sweeps (python -m paper_2201_11330_b200.build --force -DLBM_MB_OVERRIDE=n)
+template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
+constexpr int kMinBlocks = LBM_MB_OVERRIDE;
+#else
 template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
 constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 27 && STBYTES == 4 && !INPLACE) ? 3 : (Q == 19 && STBYTES == 4 && !INPLACE) ? (FORCE ? 3 : 4) : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
+#endif
 
 // ---------------------------------------------------------------------------------------
 // How a cell finds out that a link has no upstream node (template parameter BC):

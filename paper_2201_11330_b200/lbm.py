@@ -21,7 +21,8 @@ LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING = 0, 1, 2
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
 
-LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
+# LBM_B200_LIB points at another build of the same library (occupancy sweeps); it must exist just the same
+LIB_PATH = os.environ.get("LBM_B200_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (

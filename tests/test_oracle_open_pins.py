@@ -1,0 +1,228 @@
+"""Pins of the oracle's open boundaries (R22): FACE_PRESSURE (anti-bounce-back at a prescribed density)
+and FACE_MOVING with a per-cell wall-velocity profile (velocity bounce-back inlet).  The paper names a parabolic
+inlet and an outflow for its channel-cylinder example without formulae; these are the link-wise rules
+chosen from the literature.  Pinned by what the mathematics fixes, not by the oracle itself:
+
+  * an independent long-double gather on a tiny grid, written here from the formulae of R22 (every mix of
+    PRESSURE / MOVING-with-profile / BOUNCE / periodic faces, corners included: precedence MOVING > BOUNCE > PRESSURE);
+  * pressure-driven Poiseuille flow between two PRESSURE faces: the closed-form parabola (+ BGK halfway-wall slip)
+    for the pressure gradient c_s^2 (rho_in - rho_out)/L, and a linear pressure drop;
+  * parabolic inlet + pressure outlet: the prescribed volume flux arrives at every cross-section.
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle, lattice
+from oracle.binding import EQ_INCOMP, EQ_STANDARD
+
+P, B, M, PR = 0, 1, 2, 3
+
+
+# --------------------------------------------------------------------------- brute force
+def _face_cells(face, dims):
+    nx, ny, nz = dims
+    return [ny * nz, ny * nz, nx * nz, nx * nz, nx * ny, nx * ny][face]
+
+
+def _profile_index(face, c, dims):
+    nx, ny, nz = dims
+    x, y, z = c
+    return [y + ny * z, y + ny * z, x + nx * z, x + nx * z, x + nx * y, x + nx * y][face]
+
+
+def _brute_step(f, dims, E, T, omega, fk, fu, prof, frho, eq):
+    """One collide + stream step with open faces, long double, from Eq. 2/5, 6, 7, 10 and R6 / R22."""
+    LD = np.longdouble
+    Q = len(E)
+    post, rho_c, u_c = {}, {}, {}
+    for c, fc in f.items():
+        rho = sum(fc, LD(0))
+        m = [sum((LD(E[a][d]) * fc[a] for a in range(Q)), LD(0)) for d in range(3)]
+        div = rho if eq == EQ_STANDARD else LD(1)
+        u = [m[d] / div for d in range(3)]
+        usq = sum(v * v for v in u)
+        out = []
+        for a in range(Q):
+            eu = sum(E[a][d] * u[d] for d in range(3))
+            poly = 3 * eu + LD(9) / 2 * eu * eu - LD(3) / 2 * usq
+            fe = LD(T[a]) * (rho * (1 + poly) if eq == EQ_STANDARD else rho + poly)
+            out.append(fc[a] - LD(omega) * (fc[a] - fe))
+        post[c], rho_c[c], u_c[c] = out, (rho if eq == EQ_STANDARD else LD(1)), u
+    new = {}
+    for c in f:
+        vals = []
+        for a in range(Q):
+            src, crossed = [], []
+            for d in range(3):
+                s = c[d] - E[a][d]
+                if s < 0 or s >= dims[d]:
+                    face = 2 * d + (0 if s < 0 else 1)
+                    if fk[face] == P:
+                        s %= dims[d]
+                    else:
+                        crossed.append(face)
+                src.append(s)
+            if not crossed:
+                vals.append(post[tuple(src)][a])
+                continue
+            v = post[c][Q - 1 - a]
+            moving = [k for k in crossed if fk[k] == M]
+            bounce = [k for k in crossed if fk[k] == B]
+            press = [k for k in crossed if fk[k] == PR]
+            if moving:
+                k = max(moving)
+                uw = [LD(prof[k][d][_profile_index(k, c, dims)]) for d in range(3)] if k in prof else [LD(fu[k][d]) for d in range(3)]
+                v = v + 6 * LD(T[a]) * rho_c[c] * sum(E[a][d] * uw[d] for d in range(3))
+            elif not bounce and press:
+                k = max(press)
+                u = u_c[c]
+                eu = sum(E[a][d] * u[d] for d in range(3))
+                usq = sum(x * x for x in u)
+                even = LD(9) / 2 * eu * eu - LD(3) / 2 * usq
+                fe = LD(T[a]) * (LD(frho[k]) * (1 + even) if eq == EQ_STANDARD else LD(frho[k]) + even)
+                v = -v + 2 * fe
+            vals.append(v)
+        new[c] = vals
+    return new
+
+
+_CASES = [
+    ("inlet_outlet_x_walls_y", [M, PR, B, B, P, P]),
+    ("pressure_both_x_periodic", [PR, PR, P, P, P, P]),
+    ("pressure_everywhere", [PR] * 6),
+    ("all_kinds", [M, PR, PR, B, B, M]),
+    ("pressure_z_moving_y", [P, P, M, M, PR, PR]),
+]
+
+
+@pytest.mark.parametrize("name,fk", _CASES, ids=[c[0] for c in _CASES])
+@pytest.mark.parametrize("Q,eq", [(19, EQ_STANDARD), (19, EQ_INCOMP), (27, EQ_STANDARD), (9, EQ_INCOMP)])
+def test_brute_force_open_faces(name, fk, Q, eq):
+    dims = (4, 5, 3)
+    nx, ny, nz = dims
+    N = nx * ny * nz
+    if Q == 9 and (fk[4] != P or fk[5] != P):
+        fk = fk[:4] + [P, P]  # D2Q9 has no z links; keep z periodic
+    E, T = lattice(Q)
+    E = [tuple(int(v) for v in row) for row in E]
+    rng = np.random.default_rng(11 + Q)
+    f0 = (1.0 / Q) * (1.0 + 0.2 * rng.uniform(-1, 1, (Q, N)))
+    fu = np.zeros((6, 3))
+    frho = np.array([1.0, 0.97, 1.02, 0.99, 1.01, 0.98])
+    prof = {}
+    for k in range(6):
+        if fk[k] == M:
+            fu[k] = (0.01 * (k + 1), -0.015, 0.004 * k)
+            if k % 2 == 0:  # even MOVING faces get a per-cell profile, odd ones keep the uniform velocity
+                prof[k] = 0.03 * rng.uniform(-1, 1, (3, _face_cells(k, dims)))
+    tau = 0.77
+    o = Oracle(nx, ny, nz, Q, tau, eq=eq, face_kind=fk, face_u=fu, face_rho=frho)
+    for k, pr in prof.items():
+        o.set_face_velocity(k, pr)
+    o.set_f(f0)
+    cells = [(x, y, z) for z in range(nz) for y in range(ny) for x in range(nx)]
+    f = {c: [np.longdouble(f0[a, c[0] + nx * (c[1] + ny * c[2])]) for a in range(Q)] for c in cells}
+    for _ in range(3):
+        f = _brute_step(f, dims, E, T, 1.0 / tau, fk, fu, prof, frho, eq)
+    o.step(3)
+    got = o.get_f()
+    o.close()
+    ref = np.array([[float(f[c][a]) for c in cells] for a in range(Q)])
+    assert np.abs(got - ref).max() <= 1e-15
+
+
+def test_profile_can_be_removed_again():
+    fk = [M, M, P, P, P, P]
+    fu = np.zeros((6, 3))
+    fu[0] = fu[1] = (0.02, 0.0, 0.0)
+    a = Oracle(4, 3, 2, 19, 0.8, face_kind=fk, face_u=fu)
+    b = Oracle(4, 3, 2, 19, 0.8, face_kind=fk, face_u=fu)
+    b.set_face_velocity(0, np.full((3, 6), 0.5))
+    b.set_face_velocity(0, None)
+    for o in (a, b):
+        o.init_equilibrium()
+        o.step(4)
+    assert np.array_equal(a.get_f(), b.get_f())
+    a.close()
+    b.close()
+
+
+# --------------------------------------------------------------------------- closed forms
+def _slip_parabola(H, G, nu, tau):
+    """Steady profile between halfway bounce-back walls at distance H driven by G = -dp/dx (BGK): the parabola
+    plus the wall-slip constant, at the node positions k + 1/2 (same closed form as the body-forced channel pin)."""
+    y = np.arange(H) + 0.5
+    lam = (tau - 0.5) ** 2
+    return G / (2 * nu) * (y * (H - y) + 4 * lam / 3 - 0.25)
+
+
+def _pressure_channel(Q, nx, H, tau, d, steps):
+    fk = [PR, PR, B, B, P, P]
+    frho = [1.0 + d, 1.0 - d, 1, 1, 1, 1]
+    nz = 1 if Q == 9 else 2
+    o = Oracle(nx, H, nz, Q, tau, eq=EQ_INCOMP, face_kind=fk, face_rho=frho)
+    o.init_equilibrium()
+    o.step(steps)
+    rho, u, _ = o.moments(True)
+    o.close()
+    return rho.reshape(nz, H, nx)[0], u[0].reshape(nz, H, nx)[0], u[1].reshape(nz, H, nx)[0]
+
+
+@pytest.mark.parametrize("Q", [9, 19])
+def test_pressure_driven_poiseuille(Q):
+    """Two PRESSURE faces half a link outside the first / last node (distance L = nx) at densities 1 +- d, walls in
+    y (D2Q9 lives in the x-y plane), Eq. 5.  Away from the faces the flow is the Poiseuille solution for the
+    pressure gradient G = c_s^2 * 2d / L: the profile has exactly the shape of the slip parabola, the pressure is
+    linear with exactly that slope, and the flux matches the closed form up to the entrance-length effect of the
+    local anti-bounce-back rule (u_w = u of the boundary cell), which is O(H/L): measured 0.10 H/L, halving
+    when L doubles.  A wrong factor in the rule (2, c_s^2, the sign of f*, rho_face) misses by >= 50 %."""
+    H, tau, d = 9, 0.9, 2e-4
+    nu = (tau - 0.5) / 3.0
+    excess = []
+    for nx in (48, 96):
+        r, ux, uy = _pressure_channel(Q, nx, H, tau, d, 12000)
+        G = (2 * d / 3.0) / nx
+        ref = _slip_parabola(H, G, nu, tau)
+        mid = ux[:, nx // 2]
+        ratio = mid.sum() / ref.sum()
+        excess.append(ratio - 1.0)
+        assert 0.0 < ratio - 1.0 <= 0.15 * H / nx
+        assert np.abs(mid / ratio - ref).max() <= 1e-6 * ref.max()       # shape: parabola + BGK slip constant
+        assert np.abs(uy[:, nx // 2]).max() <= 1e-9 * ref.max()
+        # developed region: the pressure is linear with slope -2d/nx * ratio on every row
+        xs = np.arange(nx // 4, 3 * nx // 4)
+        slope = np.polyfit(xs, r[:, xs].mean(axis=0), 1)[0]
+        assert abs(slope / (-2 * d / nx) - ratio) <= 1e-4
+        assert np.abs(r[:, xs] - r[:, xs].mean(axis=0)[None, :]).max() <= 1e-5 * d  # uniform across the channel
+    assert excess[0] / excess[1] == pytest.approx(2.0, rel=0.1)
+
+
+def test_parabolic_inlet_delivers_its_flux():
+    """MOVING x- face with a parabolic profile (velocity bounce-back) + PRESSURE x+ face, walls in y, Eq. 5:
+    at steady state every cross-section carries the prescribed volume flux, the profile far from the inlet is the
+    Poiseuille parabola of that flux, and the y-velocity vanishes there."""
+    nx, H, tau, U = 48, 16, 0.8, 0.02
+    y = np.arange(H) + 0.5
+    uin = 4 * U * y * (H - y) / H ** 2
+    prof = np.zeros((3, H))
+    prof[0] = uin
+    fk = [M, PR, B, B, P, P]
+    o = Oracle(nx, H, 1, 9, tau, eq=EQ_INCOMP, face_kind=fk, face_rho=[1] * 6)
+    o.set_face_velocity(0, prof)
+    rho0 = np.ones(nx * H)
+    u0 = np.zeros((3, nx * H))
+    u0[0] = np.tile(uin[:, None], (1, nx)).reshape(-1)
+    o.init_equilibrium(rho0, u0)
+    o.step(20000)
+    _, u, _ = o.moments(True)
+    o.close()
+    ux = u[0].reshape(H, nx)
+    uy = u[1].reshape(H, nx)
+    flux = ux.sum(axis=0)
+    assert np.abs(flux / uin.sum() - 1).max() <= 2e-3          # every section carries the inlet flux
+    assert np.abs(flux[5:] / flux[5:].mean() - 1).max() <= 1e-5  # and the same one (continuity)
+    mid = ux[:, nx // 2]
+    # developed profile = slip parabola carrying the same flux
+    shape = _slip_parabola(H, 1.0, 1.0, tau)
+    assert np.abs(mid - shape * (mid.sum() / shape.sum())).max() <= 1e-4 * U
+    assert np.abs(uy[:, nx // 2]).max() <= 1e-5 * U
