@@ -117,6 +117,18 @@ def ncu_traffic(workload_name: str, scheme: str):
     return None
 
 
+def lattice_name(Q):
+    return "D2Q9" if Q == 9 else f"D3Q{Q}"
+
+
+def l2_note(touched_bytes):
+    """Timing rule: inputs larger than L2, or say that they are not (small configs are L2-resident by nature)."""
+    gb = touched_bytes / 1e9
+    if touched_bytes > 4 * 126e6:
+        return f"inputs larger than L2: {gb:.2f} GB touched per step vs 126 MB L2"
+    return f"NOT larger than L2: {gb:.3f} GB touched per step vs 126 MB L2 (no flush; not a roofline statement)"
+
+
 def pick_sample(w, target_cells):
     """A reduced copy of workload w (same tau, fields recipe, walls, force, geometry) with at most target_cells
     cells: every length halved until it fits."""
@@ -131,9 +143,12 @@ def oracle_mlups(ws, steps, warmup=1, budget_s=None):
     number of steps that fills about budget_s seconds, estimated from the warm-up step(s)."""
     from oracle import Oracle, num_threads
     rho, u = ws.fields()
-    o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, eq=ws.eq, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force)
+    o = Oracle(ws.nx, ws.ny, ws.nz, ws.Q, ws.tau, eq=ws.eq, face_kind=ws.face_kind, face_u=ws.face_u, force=ws.force,
+               face_rho=ws.face_rho)
     if ws.has_geometry:
         o.set_geometry(ws.geo(), ws.wall_model)
+    for face, prof in ws.face_profiles().items():
+        o.set_face_velocity(face, prof)
     o.init_equilibrium(rho, u)
     t0 = time.perf_counter()
     o.step(warmup)
@@ -162,7 +177,7 @@ def run_reference(args, w):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "tau": w.tau,
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": lattice_name(w.Q), "tau": w.tau,
                    "reference": "CPU oracle (oracle/lbm_oracle.cpp), host cores only"},
         "cpu_baseline": {"value": value, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -254,11 +269,11 @@ def run_gpu(args, w):
         "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "collision": "BGK", "tau": w.tau,
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": lattice_name(w.Q), "collision": "BGK", "tau": w.tau,
                    "equilibrium": "Eq. 5" if w.eq else "Eq. 2", "geometry": ("none" if not w.has_geometry else
                                                                               ("nodal" if w.wall_model else "halfway") + " walls, solid mask"),
                    "scheme": args.scheme, "storage": args.store, "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
-                   "l2": f"inputs larger than L2: {bytes_per_cell * w.N / 1e9:.2f} GB touched per step vs 126 MB L2"},
+                   "l2": l2_note(bytes_per_cell * w.N)},
         "clocks": clocks,
         "e2e": {"value": e2e_ups / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 32 * w.N / K, "d2h_bytes_per_step": (32 * w.N + 64) / K,
                 "what": "lbm_init_equilibrium_host(pinned rho,u) + lbm_step(K) + lbm_moments_host(pinned rho,u,diagnostics), host wall clock",
@@ -367,11 +382,11 @@ def run_gpu_slabs(args, w):
         "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": f"D3Q{w.Q}", "collision": "BGK", "tau": w.tau,
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": lattice_name(w.Q), "collision": "BGK", "tau": w.tau,
                    "scheme": "ab", "storage": args.store,
                    "parallelism": f"z-slabs: {nslabs} slab(s) on {world} GPU(s), fused halo push over peer memory",
                    "halo_bytes_per_step_per_cut": 2 * halo_dirs * w.nx * w.ny * (4 if args.store == "f32" else 8),
-                   "l2": f"inputs larger than L2: {bytes_per_cell * w.N / 1e9:.2f} GB touched per step vs 126 MB L2"},
+                   "l2": l2_note(bytes_per_cell * w.N)},
         "clocks": clocks, "e2e": None, "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "kernel": "stream_collide_ab<..., SLAB>", "bytes_per_cell_update": bytes_per_cell, "peak_source": peak_src,

@@ -56,7 +56,7 @@ enum {
   LBM_STORE_F32 = 1 << 16   /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
 };
 
-enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2 };
+enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2, LBM_FACE_PRESSURE = 3 };
 
 /* Wall model of lbm_set_geometry (D:R3, D:R16, D:R17). */
 enum {
@@ -76,7 +76,13 @@ enum {
  * LBM_FACE_PERIODIC must be set on both faces of an axis or on neither.  BOUNCE = halfway
  * bounce-back wall at rest, half a cell outside the first/last node.  MOVING = the same wall
  * moving with face_u (Ladd): a wall link a gains 6 t_a rho_w (e_a . u_w); at edges a MOVING face
- * takes precedence over BOUNCE, and among MOVING faces the highest face index wins. */
+ * takes precedence over BOUNCE, and among MOVING faces the highest face index wins.
+ * Open boundaries (D:R22; the paper names a parabolic inlet and an outflow, without formulae):
+ *   inlet  = MOVING with a per-cell wall velocity (lbm_set_face_velocity): velocity bounce-back;
+ *   outlet = PRESSURE: anti-bounce-back at a prescribed density rho_f (lbm_set_face_density, default 1):
+ *            f_a(x,t+1) = -f*_abar(x,t) + 2 feq+_a(rho_f, u(x,t)), feq+ = the part of Eq. 2 / Eq. 5 even in e_a
+ *            (Eq. 2: t_a rho_f (1 + 4.5 (e_a.u)^2 - 1.5 u.u); Eq. 5: t_a (rho_f + rho0 (4.5 (e_a.u)^2 - 1.5 u.u))).
+ *   A link that leaves through several non-periodic faces: MOVING > BOUNCE > PRESSURE (highest index within a kind). */
 typedef struct {
   int32_t face_kind[6];
   double face_u[6][3]; /* read only where face_kind == LBM_FACE_MOVING                          */
@@ -106,10 +112,23 @@ void lbm_destroy(lbm_handle h);
  *              if x + e_a is active, else f*_abar(x, t) (D:R17: links inside the wall)
  * One 32-bit link mask per node is built here and read by the step kernel (+4 B per node and
  * step); (NULL, LBM_WALL_HALFWAY) returns to the mask-free analytic box.  LBM_WALL_NODAL with
- * LBM_FACE_MOVING faces returns LBM_EUNSUPPORTED.  Synchronises the stream. */
+ * LBM_FACE_MOVING or LBM_FACE_PRESSURE faces returns LBM_EUNSUPPORTED.  Synchronises the stream. */
 int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model);
 /* Same with a HOST pointer to the N mask bytes. */
 int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model);
+
+/* D:R22.  Per-cell wall velocity of MOVING face `face` (0..5 = x-,x+,y-,y+,z-,z+): u[c*n + j], c = 0,1,2, n = cells
+ * of the face, j runs over the two in-face coordinates with the lower axis fastest (x- / x+: j = y + ny*z; y- / y+:
+ * j = x + nx*z; z- / z+: j = x + nx*y).  DEVICE pointer; the library keeps its own copy.  NULL restores the uniform
+ * face_u of lbm_create.  On a z-slab handle the profile is that of the WHOLE box face (z = global plane index).
+ * LBM_EINVAL if the face is not LBM_FACE_MOVING.  Synchronises the stream. */
+int lbm_set_face_velocity(lbm_handle h, int face, const double* u);
+/* Same with a HOST pointer. */
+int lbm_set_face_velocity_host(lbm_handle h, int face, const double* u_host);
+
+/* D:R22.  Density prescribed on the LBM_FACE_PRESSURE faces: rho6 = HOST pointer to 6 doubles in face order (entries
+ * of other faces are ignored).  Default 1.  Takes effect from the next lbm_step. */
+int lbm_set_face_density(lbm_handle h, const double* rho6);
 
 /* Momentum-exchange force on the solid nodes of geo (Eq. 13) for the last step taken:
  *   F = sum over fluid nodes x, over a with x + e_a a solid node of geo (inside the box):

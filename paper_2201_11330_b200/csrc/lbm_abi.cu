@@ -299,8 +299,8 @@ int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
   if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
-  if (wall_model == LBM_WALL_NODAL && h->p.any_moving)
-    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING faces is not supported");
+  if (wall_model == LBM_WALL_NODAL && h->p.any_open)
+    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING / LBM_FACE_PRESSURE faces is not supported");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   if (!geo_dev && wall_model == LBM_WALL_HALFWAY) {  // back to the analytic box
     free_geometry(h);
@@ -378,16 +378,17 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   if (bc) {
     for (int k = 0; k < 6; ++k) {
       const int kind = bc->face_kind[k];
-      if (kind != LBM_FACE_PERIODIC && kind != LBM_FACE_BOUNCE && kind != LBM_FACE_MOVING) {
+      if (kind != LBM_FACE_PERIODIC && kind != LBM_FACE_BOUNCE && kind != LBM_FACE_MOVING && kind != LBM_FACE_PRESSURE) {
         delete h; fail(LBM_EINVAL, "lbm_create: unknown face kind"); return nullptr;
       }
       p.wall[k] = kind != LBM_FACE_PERIODIC;
-      p.moving[k] = kind == LBM_FACE_MOVING;
+      p.kind[k] = kind;
+      p.open[k] = kind == LBM_FACE_MOVING || kind == LBM_FACE_PRESSURE;
       for (int d = 0; d < 3; ++d) {
-        p.face_u[k][d] = p.moving[k] ? bc->face_u[k][d] : 0.0;
+        p.face_u[k][d] = kind == LBM_FACE_MOVING ? bc->face_u[k][d] : 0.0;
         if (!std::isfinite(p.face_u[k][d])) { delete h; fail(LBM_EINVAL, "lbm_create: non-finite wall velocity"); return nullptr; }
       }
-      p.any_moving |= p.moving[k];
+      p.any_open |= p.open[k];
     }
     for (int d = 0; d < 3; ++d) {
       if (p.wall[2 * d] != p.wall[2 * d + 1]) { delete h; fail(LBM_EINVAL, "lbm_create: periodic must be set on both faces of an axis"); return nullptr; }
@@ -398,6 +399,9 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   }
   p.z_lo = 0;
   p.z_hi = nz;
+  p.zg_off = 0;
+  p.nz_glob = nz;
+  for (int k = 0; k < 6; ++k) p.face_rho[k] = 1.0;
   if (slab) {
     h->slab = true;
     h->z0 = z0; h->nz_global = nz_global; h->nz_local = nz - 2;
@@ -407,10 +411,12 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
     p.z_hi = nz - 1;
     // the z faces of the box act only on the slab that owns them; elsewhere the cut is an ordinary interior plane
     const bool owns_lo = z0 == 0, owns_hi = z0 + h->nz_local == nz_global;
-    if (!owns_lo) { p.wall[4] = 0; p.moving[4] = 0; }
-    if (!owns_hi) { p.wall[5] = 0; p.moving[5] = 0; }
-    p.any_moving = 0;
-    for (int k = 0; k < 6; ++k) p.any_moving |= p.moving[k];
+    if (!owns_lo) { p.wall[4] = 0; p.open[4] = 0; p.kind[4] = LBM_FACE_PERIODIC; }
+    if (!owns_hi) { p.wall[5] = 0; p.open[5] = 0; p.kind[5] = LBM_FACE_PERIODIC; }
+    p.any_open = 0;
+    for (int k = 0; k < 6; ++k) p.any_open |= p.open[k];
+    p.zg_off = z0 - 1;
+    p.nz_glob = nz_global;
   }
   // (walls: the coordinate-test kernels are needed if ANY face of this handle is a wall)
   h->walls = p.wall[0] || p.wall[1] || p.wall[2] || p.wall[3] || p.wall[4] || p.wall[5];
@@ -569,9 +575,59 @@ void lbm_destroy(lbm_handle h) {
   if (h->diag_dev) cudaFree(h->diag_dev);
   if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
   if (h->scratch) cudaFree(h->scratch);
+  for (int k = 0; k < 6; ++k)
+    if (h->p.face_prof[k]) cudaFree((void*)h->p.face_prof[k]);
   free_geometry(h);
   cudaGetLastError();
   delete h;
+}
+
+// cells of face `face` of the WHOLE box (a slab handle takes the profile of the whole face)
+static long long face_cells(const lbm_handle_s* h, int face) {
+  const long long nzg = h->slab ? h->nz_global : h->nz;
+  return face < 2 ? (long long)h->ny * nzg : face < 4 ? (long long)h->nx * nzg : (long long)h->nx * h->ny;
+}
+
+static int set_face_velocity_impl(lbm_handle h, int face, const double* u, cudaMemcpyKind kind, const char* who) {
+  if (!h) return fail(LBM_EINVAL, std::string(who) + ": NULL handle");
+  if (face < 0 || face > 5) return fail(LBM_EINVAL, std::string(who) + ": face must be 0..5");
+  // the kind the caller gave the face of the box (a slab that does not own a z face still accepts its profile)
+  const bool owns = !(h->slab && face >= 4 && h->p.kind[face] == LBM_FACE_PERIODIC);
+  if (owns && h->p.kind[face] != LBM_FACE_MOVING) return fail(LBM_EINVAL, std::string(who) + ": the face is not LBM_FACE_MOVING");
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (!u) {
+    if (h->p.face_prof[face]) cudaFree((void*)h->p.face_prof[face]);
+    h->p.face_prof[face] = nullptr;
+    return LBM_OK;
+  }
+  const size_t bytes = (size_t)face_cells(h, face) * 3 * sizeof(double);
+  double* dst = (double*)h->p.face_prof[face];
+  if (!dst) {
+    if (cudaMalloc((void**)&dst, bytes) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(LBM_ENOMEM, std::string(who) + ": out of device memory for the face profile");
+    }
+    h->p.face_prof[face] = dst;
+  }
+  CUDA_TRY(cudaMemcpyAsync(dst, u, bytes, kind, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBM_OK;
+}
+
+int lbm_set_face_velocity(lbm_handle h, int face, const double* u) {
+  return set_face_velocity_impl(h, face, u, cudaMemcpyDeviceToDevice, "lbm_set_face_velocity");
+}
+
+int lbm_set_face_velocity_host(lbm_handle h, int face, const double* u_host) {
+  return set_face_velocity_impl(h, face, u_host, cudaMemcpyHostToDevice, "lbm_set_face_velocity_host");
+}
+
+int lbm_set_face_density(lbm_handle h, const double* rho6) {
+  if (!h || !rho6) return fail(LBM_EINVAL, "lbm_set_face_density: NULL argument");
+  for (int k = 0; k < 6; ++k)
+    if (!std::isfinite(rho6[k])) return fail(LBM_EINVAL, "lbm_set_face_density: non-finite density");
+  for (int k = 0; k < 6; ++k) h->p.face_rho[k] = rho6[k];  // read by the kernels launched from now on
+  return LBM_OK;
 }
 
 int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model) {
@@ -585,8 +641,8 @@ int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model)
   if (!geo_host) return do_set_geometry(h, nullptr, wall_model);
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
-  if (wall_model == LBM_WALL_NODAL && h->p.any_moving)
-    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING faces is not supported");
+  if (wall_model == LBM_WALL_NODAL && h->p.any_open)
+    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING / LBM_FACE_PRESSURE faces is not supported");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   {
     int rc = alloc_geometry(h);

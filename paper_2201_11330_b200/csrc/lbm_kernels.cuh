@@ -87,10 +87,16 @@ struct Params {
   long long N;          // cells = plane stride of the SoA layout (64-bit: 512^3*19 > 2^31)
   double omega;         // 1/tau (D:R1)
   double F[3];          // body force (D:R7)
-  int wall[6];          // face is non-periodic (BOUNCE or MOVING), order x-,x+,y-,y+,z-,z+
-  int moving[6];        // face is MOVING
-  double face_u[6][3];  // wall velocity of MOVING faces
-  int any_moving;
+  int wall[6];          // face is non-periodic (BOUNCE, MOVING or PRESSURE), order x-,x+,y-,y+,z-,z+
+  int kind[6];          // FACE_PERIODIC / FACE_BOUNCE / FACE_MOVING / FACE_PRESSURE
+  int open[6];          // face is MOVING or PRESSURE: a wall link through it changes the bounced value (D:R6, D:R22)
+  double face_u[6][3];  // wall velocity of MOVING faces (uniform part)
+  // D:R22: optional per-cell wall velocity of a MOVING face (velocity inlet), u[c*n + j], j over the two in-face
+  // coordinates (lower axis fastest; z is the GLOBAL plane index), n = cells of the face; NULL = uniform face_u
+  const double* face_prof[6];
+  double face_rho[6];   // D:R22: density prescribed on PRESSURE faces (anti-bounce-back)
+  int any_open;
+  int zg_off, nz_glob;  // global plane index of local plane z = z + zg_off; planes of the whole box (slabs: D:R21)
   // BC_GEO only (D:R16): bit a (a != rest) of links[i]: node i - e_a is not an active node (solid,
   // or beyond a non-periodic face); bit `rest`: node i itself is inactive.
   const uint32_t* links;
@@ -111,6 +117,7 @@ struct Params {
 };
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
+enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3 };
 
 // Position of a cell relative to the non-periodic faces, and (BC_GEO) its link mask.
 template <int BC>
@@ -278,6 +285,91 @@ __device__ __forceinline__ void equilibrium(double (&feq)[Q], double rho, double
   });
 }
 
+// Faces that change the value a wall link bounces back (D:R6 Ladd moving wall; D:R22 velocity inlet and pressure
+// outlet).  Both rules are folded in on the collide side, while rho and u of time t are live: the slot an outgoing
+// wall link b of cell x would have streamed into is read by nobody but x's own bounce-back along a = opp(b) one
+// step later, so the cell stores there what that bounce-back must return:
+//   MOVING   f_a(x,t+1) = f*_b(x,t) + 6 t_a rho_w (e_a.u_w) = f*_b - 6 t_b rho_w (e_b.u_w),  u_w uniform or per cell
+//   PRESSURE f_a(x,t+1) = -f*_b(x,t) + 2 feq+_b(rho_face, u(x,t)),  feq+ = the part of Eq. 2 / Eq. 5 even in e
+// Precedence when x + e_b lies beyond several non-periodic faces: MOVING (highest face index) > BOUNCE > PRESSURE
+// (highest face index).  `touches_open` keeps the per-direction tests off every cell not next to such a face.
+template <int BC>
+__device__ __forceinline__ bool touches_open(const Params& p, const CellFlags<BC>& c) {
+  if constexpr (BC == BC_PERIODIC) return false;
+  if (!p.any_open) return false;
+  return (c.lo[0] && p.open[0]) || (c.hi[0] && p.open[1]) || (c.lo[1] && p.open[2]) || (c.hi[1] && p.open[3]) ||
+         (c.lo[2] && p.open[4]) || (c.hi[2] && p.open[5]);
+}
+
+struct CellState {  // what the open faces need from the collision of this cell
+  double rw;              // rho(x,t) under Eq. 2, rho0 = 1 under Eq. 5
+  double ux, uy, uz, usq15;
+  int ic, z;              // in-plane index and (local) plane of the cell
+};
+
+// v = post-collision value of outgoing direction B (in the stored variable: f*, or f* - t_B if SHIFTED);
+// returns what the slot must hold.
+template <int Q, int EQ, int BC, int B, bool SHIFTED>
+__device__ __forceinline__ double open_link(double v, const Params& p, const CellFlags<BC>& c, const CellState& s) {
+  using D = Dir<Q, B>;
+  if constexpr (BC == BC_PERIODIC || D::s == 0) {
+    return v;
+  } else {
+    int mface = -1, pface = -1;
+    bool bounce = false;
+    auto crossed = [&](int face) {
+      const int k = p.kind[face];
+      if (k == FACE_MOVING) mface = face;
+      else if (k == FACE_PRESSURE) pface = face;
+      else bounce = true;
+    };
+    // x, then y, then z: the highest face index crossed wins within a kind
+    if constexpr (D::ex != 0) {
+      if (D::ex == 1 ? c.hi[0] : c.lo[0]) crossed(D::ex == 1 ? 1 : 0);
+    }
+    if constexpr (D::ey != 0) {
+      if (D::ey == 1 ? c.hi[1] : c.lo[1]) crossed(D::ey == 1 ? 3 : 2);
+    }
+    if constexpr (D::ez != 0) {
+      if (D::ez == 1 ? c.hi[2] : c.lo[2]) crossed(D::ez == 1 ? 5 : 4);
+    }
+    if (mface >= 0) {
+      double wx = p.face_u[mface][0], wy = p.face_u[mface][1], wz = p.face_u[mface][2];
+      const double* prof = p.face_prof[mface];
+      if (prof) {
+        // in-face index of the cell from its in-plane index: the face fixes one coordinate
+        const int axis = mface >> 1, side = mface & 1;
+        const int zg = s.z + p.zg_off;
+        long long j, n;
+        if (axis == 0) {        // j = y + ny*zg
+          const int xf = side ? p.nx - 1 : 0;
+          j = (s.ic - xf) / p.nx + (long long)p.ny * p.zg_off;
+          n = (long long)p.ny * p.nz_glob;
+        } else if (axis == 1) { // j = x + nx*zg
+          const int yf = side ? p.ny - 1 : 0;
+          j = (long long)(s.ic - p.nx * yf - p.nx * p.ny * s.z) + (long long)p.nx * zg;
+          n = (long long)p.nx * p.nz_glob;
+        } else {                // j = x + nx*y
+          j = s.ic - p.nx * p.ny * s.z;
+          n = (long long)p.nx * p.ny;
+        }
+        wx = __ldg(prof + j); wy = __ldg(prof + n + j); wz = __ldg(prof + 2 * n + j);
+      }
+      return v - (6.0 * D::t) * s.rw * edot<Q, B>(wx, wy, wz);
+    }
+    if (pface >= 0 && !bounce) {
+      const double eu = edot<Q, B>(s.ux, s.uy, s.uz);
+      const double rf = p.face_rho[pface];
+      const double poly = fma(4.5 * eu, eu, -s.usq15);
+      // Eq. 2: t rf (1 + poly);  Eq. 5: t (rf + rho0 poly);  SHIFTED: minus t_B for the stored variable
+      double even = (EQ == EQ_STANDARD) ? fma(rf, poly, rf) : rf + poly;
+      if constexpr (SHIFTED) even -= 1.0;
+      return fma(2.0 * D::t, even, -v);
+    }
+    return v;
+  }
+}
+
 // BGK relaxation, Eq. 6: f* = f - omega (f - feq), plus Guo's source (D:R7)
 //   S_a = (1 - omega/2) t_a [3 (e_a - u) + 9 (e_a.u) e_a] . F
 // and, on cells touching a MOVING face, the Ladd term folded into the outgoing wall links
@@ -285,7 +377,7 @@ __device__ __forceinline__ void equilibrium(double (&feq)[Q], double rho, double
 // bounce-back read f_bbar(x, t+1) = stored_b(x) turns into f*_b + 6 t_bbar rho_w (e_bbar . u_w).
 // f is replaced by the post-collision populations.
 template <int Q, int EQ, int BC, bool FORCE>
-__device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const CellFlags<BC>& c) {
+__device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const CellFlags<BC>& c, int ic, int z) {
   double rho, ux, uy, uz;
   moments<Q, EQ, FORCE>(f, p, rho, ux, uy, uz);
   const double om = p.omega, om1 = 1.0 - p.omega;
@@ -318,37 +410,36 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
     }
   });
   if constexpr (BC != BC_PERIODIC) {
-    if (p.any_moving) {
-      // moving face crossed by a link leaving along +e on axis d: hi face (2d+1); along -e: lo face (2d)
-      const bool touch = (c.lo[0] && p.moving[0]) || (c.hi[0] && p.moving[1]) || (c.lo[1] && p.moving[2]) ||
-                         (c.hi[1] && p.moving[3]) || (c.lo[2] && p.moving[4]) || (c.hi[2] && p.moving[5]);
-      if (touch) {
-        const double rw = (EQ == EQ_STANDARD) ? rho : 1.0;
-        static_for<0, Q>([&](auto BB) {
-          constexpr int b = decltype(BB)::value;
-          using D = Dir<Q, b>;
-          if constexpr (D::s > 0) {
-            // highest-index MOVING face crossed by x + e_b: test z, then y, then x (D:R6 tie-break)
-            int face = -1;
-            if constexpr (D::ex != 0) {
-              constexpr int fx = (D::ex == 1) ? 1 : 0;
-              if ((D::ex == 1 ? c.hi[0] : c.lo[0]) && p.moving[fx]) face = fx;
-            }
-            if constexpr (D::ey != 0) {
-              constexpr int fy = (D::ey == 1) ? 3 : 2;
-              if ((D::ey == 1 ? c.hi[1] : c.lo[1]) && p.moving[fy]) face = fy;
-            }
-            if constexpr (D::ez != 0) {
-              constexpr int fz = (D::ez == 1) ? 5 : 4;
-              if ((D::ez == 1 ? c.hi[2] : c.lo[2]) && p.moving[fz]) face = fz;
-            }
-            if (face >= 0) {
-              const double euw = edot<Q, b>(p.face_u[face][0], p.face_u[face][1], p.face_u[face][2]);
-              f[b] -= (6.0 * D::t) * rw * euw;
-            }
-          }
-        });
+    if (touches_open<BC>(p, c)) {
+      // rho and u of time t are recomputed from f*: the collision conserves mass and changes sum e f by exactly F
+      // (Guo), so u = (sum e f* - F/2)/rho.  Nothing of the collision stays live across it for these few cells.
+      double r = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
+      static_for<0, Q>([&](auto BB) {
+        constexpr int b = decltype(BB)::value;
+        using D = Dir<Q, b>;
+        r += f[b];
+        if constexpr (D::ex == 1) mx += f[b];
+        if constexpr (D::ex == -1) mx -= f[b];
+        if constexpr (D::ey == 1) my += f[b];
+        if constexpr (D::ey == -1) my -= f[b];
+        if constexpr (D::ez == 1) mz += f[b];
+        if constexpr (D::ez == -1) mz -= f[b];
+      });
+      if constexpr (FORCE) {
+        mx -= 0.5 * p.F[0];
+        my -= 0.5 * p.F[1];
+        mz -= 0.5 * p.F[2];
       }
+      CellState st;
+      st.rw = (EQ == EQ_STANDARD) ? r : 1.0;
+      const double inv = (EQ == EQ_STANDARD) ? 1.0 / r : 1.0;
+      st.ux = mx * inv; st.uy = my * inv; st.uz = mz * inv;
+      st.usq15 = 1.5 * (st.ux * st.ux + st.uy * st.uy + st.uz * st.uz);
+      st.ic = ic; st.z = z;
+      static_for<0, Q>([&](auto BB) {
+        constexpr int b = decltype(BB)::value;
+        f[b] = open_link<Q, EQ, BC, b, false>(f[b], p, c, st);
+      });
     }
   }
 }
@@ -359,7 +450,7 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
 // so the populations stay packed as floats in registers until they are used, no t_a is added or subtracted and
 // the small deviations are not rounded against O(t_a).  `store(IC<a>, g*_a)` writes one result.
 template <int Q, int EQ, int BC, bool FORCE, typename StoreF>
-__device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Params& p, const CellFlags<BC>& c, StoreF&& store) {
+__device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Params& p, const CellFlags<BC>& c, int ic, int z, StoreF&& store) {
   double dr = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
   static_for<0, Q>([&](auto AA) {
     constexpr int a = decltype(AA)::value;
@@ -393,37 +484,15 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
     k = 1.0 - 0.5 * om;
     uF3 = 3.0 * (ux * p.F[0] + uy * p.F[1] + uz * p.F[2]);
   }
-  // Ladd term of an outgoing wall link b through a MOVING face (D:R6), 0 elsewhere; `touch` keeps the
-  // per-direction tests off every cell that is not next to a MOVING face
-  bool touch = false;
-  if constexpr (BC != BC_PERIODIC) {
-    if (p.any_moving)
-      touch = (c.lo[0] && p.moving[0]) || (c.hi[0] && p.moving[1]) || (c.lo[1] && p.moving[2]) || (c.hi[1] && p.moving[3]) ||
-              (c.lo[2] && p.moving[4]) || (c.hi[2] && p.moving[5]);
-  }
-  auto ladd = [&](auto BB) -> double {
+  // open faces (D:R6, D:R22): what an outgoing wall link keeps in its slot; identity on every other cell
+  const bool touch = touches_open<BC>(p, c);
+  const CellState st{A, ux, uy, uz, usq15, ic, z};
+  auto open = [&](auto BB, double v) -> double {
     constexpr int b = decltype(BB)::value;
-    using D = Dir<Q, b>;
-    double corr = 0.0;
-    if constexpr (BC != BC_PERIODIC && D::s > 0) {
-      if (touch) {
-        int face = -1;
-        if constexpr (D::ex != 0) {
-          constexpr int fx = (D::ex == 1) ? 1 : 0;
-          if ((D::ex == 1 ? c.hi[0] : c.lo[0]) && p.moving[fx]) face = fx;
-        }
-        if constexpr (D::ey != 0) {
-          constexpr int fy = (D::ey == 1) ? 3 : 2;
-          if ((D::ey == 1 ? c.hi[1] : c.lo[1]) && p.moving[fy]) face = fy;
-        }
-        if constexpr (D::ez != 0) {
-          constexpr int fz = (D::ez == 1) ? 5 : 4;
-          if ((D::ez == 1 ? c.hi[2] : c.lo[2]) && p.moving[fz]) face = fz;
-        }
-        if (face >= 0) corr = (6.0 * D::t) * A * edot<Q, b>(p.face_u[face][0], p.face_u[face][1], p.face_u[face][2]);
-      }
+    if constexpr (BC != BC_PERIODIC && Dir<Q, b>::s > 0) {
+      if (touch) return open_link<Q, EQ, BC, b, true>(v, p, c, st);
     }
-    return corr;
+    return v;
   };
   static_for<0, (Q + 1) / 2>([&](auto AA) {
     constexpr int a = decltype(AA)::value;
@@ -441,8 +510,8 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
         s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
         d = fma(3.0 * k * D::t, eF, d);
       }
-      store(IC<a>{}, fma(om1, (double)g[a], s + d) - ladd(IC<a>{}));
-      store(IC<D::opp>{}, fma(om1, (double)g[D::opp], s - d) - ladd(IC<D::opp>{}));
+      store(IC<a>{}, open(IC<a>{}, fma(om1, (double)g[a], s + d)));
+      store(IC<D::opp>{}, open(IC<D::opp>{}, fma(om1, (double)g[D::opp], s - d)));
     }
   });
 }
@@ -534,7 +603,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
     if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
     nodal_replicate<Q, BC>(g, p, c);
-    collide_shifted<Q, EQ, BC, FORCE>(g, p, c, [&](auto A, double v) {
+    collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.ic, z, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
       const float s = (float)v;
       plane<a>(dst, p.N)[nb.ic] = s;
@@ -544,7 +613,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     double f[Q];
     if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
     nodal_replicate<Q, BC>(f, p, c);
-    collide<Q, EQ, BC, FORCE>(f, p, c);
+    collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
@@ -574,7 +643,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   });
   if (!c.template active<Q>()) return;  // after the loads: they do not wait for the link mask (see gather)
   nodal_replicate<Q, BC>(f, p, c);
-  collide<Q, EQ, BC, FORCE>(f, p, c);
+  collide<Q, EQ, BC, FORCE>(f, p, c, ic, z);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     st_pop<ST, Q, a>(plane<Dir<Q, a>::opp>(buf, p.N), ic, f[a]);
@@ -595,7 +664,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   auto wall = [&](auto A) { return (const ST*)plane<decltype(A)::value>(buf, p.N) + nb.ic; };
   if (!gather<Q, BC>(f, c, link, wall, [](auto A, const ST* q) { return ld_pop_rw<ST, Q, decltype(A)::value>(q, 0); })) return;
   nodal_replicate<Q, BC>(f, p, c);
-  collide<Q, EQ, BC, FORCE>(f, p, c);
+  collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;

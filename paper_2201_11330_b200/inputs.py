@@ -13,13 +13,13 @@ Layouts: rho[i], u[c*N + i], i = x + nx*(y + ny*z).
 """
 from __future__ import annotations
 
-from dataclasses import dataclass, field
+from dataclasses import dataclass, field, replace
 
 import numpy as np
 
 SEED_BASE = 0x22011330
 
-FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING = 0, 1, 2
+FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE = 0, 1, 2, 3
 EQ_STANDARD, EQ_INCOMP = 0, 1
 WALL_HALFWAY, WALL_NODAL = 0, 1
 
@@ -110,6 +110,20 @@ def sphere_mask(nx, ny, nz, centre, radius):
     return ((x * x + y * y + z * z) <= radius * radius).astype(np.uint8).reshape(-1)
 
 
+def cylinder_mask(nx, ny, nz, centre, radius):
+    """uint8[N]: 1 where (x-cx)^2 + (y-cy)^2 <= r^2 — a z-invariant circular cylinder (Fig. 3)."""
+    x = np.arange(nx)[None, None, :] - centre[0]
+    y = np.arange(ny)[None, :, None] - centre[1]
+    m = ((x * x + y * y) <= radius * radius) & np.ones((nz, 1, 1), dtype=bool)
+    return m.astype(np.uint8).reshape(-1)
+
+
+def parabola(n, umax):
+    """Poiseuille profile between halfway walls at -1/2 and n-1/2: umax * 4 (k+1/2)(n-k-1/2)/n^2, k = 0..n-1."""
+    k = np.arange(n) + 0.5
+    return umax * 4.0 * k * (n - k) / (n * n)
+
+
 @dataclass
 class Workload:
     """One BASELINE.json config: geometry, physics parameters and how to make its fields."""
@@ -130,6 +144,9 @@ class Workload:
     eq: int = EQ_STANDARD
     wall_model: int = WALL_HALFWAY
     sphere: tuple | None = None  # (cx, cy, cz, r): nodes with |x - c| <= r are solid
+    cylinder: tuple | None = None  # (cx, cy, r): z-invariant circular cylinder
+    face_rho: tuple | None = None  # density prescribed on FACE_PRESSURE faces (6 values)
+    inlet_umax: float = 0.0  # "channel": parabolic profile u_x(y) on the x- MOVING face and as the initial field
 
     @property
     def N(self):
@@ -137,34 +154,50 @@ class Workload:
 
     @property
     def has_geometry(self):
-        return self.sphere is not None or self.wall_model != WALL_HALFWAY
+        return self.sphere is not None or self.cylinder is not None or self.wall_model != WALL_HALFWAY
 
     def geo(self):
         """Solid mask (uint8[N], 1 = solid node; the paper's `geo`) or None."""
-        if self.sphere is None:
-            return None
-        return sphere_mask(self.nx, self.ny, self.nz, self.sphere[:3], self.sphere[3])
+        if self.sphere is not None:
+            return sphere_mask(self.nx, self.ny, self.nz, self.sphere[:3], self.sphere[3])
+        if self.cylinder is not None:
+            return cylinder_mask(self.nx, self.ny, self.nz, self.cylinder[:2], self.cylinder[2])
+        return None
+
+    def face_profiles(self):
+        """{face: u[3, n]} per-cell wall velocities of MOVING faces (lower in-face axis fastest); {} = uniform."""
+        if self.kind != "channel":
+            return {}
+        prof = np.zeros((3, self.ny * self.nz))
+        prof[0] = np.tile(parabola(self.ny, self.inlet_umax), self.nz)  # j = y + ny*z
+        return {0: prof}
 
     def shrunk(self, k, steps=None):
-        """Same workload with every length (grid, sphere) divided by k."""
+        """Same workload with every length (grid, sphere, cylinder) divided by k."""
         sp = None if self.sphere is None else tuple(v / k for v in self.sphere)
-        return Workload(f"{self.name}/{k}", self.nx // k, self.ny // k, self.nz // k, self.Q, self.tau, steps or self.steps,
-                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind, self.eq,
-                        self.wall_model, sp)
+        # node j sits at j + 1/2 between the halfway walls: scale that position, not the index
+        cy = None if self.cylinder is None else ((self.cylinder[0] + 0.5) / k - 0.5, (self.cylinder[1] + 0.5) / k - 0.5, self.cylinder[2] / k)
+        return replace(self, name=f"{self.name}/{k}", nx=self.nx // k, ny=self.ny // k, nz=max(1, self.nz // k),
+                       steps=steps or self.steps, sphere=sp, cylinder=cy)
 
     def fields(self, box=None):
         """(rho[n], u[3,n]) on the full grid or on a periodically wrapped sub-box."""
         if self.kind == "tgv":
             return taylor_green(self.nx, self.ny, self.nz, self.u0, self.noise, self.seed, box)
         rho = density_noise(self.nx, self.ny, self.nz, self.noise, self.seed, box)
-        return rho, np.zeros((3, rho.size))
+        u = np.zeros((3, rho.size))
+        if self.kind == "channel":
+            # the inlet profile at every x (P:466: "steady-state inviscid flow with randomly distributed perturbation")
+            b = box or ((0, self.nx), (0, self.ny), (0, self.nz))
+            gy = _axes(self.ny, *b[1], True)
+            ux = parabola(self.ny, self.inlet_umax)[gy]
+            u[0] = np.broadcast_to(ux[None, :, None], (b[2][1] - b[2][0], gy.size, b[0][1] - b[0][0])).reshape(-1)
+        return rho, u
 
     def scaled(self, n, steps=None, name=None):
         """Same parameters on an n^3 grid (reduced analogue for oracle-affordable parity)."""
         sp = None if self.sphere is None else tuple(v * n / self.ny for v in self.sphere)
-        return Workload(name or f"{self.name}@{n}", n, n, n, self.Q, self.tau, steps or self.steps,
-                        self.face_kind, self.face_u, self.force, self.u0, self.noise, self.seed, self.kind, self.eq,
-                        self.wall_model, sp)
+        return replace(self, name=name or f"{self.name}@{n}", nx=n, ny=n, nz=n, steps=steps or self.steps, sphere=sp)
 
 
 _CAVITY_FACES = (FACE_BOUNCE,) * 5 + (FACE_MOVING,)
@@ -194,4 +227,20 @@ def config(i: int) -> Workload:
         return Workload("cfg5_q27_sphere512x128x128", 512, 128, 128, 27, 1.0 / 1.8, 6401, force=(1e-6, 0.0, 0.0),
                         noise=1e-5, seed=SEED_BASE + 6, kind="rest", eq=EQ_INCOMP, wall_model=WALL_NODAL,
                         sphere=(64.0, 64.0, 64.0, 8.0))
+    if i in (6, 7):
+        # Not in BASELINE.json: the paper's 2-D channel-cylinder example (section 4), D2Q9, Eq. 5 model.
+        #   case 1 (i = 6): 1024 x 1024, D = 32, centre 512 from the inlet, omega = 1.8,   Re = U D / nu = 20  (C_D -> 2.06)
+        #   case 2 (i = 7):  512 x  128, D = 16, centre  64 from the inlet, omega = 1.953, Re = 100            (C_D ~ 1.46)
+        # Inlet = parabolic velocity profile on x- (MOVING + per-cell wall velocity), outlet = PRESSURE rho = 1 on x+,
+        # no-slip BOUNCE walls on y-, y+ (R22: the paper gives no formulae for its inlet / outflow); U = the
+        # centreline inlet velocity (R23).  The cylinder is a solid mask with halfway bounce-back.
+        nx, ny, D, cx, omega, Re, steps = ((1024, 1024, 32.0, 512.0, 1.8, 20.0, 200000) if i == 6
+                                           else (512, 128, 16.0, 64.0, 1.953, 100.0, 100000))
+        tau = 1.0 / omega
+        nu = (tau - 0.5) / 3.0
+        U = Re * nu / D
+        return Workload(f"cfg{i}_q9_cylinder{nx}x{ny}", nx, ny, 1, 9, tau, steps,
+                        face_kind=(FACE_MOVING, FACE_PRESSURE, FACE_BOUNCE, FACE_BOUNCE, FACE_PERIODIC, FACE_PERIODIC),
+                        noise=1e-5, seed=SEED_BASE + i + 1, kind="channel", eq=EQ_INCOMP,
+                        cylinder=(cx, (ny - 1) / 2.0, D / 2.0), face_rho=(1.0,) * 6, inlet_umax=U)
     raise IndexError(i)

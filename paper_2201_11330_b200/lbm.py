@@ -17,7 +17,7 @@ LBM_D2Q9, LBM_D3Q19, LBM_D3Q27 = 9, 19, 27
 LBM_EQ_STANDARD, LBM_EQ_INCOMP = 0, 1 << 8
 LBM_SCHEME_AUTO, LBM_SCHEME_AB, LBM_SCHEME_AA = 0, 1 << 12, 2 << 12
 LBM_STORE_F64, LBM_STORE_F32 = 0, 1 << 16
-LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING = 0, 1, 2
+LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE = 0, 1, 2, 3
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
 
@@ -30,6 +30,7 @@ SYMBOLS = (
     "lbm_moments", "lbm_moments_host", "lbm_get_populations", "lbm_set_populations", "lbm_lattice",
     "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_last_error",
     "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
+    "lbm_set_face_velocity", "lbm_set_face_velocity_host", "lbm_set_face_density",
     "lbm_create_slab", "lbm_slab_export", "lbm_slab_connect", "lbm_slab_set_sync",
 )
 
@@ -105,6 +106,11 @@ def load():
         getattr(lib, name).argtypes = [vp, C.c_void_p, i32]
     lib.lbm_boundary_force.restype = i32
     lib.lbm_boundary_force.argtypes = [vp, C.c_void_p]
+    for name in ("lbm_set_face_velocity", "lbm_set_face_velocity_host"):
+        getattr(lib, name).restype = i32
+        getattr(lib, name).argtypes = [vp, i32, dp]
+    lib.lbm_set_face_density.restype = i32
+    lib.lbm_set_face_density.argtypes = [vp, C.c_void_p]
     lib.lbm_create_slab.restype = vp
     lib.lbm_create_slab.argtypes = [i32, i32, i32, i32, i32, i32, C.c_double, C.POINTER(lbm_bc_t)]
     lib.lbm_slab_export.restype = i32
@@ -212,6 +218,20 @@ def lbm_boundary_force(h):
     return F
 
 
+def lbm_set_face_velocity(h, face, u=None):
+    """u: float64 CUDA tensor [3*n] over the cells of the face (lower in-face axis fastest) or None (uniform face_u)."""
+    _check(load().lbm_set_face_velocity(h, int(face), _ptr(u)))
+
+
+def lbm_set_face_velocity_host(h, face, u=None):
+    _check(load().lbm_set_face_velocity_host(h, int(face), _ptr(u, device="cpu")))
+
+
+def lbm_set_face_density(h, rho6):
+    r = np.ascontiguousarray(rho6, dtype=np.float64).reshape(6)
+    _check(load().lbm_set_face_density(h, r.ctypes.data))
+
+
 def lbm_init_equilibrium(h, rho=None, u=None):
     _check(load().lbm_init_equilibrium(h, _ptr(rho), _ptr(u)))
 
@@ -291,6 +311,10 @@ class Solver:
         if getattr(w, "has_geometry", False):
             geo = w.geo()
             s.set_geometry(None if geo is None else torch.from_numpy(geo), w.wall_model)
+        if getattr(w, "face_rho", None) is not None:
+            s.set_face_density(w.face_rho)
+        for face, prof in getattr(w, "face_profiles", dict)().items():
+            s.set_face_velocity(face, torch.from_numpy(np.ascontiguousarray(prof).reshape(-1)))
         return s
 
     def close(self):
@@ -313,6 +337,16 @@ class Solver:
 
     def boundary_force(self):
         return lbm_boundary_force(self.h)
+
+    def set_face_velocity(self, face, u=None):
+        """Per-cell wall velocity of MOVING face `face`: float64 tensor [3*n] (CUDA or CPU) or None."""
+        if u is not None and u.device.type == "cpu":
+            lbm_set_face_velocity_host(self.h, face, u)
+        else:
+            lbm_set_face_velocity(self.h, face, u)
+
+    def set_face_density(self, rho6):
+        lbm_set_face_density(self.h, rho6)
 
     def init_equilibrium(self, rho=None, u=None):
         lbm_init_equilibrium(self.h, rho, u)

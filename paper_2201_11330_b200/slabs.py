@@ -115,6 +115,11 @@ class Slab:
         eq = lbm.LBM_EQ_INCOMP if getattr(w, "eq", 0) else lbm.LBM_EQ_STANDARD
         self.bc = lbm.make_bc(w.face_kind, w.face_u, w.force, None if stream is None else stream.cuda_stream)
         self.h = lbm.lbm_create_slab(self.nx, self.ny, self.nz_local, self.z0, w.nz, int(w.Q) | eq | scheme | store, w.tau, self.bc)
+        # open boundaries (D:R22): every slab takes the density and the per-cell velocity of the WHOLE box faces
+        if getattr(w, "face_rho", None) is not None:
+            lbm.lbm_set_face_density(self.h, w.face_rho)
+        for face, prof in getattr(w, "face_profiles", dict)().items():
+            lbm.lbm_set_face_velocity(self.h, face, torch.from_numpy(np.ascontiguousarray(prof).reshape(-1)).cuda())
 
     def descriptor(self) -> bytes:
         return bytes(lbm.lbm_slab_export(self.h))
