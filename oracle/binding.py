@@ -15,7 +15,7 @@ _lib = None
 
 EQ_STANDARD, EQ_INCOMP = 0, 1
 WALL_HALFWAY, WALL_NODAL = 0, 1
-FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE = 0, 1, 2, 3
+FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE, FACE_SYMMETRY = 0, 1, 2, 3, 4
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)

@@ -31,6 +31,13 @@
 //                               paper's own claim), wall position, mirror symmetry
 //   momentum exchange (Eq. 13)  pinned: exact momentum balance of the fluid region per step;
 //                               steady drag = total body force
+//   open faces (D:R22) ........ pinned: brute-force gather over every face mix, pressure-driven Poiseuille closed
+//                               form, inlet flux (tests/test_oracle_open_pins.py)
+//   symmetry faces (D:R25), open faces next to nodal walls (D:R24)
+//                               pinned: equality with the mirror-extended domain (one plane, two planes, an edge,
+//                               a body cut by the plane, both wall models), free slip, half channel = full channel
+//                               closed form, brute-force gather over every rule at once
+//                               (tests/test_oracle_symmetry_pins.py)
 //
 // Floating point: IEEE double throughout ("double precision"); compile with
 // -ffp-contract=off so that no FMA contraction happens.  Reductions for the
@@ -84,10 +91,12 @@ bool make_lattice(int Q, Lattice& L) {
 }
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };              // Eq. 2 | Eq. 5
-enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3 };
+enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3, FACE_SYMMETRY = 4 };
 // D:R22 (open boundaries; the paper names a parabolic inlet and an outflow, with no formulae):
 //   inlet  = FACE_MOVING with a per-cell wall velocity profile (velocity bounce-back, Ladd),
 //   outlet = FACE_PRESSURE: anti-bounce-back at the prescribed density face_rho.
+// D:R25 ("the left and right boundaries are symmetric", no formula): FACE_SYMMETRY = a mirror plane half a
+//   link beyond the last node (specular reflection, free slip).
 // D:R3 / D:R16.  HALFWAY: the wall lies half a link beyond the last fluid node (BASELINE.json
 // configs).  NODAL: the paper's "modified nodal bounce back" (Eq. 10): wall nodes lie on
 // the wall, receive f_alpha = f_abar for the directions no node streams into them, and collide.
@@ -146,32 +155,19 @@ inline void moments_of(const Oracle& o, const double* fc, double& rho, double u[
   for (int d = 0; d < 3; ++d) u[d] = (m[d] + 0.5 * o.F[d]) / div;
 }
 
-// Node x + s*e_iq with periodic wrap.  Returns false if it lies outside the box through a
-// non-periodic face; then `moving_face` is the MOVING face crossed (D:R6 tie-break: the highest
-// face index among the MOVING faces crossed) or -1, and `pressure_face` (D:R22) the PRESSURE face that
-// resolves the link: the highest-index PRESSURE face crossed, but only if the link crosses no MOVING
-// and no BOUNCE face (precedence MOVING > BOUNCE > PRESSURE), else -1.
-inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int out[3], int* moving_face,
-                      int* pressure_face = nullptr) {
+// Node x + s*e_iq with periodic wrap; false if it lies outside the box through a non-periodic face of any kind
+// (used where only nodes of the box count: node classification, D:R16, and the body force, Eq. 13).
+inline bool neighbour(const Oracle& o, int x, int y, int z, int iq, int sgn, int out[3]) {
   const int c[3] = {x, y, z}, n[3] = {o.nx, o.ny, o.nz};
-  bool inside = true, bounce = false;
-  int mf = -1, pf = -1;
+  bool inside = true;
   for (int d = 0; d < 3; ++d) {
     out[d] = c[d] + sgn * o.L.e[iq][d];
     if (out[d] < 0 || out[d] >= n[d]) {
       const int face = 2 * d + (out[d] < 0 ? 0 : 1);
-      if (o.face_kind[face] == FACE_PERIODIC) {
-        out[d] = ((out[d] % n[d]) + n[d]) % n[d];
-      } else {
-        inside = false;
-        if (o.face_kind[face] == FACE_MOVING && face > mf) mf = face;
-        if (o.face_kind[face] == FACE_BOUNCE) bounce = true;
-        if (o.face_kind[face] == FACE_PRESSURE && face > pf) pf = face;
-      }
+      if (o.face_kind[face] == FACE_PERIODIC) out[d] = ((out[d] % n[d]) + n[d]) % n[d];
+      else inside = false;
     }
   }
-  if (moving_face) *moving_face = mf;
-  if (pressure_face) *pressure_face = (mf < 0 && !bounce) ? pf : -1;
   return inside;
 }
 
@@ -190,6 +186,71 @@ inline void wall_velocity(const Oracle& o, int face, int x, int y, int z, double
   for (int d = 0; d < 3; ++d) uw[d] = o.face_profile[face][(size_t)d * n + j];
 }
 
+// Where the population that arrives at node (x,y,z) along iq comes from (sgn = -1), or where the one that leaves
+// along iq goes to (sgn = +1).  D:R6 / D:R22 / D:R24 / D:R25.  The node (x,y,z) + sgn*e_iq is wrapped on periodic
+// axes; if it lies beyond non-periodic faces the kinds of ALL faces crossed decide, in this order:
+//   any MOVING   -> LINK_MOVING   (face = the highest-index MOVING face crossed):   velocity bounce-back (Ladd)
+//   any BOUNCE   -> LINK_WALL:     a wall link (halfway bounce-back, or unknown of Eq. 10 under the nodal model)
+//   any PRESSURE -> LINK_PRESSURE (face = the highest-index PRESSURE face crossed): anti-bounce-back
+//   else (only SYMMETRY faces)     -> LINK_NODE at the mirror image: the coordinates along the crossed axes stay
+//                                    those of (x,y,z), `dir` = e_iq with those components negated.
+// LINK_NODE says nothing about the node being active: the caller checks, and treats an inactive one as LINK_WALL.
+enum { LINK_NODE = 0, LINK_WALL = 1, LINK_MOVING = 2, LINK_PRESSURE = 3 };
+struct Link {
+  int kind;
+  int node[3];
+  int dir;   // direction index the population has at `node` (LINK_NODE)
+  int face;  // LINK_MOVING / LINK_PRESSURE
+};
+
+inline int direction_index(const Lattice& L, const int e[3]) {
+  for (int iq = 0; iq < L.Q; ++iq)
+    if (L.e[iq][0] == e[0] && L.e[iq][1] == e[1] && L.e[iq][2] == e[2]) return iq;
+  return -1;
+}
+
+inline Link resolve(const Oracle& o, int x, int y, int z, int iq, int sgn) {
+  const int c[3] = {x, y, z}, n[3] = {o.nx, o.ny, o.nz};
+  Link L;
+  L.kind = LINK_NODE;
+  L.dir = iq;
+  L.face = -1;
+  bool inside = true;
+  for (int d = 0; d < 3; ++d) {
+    L.node[d] = c[d] + sgn * o.L.e[iq][d];
+    inside = inside && L.node[d] >= 0 && L.node[d] < n[d];
+  }
+  if (inside) return L;  // the bulk of the nodes
+  int mf = -1, pf = -1, e2[3];
+  bool bounce = false, sym = false;
+  for (int d = 0; d < 3; ++d) {
+    e2[d] = o.L.e[iq][d];
+    if (L.node[d] < 0 || L.node[d] >= n[d]) {
+      const int face = 2 * d + (L.node[d] < 0 ? 0 : 1);
+      switch (o.face_kind[face]) {
+        case FACE_PERIODIC: L.node[d] = ((L.node[d] % n[d]) + n[d]) % n[d]; break;
+        case FACE_MOVING: if (face > mf) mf = face; break;
+        case FACE_BOUNCE: bounce = true; break;
+        case FACE_PRESSURE: if (face > pf) pf = face; break;
+        default:  // FACE_SYMMETRY: mirror image
+          sym = true;
+          L.node[d] = c[d];
+          e2[d] = -e2[d];
+          break;
+      }
+    }
+  }
+  if (mf >= 0) { L.kind = LINK_MOVING; L.face = mf; }
+  else if (bounce) L.kind = LINK_WALL;
+  else if (pf >= 0) { L.kind = LINK_PRESSURE; L.face = pf; }
+  else if (sym) L.dir = direction_index(o.L, e2);
+  return L;
+}
+
+inline bool link_has_active_node(const Oracle& o, const Link& L) {
+  return L.kind == LINK_NODE && o.active[o.cell(L.node[0], L.node[1], L.node[2])];
+}
+
 // D:R16.  HALFWAY: the active nodes are the fluid nodes (geo = 0).  NODAL: also every solid node
 // with at least one fluid node among its lattice neighbours — these are the wall nodes on which
 // "a collision operation is then applied ... like in the fluid bulk"; deeper solid nodes
@@ -203,7 +264,7 @@ void classify_nodes(Oracle& o) {
         if (!a && o.wall_model == WALL_NODAL) {
           for (int iq = 0; iq < o.L.Q && !a; ++iq) {
             int s[3];
-            if (neighbour(o, x, y, z, iq, +1, s, nullptr) && o.geo[o.cell(s[0], s[1], s[2])] == 0) a = 1;
+            if (neighbour(o, x, y, z, iq, +1, s) && o.geo[o.cell(s[0], s[1], s[2])] == 0) a = 1;
           }
         }
         o.active[i] = a;
@@ -219,11 +280,10 @@ void replicate_nodal(Oracle& o, int x, int y, int z, const double* keep /* fb of
   const int Q = o.L.Q;
   const int64_t i = o.cell(x, y, z);
   for (int iq = 0; iq < Q; ++iq) {
-    int up[3], dn[3];
-    const bool up_active = neighbour(o, x, y, z, iq, -1, up, nullptr) && o.active[o.cell(up[0], up[1], up[2])];
-    if (up_active) continue;
-    const bool dn_active = neighbour(o, x, y, z, iq, +1, dn, nullptr) && o.active[o.cell(dn[0], dn[1], dn[2])];
-    if (dn_active) o.f[i * Q + iq] = o.f[i * Q + (Q - 1 - iq)];
+    const Link up = resolve(o, x, y, z, iq, -1);
+    // D:R24: a link through an open face (MOVING / PRESSURE) is no wall link: its value is the face's rule
+    if (up.kind == LINK_MOVING || up.kind == LINK_PRESSURE || link_has_active_node(o, up)) continue;
+    if (link_has_active_node(o, resolve(o, x, y, z, iq, +1))) o.f[i * Q + iq] = o.f[i * Q + (Q - 1 - iq)];
     else if (keep) o.f[i * Q + iq] = keep[Q - 1 - iq];
   }
 }
@@ -306,32 +366,30 @@ void propagation(Oracle& o) {
         const int64_t i = o.cell(x, y, z);
         if (!o.active[i]) continue;
         for (int iq = 0; iq < Q; ++iq) {
-          int s[3], moving_face, pressure_face;
-          const bool inside = neighbour(o, x, y, z, iq, -1, s, &moving_face, &pressure_face);
-          if (inside && o.active[o.cell(s[0], s[1], s[2])]) {
-            o.f[i * Q + iq] = o.fb[o.cell(s[0], s[1], s[2]) * Q + iq];
-          } else if (o.wall_model == WALL_HALFWAY) {
-            double v = o.fb[i * Q + (Q - 1 - iq)];
-            if (!inside && moving_face >= 0) {
-              double uw[3], eduw = 0.0;
-              wall_velocity(o, moving_face, x, y, z, uw);
-              for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * uw[d];
-              v += 6.0 * o.L.t[iq] * o.rho_w[i] * eduw;
-            } else if (!inside && pressure_face >= 0) {
-              // D:R22 anti-bounce-back: f_a = -f*_abar + 2 feq+_a(rho_face, u(x,t)), feq+ = the part of the
-              // equilibrium that is even in e (Eq. 2: t rho (1 + 4.5 (e.u)^2 - 1.5 u.u); Eq. 5: t (rho + rho0 (...)))
-              const double* uu = &o.u_w[i * 3];
-              double edu = 0.0, udu = 0.0;
-              for (int d = 0; d < 3; ++d) {
-                edu += o.L.e[iq][d] * uu[d];
-                udu += uu[d] * uu[d];
-              }
-              const double rf = o.face_rho[pressure_face];
-              const double even = (o.eq == EQ_STANDARD) ? o.L.t[iq] * rf * (1.0 + 4.5 * edu * edu - 1.5 * udu)
-                                                        : o.L.t[iq] * (rf + o.rho0 * (4.5 * edu * edu - 1.5 * udu));
-              v = -v + 2.0 * even;
+          const Link L = resolve(o, x, y, z, iq, -1);
+          if (link_has_active_node(o, L)) {
+            // Eq. 7; through a SYMMETRY face (D:R25) the mirror image: direction L.dir of the mirrored node
+            o.f[i * Q + iq] = o.fb[o.cell(L.node[0], L.node[1], L.node[2]) * Q + L.dir];
+          } else if (L.kind == LINK_MOVING) {
+            double uw[3], eduw = 0.0;
+            wall_velocity(o, L.face, x, y, z, uw);
+            for (int d = 0; d < 3; ++d) eduw += o.L.e[iq][d] * uw[d];
+            o.f[i * Q + iq] = o.fb[i * Q + (Q - 1 - iq)] + 6.0 * o.L.t[iq] * o.rho_w[i] * eduw;
+          } else if (L.kind == LINK_PRESSURE) {
+            // D:R22 anti-bounce-back: f_a = -f*_abar + 2 feq+_a(rho_face, u(x,t)), feq+ = the part of the
+            // equilibrium that is even in e (Eq. 2: t rho (1 + 4.5 (e.u)^2 - 1.5 u.u); Eq. 5: t (rho + rho0 (...)))
+            const double* uu = &o.u_w[i * 3];
+            double edu = 0.0, udu = 0.0;
+            for (int d = 0; d < 3; ++d) {
+              edu += o.L.e[iq][d] * uu[d];
+              udu += uu[d] * uu[d];
             }
-            o.f[i * Q + iq] = v;
+            const double rf = o.face_rho[L.face];
+            const double even = (o.eq == EQ_STANDARD) ? o.L.t[iq] * rf * (1.0 + 4.5 * edu * edu - 1.5 * udu)
+                                                      : o.L.t[iq] * (rf + o.rho0 * (4.5 * edu * edu - 1.5 * udu));
+            o.f[i * Q + iq] = -o.fb[i * Q + (Q - 1 - iq)] + 2.0 * even;
+          } else if (o.wall_model == WALL_HALFWAY) {
+            o.f[i * Q + iq] = o.fb[i * Q + (Q - 1 - iq)];  // Eq. 10 for a wall half-way between nodes (D:R3)
           }
         }
         if (o.wall_model == WALL_NODAL) replicate_nodal(o, x, y, z, &o.fb[i * Q]);
@@ -354,7 +412,7 @@ void boundary_force(const Oracle& o, double F[3]) {
         if (o.geo[i] != 0 || !o.active[i]) continue;
         for (int iq = 0; iq < Q; ++iq) {
           int d3[3];
-          if (!neighbour(o, x, y, z, iq, +1, d3, nullptr)) continue;
+          if (!neighbour(o, x, y, z, iq, +1, d3)) continue;
           if (o.geo[o.cell(d3[0], d3[1], d3[2])] == 0) continue;
           const double term = o.fb[i * Q + iq] + o.f[i * Q + (Q - 1 - iq)];
           for (int d = 0; d < 3; ++d) acc[d] += (long double)term * o.L.e[iq][d];

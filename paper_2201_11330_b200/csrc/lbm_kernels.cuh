@@ -200,6 +200,35 @@ __device__ __forceinline__ T* plane(T* buf, long long N) {
   return buf + (long long)A * N;
 }
 
+// Cache policy of the population streams of the A/B step kernel (tuning hooks; defaults chosen by measurement,
+// DESIGN.md section 6): every population is read once and written once per step, nothing is re-used.
+//   LBM_LD_POLICY 0 ld.global.nc (__ldg)  1 .cs (streaming)  2 .cg (L2 only)  3 .lu (last use)
+//   LBM_ST_POLICY 0 plain st.global       1 .cs              2 .cg            3 .wt
+#ifndef LBM_LD_POLICY
+#define LBM_LD_POLICY 0
+#endif
+#ifndef LBM_ST_POLICY
+#define LBM_ST_POLICY 0
+#endif
+#if LBM_LD_POLICY == 1
+#define LBM_LD_STREAM(q) __ldcs(q)
+#elif LBM_LD_POLICY == 2
+#define LBM_LD_STREAM(q) __ldcg(q)
+#elif LBM_LD_POLICY == 3
+#define LBM_LD_STREAM(q) __ldlu(q)
+#else
+#define LBM_LD_STREAM(q) __ldg(q)
+#endif
+#if LBM_ST_POLICY == 1
+#define LBM_ST_STREAM(q, v) __stcs(q, v)
+#elif LBM_ST_POLICY == 2
+#define LBM_ST_STREAM(q, v) __stcg(q, v)
+#elif LBM_ST_POLICY == 3
+#define LBM_ST_STREAM(q, v) __stwt(q, v)
+#else
+#define LBM_ST_STREAM(q, v) (*(q) = (v))
+#endif
+
 // ---------------------------------------------------------------------------------------
 // Storage element access.  fp64: the value itself.  fp32 storage (S:§8f NEXT-1): f - t_a is
 // kept as float, arithmetic stays fp64.
@@ -601,22 +630,22 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   auto wall = [&](auto A) { return plane<Dir<Q, decltype(A)::value>::opp>(src, p.N) + nb.ic; };  // t_a == t_abar: same shift
   if constexpr (sizeof(ST) == 4) {
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
-    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
+    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); })) return;
     nodal_replicate<Q, BC>(g, p, c);
     collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.ic, z, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
       const float s = (float)v;
-      plane<a>(dst, p.N)[nb.ic] = s;
+      LBM_ST_STREAM(plane<a>(dst, p.N) + nb.ic, s);
       if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], s);
     });
   } else {
     double f[Q];
-    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return __ldg(q); })) return;
+    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); })) return;
     nodal_replicate<Q, BC>(f, p, c);
     collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
-      st_pop<ST, Q, a>(plane<a>(dst, p.N), nb.ic, f[a]);
+      LBM_ST_STREAM(plane<a>(dst, p.N) + nb.ic, f[a]);  // ST = double in this branch
       if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], f[a]);
     });
   }
