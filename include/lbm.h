@@ -56,7 +56,7 @@ enum {
   LBM_STORE_F32 = 1 << 16   /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
 };
 
-enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2, LBM_FACE_PRESSURE = 3 };
+enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2, LBM_FACE_PRESSURE = 3, LBM_FACE_SYMMETRY = 4 };
 
 /* Wall model of lbm_set_geometry (D:R3, D:R16, D:R17). */
 enum {
@@ -82,7 +82,15 @@ enum {
  *   outlet = PRESSURE: anti-bounce-back at a prescribed density rho_f (lbm_set_face_density, default 1):
  *            f_a(x,t+1) = -f*_abar(x,t) + 2 feq+_a(rho_f, u(x,t)), feq+ = the part of Eq. 2 / Eq. 5 even in e_a
  *            (Eq. 2: t_a rho_f (1 + 4.5 (e_a.u)^2 - 1.5 u.u); Eq. 5: t_a (rho_f + rho0 (4.5 (e_a.u)^2 - 1.5 u.u))).
- *   A link that leaves through several non-periodic faces: MOVING > BOUNCE > PRESSURE (highest index within a kind). */
+ *   A link that leaves through several non-periodic faces: MOVING > BOUNCE > PRESSURE (highest index within a kind).
+ * SYMMETRY (D:R25; "the left and right boundaries are symmetric"): a mirror plane half a link beyond the last
+ *   node (specular reflection, free slip).  A link that leaves through SYMMETRY faces only connects the node with the
+ *   mirror image: f_a(x,t+1) = f*_a'(x', t), x' = x - e_a on the axes not crossed, a' = e_a with the crossed components
+ *   negated; if x' is not an active node the link is a wall link.  Together with a face of another kind, that kind
+ *   decides.  Handles with a SYMMETRY face always use the link mask of lbm_set_geometry (+4 B per node and step); they
+ *   need LBM_SCHEME_AB and are not available as z-slabs (LBM_EUNSUPPORTED).
+ * Under LBM_WALL_NODAL (D:R24) the MOVING / PRESSURE / SYMMETRY faces keep these link-wise rules; Eq. 10 acts on the
+ *   wall links only (BOUNCE faces and solid nodes). */
 typedef struct {
   int32_t face_kind[6];
   double face_u[6][3]; /* read only where face_kind == LBM_FACE_MOVING                          */
@@ -111,8 +119,7 @@ void lbm_destroy(lbm_handle h);
  *     NODAL  : f_a(x, t+1) = f_abar(x, t+1) (Eq. 10: the value that has just arrived along abar)
  *              if x + e_a is active, else f*_abar(x, t) (D:R17: links inside the wall)
  * One 32-bit link mask per node is built here and read by the step kernel (+4 B per node and
- * step); (NULL, LBM_WALL_HALFWAY) returns to the mask-free analytic box.  LBM_WALL_NODAL with
- * LBM_FACE_MOVING or LBM_FACE_PRESSURE faces returns LBM_EUNSUPPORTED.  Synchronises the stream. */
+ * step); (NULL, LBM_WALL_HALFWAY) returns to the mask-free analytic box.  Synchronises the stream. */
 int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model);
 /* Same with a HOST pointer to the N mask bytes. */
 int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model);

@@ -72,7 +72,7 @@ struct lbm_handle_s {
   uint32_t* peer_hi_flag;
   void* ipc_opened[6];
   int n_ipc_opened;
-  int bx, by;         // block shape of the fused kernel (lbm_set_block)
+  int bx, by;         // block shape of the fused kernel (lbm_set_block), 0,0 = default_block()
   int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
   size_t elem() const { return f32 ? 4 : 8; }
   size_t buf_bytes() const { return (size_t)N * Q * elem(); }
@@ -97,14 +97,29 @@ int flat_grid(const lbm_handle_s* h) {
   return (int)(b < kReduceBlocks ? b : kReduceBlocks);
 }
 
+// Default block of the fused kernels, by measurement: rows of 256 threads for the kernels that
+// keep three or four 256-thread blocks per SM (D3Q19 / D2Q9 A/B without forcing or mask); 128 threads where the
+// register count allows only two of them (D3Q27, forcing) and for the link-mask kernels, whose face / wall cells make
+// single warps run long: a block holds its registers until its last warp retires, smaller blocks hold fewer.
+void default_block(const lbm_handle_s* h, int& bx, int& by) {
+  const bool small = h->scheme == LBM_SCHEME_AB && (h->Q == 27 || h->forced || h->has_geo);
+  const int threads = small ? 128 : 256;
+  bx = 32;
+  while (bx < h->nx && bx < threads) bx *= 2;
+  by = threads / bx;
+  while (by > 1 && (h->ny + by - 1) / by > 65535) by /= 2;
+}
+
 Ctx make_ctx(const lbm_handle_s* h) {
   Ctx c;
+  int bx = h->bx, by = h->by;
+  if (bx == 0) default_block(h, bx, by);
   c.eq = h->eq ? EQ_INCOMP : EQ_STANDARD;
   c.bc = h->has_geo ? BC_GEO : (h->walls ? BC_WALLS : BC_PERIODIC);
   c.forced = h->forced;
   c.f32 = h->f32;
-  c.block = dim3(h->bx, h->by, 1);
-  c.grid = dim3((h->nx + h->bx - 1) / h->bx, (h->ny + h->by - 1) / h->by, h->p.z_hi - h->p.z_lo);
+  c.block = dim3(bx, by, 1);
+  c.grid = dim3((h->nx + bx - 1) / bx, (h->ny + by - 1) / by, h->p.z_hi - h->p.z_lo);
   c.flat_grid = flat_grid(h);
   c.fbx = h->fbx;
   c.stream = h->stream;
@@ -299,10 +314,8 @@ int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
   if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
-  if (wall_model == LBM_WALL_NODAL && h->p.any_open)
-    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING / LBM_FACE_PRESSURE faces is not supported");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
-  if (!geo_dev && wall_model == LBM_WALL_HALFWAY) {  // back to the analytic box
+  if (!geo_dev && wall_model == LBM_WALL_HALFWAY && !h->p.any_sym) {  // back to the analytic box
     free_geometry(h);
     return LBM_OK;
   }
@@ -378,12 +391,14 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   if (bc) {
     for (int k = 0; k < 6; ++k) {
       const int kind = bc->face_kind[k];
-      if (kind != LBM_FACE_PERIODIC && kind != LBM_FACE_BOUNCE && kind != LBM_FACE_MOVING && kind != LBM_FACE_PRESSURE) {
+      if (kind != LBM_FACE_PERIODIC && kind != LBM_FACE_BOUNCE && kind != LBM_FACE_MOVING && kind != LBM_FACE_PRESSURE && kind != LBM_FACE_SYMMETRY) {
         delete h; fail(LBM_EINVAL, "lbm_create: unknown face kind"); return nullptr;
       }
       p.wall[k] = kind != LBM_FACE_PERIODIC;
       p.kind[k] = kind;
       p.open[k] = kind == LBM_FACE_MOVING || kind == LBM_FACE_PRESSURE;
+      p.sym[k] = kind == LBM_FACE_SYMMETRY;
+      p.any_sym |= p.sym[k];
       for (int d = 0; d < 3; ++d) {
         p.face_u[k][d] = kind == LBM_FACE_MOVING ? bc->face_u[k][d] : 0.0;
         if (!std::isfinite(p.face_u[k][d])) { delete h; fail(LBM_EINVAL, "lbm_create: non-finite wall velocity"); return nullptr; }
@@ -396,6 +411,12 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
       if (!std::isfinite(p.F[d])) { delete h; fail(LBM_EINVAL, "lbm_create: non-finite force"); return nullptr; }
     }
     h->stream = (cudaStream_t)bc->stream;
+  }
+  if (p.any_sym && scheme == LBM_SCHEME_AA) {
+    delete h; fail(LBM_EUNSUPPORTED, "lbm_create: LBM_FACE_SYMMETRY needs LBM_SCHEME_AB"); return nullptr;
+  }
+  if (p.any_sym && slab) {
+    delete h; fail(LBM_EUNSUPPORTED, "lbm_create_slab: LBM_FACE_SYMMETRY is not supported on z-slab handles (it needs the link mask)"); return nullptr;
   }
   p.z_lo = 0;
   p.z_hi = nz;
@@ -424,7 +445,7 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   // default block: as long along x as the row allows (coalesced, vector-friendly), 256 threads
   int bx = 32;
   while (bx < nx && bx < 256) bx *= 2;
-  h->bx = bx; h->by = 256 / bx;
+  h->bx = h->by = 0;  // default_block() at launch time (it depends on the geometry)
   h->fbx = bx;
 
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
@@ -444,6 +465,14 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
     lbm_destroy(h);
     fail(oom ? LBM_ENOMEM : LBM_ECUDA, msg);
     return nullptr;
+  }
+  if (p.any_sym) {  // D:R25: mirror links are resolved through the link mask: build it for the empty geometry
+    if (do_set_geometry(h, nullptr, LBM_WALL_HALFWAY) != LBM_OK) {
+      const std::string msg = g_err;
+      lbm_destroy(h);
+      g_err = msg;
+      return nullptr;
+    }
   }
   return h;
 }
@@ -641,8 +670,6 @@ int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model)
   if (!geo_host) return do_set_geometry(h, nullptr, wall_model);
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
-  if (wall_model == LBM_WALL_NODAL && h->p.any_open)
-    return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: LBM_WALL_NODAL with LBM_FACE_MOVING / LBM_FACE_PRESSURE faces is not supported");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   {
     int rc = alloc_geometry(h);
@@ -777,9 +804,8 @@ int64_t lbm_launch_count(lbm_handle h) { return h ? h->launches : -1; }
 int lbm_set_block(lbm_handle h, int bx, int by) {
   if (!h) return fail(LBM_EINVAL, "lbm_set_block: NULL handle");
   if (bx == 0 && by == 0) {
-    bx = 32;
-    while (bx < h->nx && bx < 256) bx *= 2;
-    by = 256 / bx;
+    h->bx = h->by = 0;
+    return LBM_OK;
   }
   if (bx < 1 || by < 1 || bx * by > 256 || (bx * by) % 32 != 0)
     return fail(LBM_EINVAL, "lbm_set_block: bx*by must be a multiple of 32 and <= 256");

@@ -5,6 +5,7 @@
 // cores, no shared-memory staging; one thread owns one cell, the Q populations live in
 // registers, every per-direction stream is unit-stride in x (SoA f[a][z][y][x]).
 #pragma once
+#include <type_traits>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -71,7 +72,7 @@ template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
 constexpr int kMinBlocks = LBM_MB_OVERRIDE;
 #else
 template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
-constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 27 && STBYTES == 4 && !INPLACE) ? 3 : (Q == 19 && STBYTES == 4 && !INPLACE) ? (FORCE ? 3 : 4) : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
+constexpr int kMinBlocks = (Q == 9) ? (FORCE || INPLACE ? 3 : 4) : (Q == 27 && STBYTES == 4 && !INPLACE) ? 3 : (Q == 19 && STBYTES == 4 && !INPLACE) ? (FORCE ? 3 : 4) : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
 #endif
 
 // ---------------------------------------------------------------------------------------
@@ -79,7 +80,8 @@ constexpr int kMinBlocks = (Q == 9) ? 3 : (Q == 27 && STBYTES == 4 && !INPLACE) 
 //   BC_PERIODIC  never                                           (no test at all)
 //   BC_WALLS     coordinate tests against the non-periodic faces (0 B/cell)
 //   BC_GEO       one 32-bit link mask per cell, built once by build_links_kernel from the
-//                solid mask `geo` and the faces           (4 B/cell read per step)
+//                solid mask `geo` and the faces           (4 B/cell read per step);
+//                also every handle with a SYMMETRY face (D:R25)
 enum { BC_PERIODIC = 0, BC_WALLS = 1, BC_GEO = 2 };
 
 struct Params {
@@ -96,9 +98,12 @@ struct Params {
   const double* face_prof[6];
   double face_rho[6];   // D:R22: density prescribed on PRESSURE faces (anti-bounce-back)
   int any_open;
+  int sym[6];           // face is SYMMETRY (D:R25); such handles always run the BC_GEO kernels (link mask)
+  int any_sym;
   int zg_off, nz_glob;  // global plane index of local plane z = z + zg_off; planes of the whole box (slabs: D:R21)
-  // BC_GEO only (D:R16): bit a (a != rest) of links[i]: node i - e_a is not an active node (solid,
-  // or beyond a non-periodic face); bit `rest`: node i itself is inactive.
+  // BC_GEO only (D:R16): bit a (a != rest) of links[i]: link a of node i has no active source node — i - e_a is
+  // solid, or lies beyond a non-periodic face; through SYMMETRY faces only (D:R25) the source is the mirror image
+  // and the bit says whether THAT node is inactive.  Bit `rest`: node i itself is inactive.
   const uint32_t* links;
   int nodal;            // D:R3/R17: the paper's modified nodal bounce-back (Eq. 10) instead of halfway
   // Planes [z_lo, z_hi) are the ones this handle updates and the z faces of the box lie at z_lo and z_hi-1.
@@ -117,7 +122,7 @@ struct Params {
 };
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
-enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3 };
+enum { FACE_PERIODIC = 0, FACE_BOUNCE = 1, FACE_MOVING = 2, FACE_PRESSURE = 3, FACE_SYMMETRY = 4 };
 
 // Position of a cell relative to the non-periodic faces, and (BC_GEO) its link mask.
 template <int BC>
@@ -193,6 +198,44 @@ struct Neigh {
     return ox[1 + S * Dir<Q, A>::ex] + oy[1 + S * Dir<Q, A>::ey] + oz[1 + S * Dir<Q, A>::ez];
   }
 };
+
+// Index of the lattice vector (ex,ey,ez) in Lattice<Q> (compile time), -1 if the set has no such vector.
+template <int Q>
+__host__ __device__ constexpr int dir_index(int ex, int ey, int ez) {
+  for (int a = 0; a < Q; ++a)
+    if (Lattice<Q>::e[a][0] == ex && Lattice<Q>::e[a][1] == ey && Lattice<Q>::e[a][2] == ez) return a;
+  return -1;
+}
+
+// SYMMETRY faces (D:R25; "the left and right boundaries are symmetric"): a mirror plane half a link beyond
+// the last node.  If the node x + S*e_A lies beyond SYMMETRY faces ONLY, the link connects x with the mirror image:
+// the node whose coordinates along the crossed axes are those of x, and the population there has the direction
+// e_A with those components negated.  Returns false for every other link (inside the box, or through a face of
+// another kind: MOVING > BOUNCE > PRESSURE decide those, D:R22).  idx = in-plane index of that node.
+template <int BC>
+__device__ __forceinline__ bool touches_sym(const Params& p, const CellFlags<BC>& c) {
+  if constexpr (BC == BC_PERIODIC) return false;
+  if (!p.any_sym) return false;
+  return (c.lo[0] && p.sym[0]) || (c.hi[0] && p.sym[1]) || (c.lo[1] && p.sym[2]) || (c.hi[1] && p.sym[3]) ||
+         (c.lo[2] && p.sym[4]) || (c.hi[2] && p.sym[5]);
+}
+
+template <int Q, int A, int S, int BC>
+__device__ __forceinline__ bool mirror_link(const Params& p, const CellFlags<BC>& c, const Neigh& nb, int& dir, int& idx) {
+  using D = Dir<Q, A>;
+  constexpr int dx = S * D::ex, dy = S * D::ey, dz = S * D::ez;
+  const bool cx = (dx == -1) ? c.lo[0] : (dx == 1) ? c.hi[0] : false;
+  const bool cy = (dy == -1) ? c.lo[1] : (dy == 1) ? c.hi[1] : false;
+  const bool cz = (dz == -1) ? c.lo[2] : (dz == 1) ? c.hi[2] : false;
+  const bool sx = cx && p.sym[dx == 1 ? 1 : 0], sy = cy && p.sym[dy == 1 ? 3 : 2], sz = cz && p.sym[dz == 1 ? 5 : 4];
+  if ((cx && !sx) || (cy && !sy) || (cz && !sz) || !(sx || sy || sz)) return false;
+  idx = (sx ? nb.ox[1] : nb.ox[1 + dx]) + (sy ? nb.oy[1] : nb.oy[1 + dy]) + (sz ? nb.oz[1] : nb.oz[1 + dz]);
+  constexpr int t1 = dir_index<Q>(-D::ex, D::ey, D::ez), t2 = dir_index<Q>(D::ex, -D::ey, D::ez), t3 = dir_index<Q>(-D::ex, -D::ey, D::ez),
+                t4 = dir_index<Q>(D::ex, D::ey, -D::ez), t5 = dir_index<Q>(-D::ex, D::ey, -D::ez), t6 = dir_index<Q>(D::ex, -D::ey, -D::ez),
+                t7 = dir_index<Q>(-D::ex, -D::ey, -D::ez);
+  dir = sz ? (sy ? (sx ? t7 : t6) : (sx ? t5 : t4)) : (sy ? (sx ? t3 : t2) : (sx ? t1 : A));
+  return true;
+}
 
 // Base of direction plane A of a population buffer (64-bit, thread-invariant).
 template <int A, typename T>
@@ -334,7 +377,58 @@ struct CellState {  // what the open faces need from the collision of this cell
   double rw;              // rho(x,t) under Eq. 2, rho0 = 1 under Eq. 5
   double ux, uy, uz, usq15;
   int ic, z;              // in-plane index and (local) plane of the cell
+  // Fast path: the cell touches exactly ONE non-periodic face (every face cell except edges and corners), so every
+  // link that leaves the box leaves through it.  With the inlet / outlet on the x faces there is one such cell per
+  // row, i.e. one lane of one warp in every block runs this code while the rest of the block waits for it: it has
+  // to be short (512x128x128 D3Q27 with inlet + outlet: 673 -> ... us per step once the per-direction face
+  // classification was taken off this path).
+  int face;               // that face, or -1: classify every direction (edges, corners)
+  int kind;               // its kind (FACE_MOVING or FACE_PRESSURE)
+  double wx, wy, wz, rf;  // its wall velocity at this cell / its density
 };
+
+// Wall velocity of MOVING face `face` at the cell with in-plane index ic in local plane z: the uniform face_u or the
+// cell's entry of the per-cell profile (D:R22).
+__device__ __forceinline__ void wall_velocity(const Params& p, int face, int ic, int z, double& wx, double& wy, double& wz) {
+  wx = p.face_u[face][0]; wy = p.face_u[face][1]; wz = p.face_u[face][2];
+  const double* prof = p.face_prof[face];
+  if (prof) {
+    // in-face index of the cell from its in-plane index: the face fixes one coordinate
+    const int axis = face >> 1, side = face & 1;
+    const int zg = z + p.zg_off;
+    long long j, n;
+    if (axis == 0) {        // j = y + ny*zg
+      const int xf = side ? p.nx - 1 : 0;
+      j = (ic - xf) / p.nx + (long long)p.ny * p.zg_off;
+      n = (long long)p.ny * p.nz_glob;
+    } else if (axis == 1) { // j = x + nx*zg
+      const int yf = side ? p.ny - 1 : 0;
+      j = (long long)(ic - p.nx * yf - p.nx * p.ny * z) + (long long)p.nx * zg;
+      n = (long long)p.nx * p.nz_glob;
+    } else {                // j = x + nx*y
+      j = ic - p.nx * p.ny * z;
+      n = (long long)p.nx * p.ny;
+    }
+    wx = __ldg(prof + j); wy = __ldg(prof + n + j); wz = __ldg(prof + 2 * n + j);
+  }
+}
+
+// Fill the single-face part of the cell state (call once per cell that touches an open face).
+template <int BC>
+__device__ __forceinline__ void classify_open_cell(CellState& s, const Params& p, const CellFlags<BC>& c) {
+  s.face = -1;
+  s.kind = 0;
+  s.wx = s.wy = s.wz = 0.0;
+  s.rf = 1.0;
+  const int nwall = (int)c.lo[0] + (int)c.hi[0] + (int)c.lo[1] + (int)c.hi[1] + (int)c.lo[2] + (int)c.hi[2];
+  if (nwall == 1) {
+    const int k = c.lo[0] ? 0 : c.hi[0] ? 1 : c.lo[1] ? 2 : c.hi[1] ? 3 : c.lo[2] ? 4 : 5;
+    s.face = k;
+    s.kind = p.kind[k];  // MOVING or PRESSURE: the caller checked touches_open and this is the only face
+    if (s.kind == FACE_MOVING) wall_velocity(p, k, s.ic, s.z, s.wx, s.wy, s.wz);
+    else s.rf = p.face_rho[k];
+  }
+}
 
 // v = post-collision value of outgoing direction B (in the stored variable: f*, or f* - t_B if SHIFTED);
 // returns what the slot must hold.
@@ -344,13 +438,28 @@ __device__ __forceinline__ double open_link(double v, const Params& p, const Cel
   if constexpr (BC == BC_PERIODIC || D::s == 0) {
     return v;
   } else {
+    auto moving = [&](double wx, double wy, double wz) { return v - (6.0 * D::t) * s.rw * edot<Q, B>(wx, wy, wz); };
+    auto pressure = [&](double rf) {
+      const double eu = edot<Q, B>(s.ux, s.uy, s.uz);
+      const double poly = fma(4.5 * eu, eu, -s.usq15);
+      // Eq. 2: t rf (1 + poly);  Eq. 5: t (rf + rho0 poly);  SHIFTED: minus t_B for the stored variable
+      double even = (EQ == EQ_STANDARD) ? fma(rf, poly, rf) : rf + poly;
+      if constexpr (SHIFTED) even -= 1.0;
+      return fma(2.0 * D::t, even, -v);
+    };
+    if (s.face >= 0) {  // one face only: the link leaves through it or not at all
+      const bool leaves = (D::ex == -1 && s.face == 0) || (D::ex == 1 && s.face == 1) || (D::ey == -1 && s.face == 2) ||
+                          (D::ey == 1 && s.face == 3) || (D::ez == -1 && s.face == 4) || (D::ez == 1 && s.face == 5);
+      if (!leaves) return v;
+      return s.kind == FACE_MOVING ? moving(s.wx, s.wy, s.wz) : pressure(s.rf);
+    }
     int mface = -1, pface = -1;
     bool bounce = false;
     auto crossed = [&](int face) {
       const int k = p.kind[face];
       if (k == FACE_MOVING) mface = face;
       else if (k == FACE_PRESSURE) pface = face;
-      else bounce = true;
+      else if (k == FACE_BOUNCE) bounce = true;  // a SYMMETRY face crossed together with another kind: the other decides
     };
     // x, then y, then z: the highest face index crossed wins within a kind
     if constexpr (D::ex != 0) {
@@ -363,38 +472,11 @@ __device__ __forceinline__ double open_link(double v, const Params& p, const Cel
       if (D::ez == 1 ? c.hi[2] : c.lo[2]) crossed(D::ez == 1 ? 5 : 4);
     }
     if (mface >= 0) {
-      double wx = p.face_u[mface][0], wy = p.face_u[mface][1], wz = p.face_u[mface][2];
-      const double* prof = p.face_prof[mface];
-      if (prof) {
-        // in-face index of the cell from its in-plane index: the face fixes one coordinate
-        const int axis = mface >> 1, side = mface & 1;
-        const int zg = s.z + p.zg_off;
-        long long j, n;
-        if (axis == 0) {        // j = y + ny*zg
-          const int xf = side ? p.nx - 1 : 0;
-          j = (s.ic - xf) / p.nx + (long long)p.ny * p.zg_off;
-          n = (long long)p.ny * p.nz_glob;
-        } else if (axis == 1) { // j = x + nx*zg
-          const int yf = side ? p.ny - 1 : 0;
-          j = (long long)(s.ic - p.nx * yf - p.nx * p.ny * s.z) + (long long)p.nx * zg;
-          n = (long long)p.nx * p.nz_glob;
-        } else {                // j = x + nx*y
-          j = s.ic - p.nx * p.ny * s.z;
-          n = (long long)p.nx * p.ny;
-        }
-        wx = __ldg(prof + j); wy = __ldg(prof + n + j); wz = __ldg(prof + 2 * n + j);
-      }
-      return v - (6.0 * D::t) * s.rw * edot<Q, B>(wx, wy, wz);
+      double wx, wy, wz;
+      wall_velocity(p, mface, s.ic, s.z, wx, wy, wz);
+      return moving(wx, wy, wz);
     }
-    if (pface >= 0 && !bounce) {
-      const double eu = edot<Q, B>(s.ux, s.uy, s.uz);
-      const double rf = p.face_rho[pface];
-      const double poly = fma(4.5 * eu, eu, -s.usq15);
-      // Eq. 2: t rf (1 + poly);  Eq. 5: t (rf + rho0 poly);  SHIFTED: minus t_B for the stored variable
-      double even = (EQ == EQ_STANDARD) ? fma(rf, poly, rf) : rf + poly;
-      if constexpr (SHIFTED) even -= 1.0;
-      return fma(2.0 * D::t, even, -v);
-    }
+    if (pface >= 0 && !bounce) return pressure(p.face_rho[pface]);
     return v;
   }
 }
@@ -465,6 +547,7 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
       st.ux = mx * inv; st.uy = my * inv; st.uz = mz * inv;
       st.usq15 = 1.5 * (st.ux * st.ux + st.uy * st.uy + st.uz * st.uz);
       st.ic = ic; st.z = z;
+      classify_open_cell<BC>(st, p, c);
       static_for<0, Q>([&](auto BB) {
         constexpr int b = decltype(BB)::value;
         f[b] = open_link<Q, EQ, BC, b, false>(f[b], p, c, st);
@@ -515,7 +598,8 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
   }
   // open faces (D:R6, D:R22): what an outgoing wall link keeps in its slot; identity on every other cell
   const bool touch = touches_open<BC>(p, c);
-  const CellState st{A, ux, uy, uz, usq15, ic, z};
+  CellState st{A, ux, uy, uz, usq15, ic, z, -1, 0, 0.0, 0.0, 0.0, 1.0};
+  if (touch) classify_open_cell<BC>(st, p, c);
   auto open = [&](auto BB, double v) -> double {
     constexpr int b = decltype(BB)::value;
     if constexpr (BC != BC_PERIODIC && Dir<Q, b>::s > 0) {
@@ -545,20 +629,54 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
   });
 }
 
+// D:R24: true if the outgoing link B of this cell (node x + e_B) is resolved by an open face — it crosses a MOVING
+// face, or a PRESSURE face and no BOUNCE face.  Such a link is no wall link: Eq. 10 leaves it alone.
+template <int Q, int B, int BC>
+__device__ __forceinline__ bool open_resolved(const Params& p, const CellFlags<BC>& c) {
+  using D = Dir<Q, B>;
+  bool moving = false, pressure = false, bounce = false;
+  auto crossed = [&](int face) {
+    const int k = p.kind[face];
+    moving = moving | (k == FACE_MOVING);
+    pressure = pressure | (k == FACE_PRESSURE);
+    bounce = bounce | (k == FACE_BOUNCE);
+  };
+  if constexpr (D::ex != 0) {
+    if (D::ex == 1 ? c.hi[0] : c.lo[0]) crossed(D::ex == 1 ? 1 : 0);
+  }
+  if constexpr (D::ey != 0) {
+    if (D::ey == 1 ? c.hi[1] : c.lo[1]) crossed(D::ey == 1 ? 3 : 2);
+  }
+  if constexpr (D::ez != 0) {
+    if (D::ez == 1 ? c.hi[2] : c.lo[2]) crossed(D::ez == 1 ? 5 : 4);
+  }
+  return moving | (pressure & !bounce);
+}
+
 // Eq. 10 of the paper's modified nodal bounce-back (D:R17), applied to the populations a
 // wall node has just gathered: a direction a nothing streamed in along (link bit a set) takes the
 // value that arrived along its opposite, f_a = f_abar, if abar did arrive from an active node (bit
-// abar clear).  When neither end of the link is active the halfway value already in f[a] stays.
+// abar clear).  When neither end of the link is active the halfway value already in f[a] stays; so does the value of
+// a link through an open face (D:R24: MOVING / PRESSURE faces keep their own rule next to nodal walls).
 template <int Q, int BC, typename T>
 __device__ __forceinline__ void nodal_replicate(T (&f)[Q], const Params& p, const CellFlags<BC>& c) {
   if constexpr (BC == BC_GEO) {
     if (p.nodal && (c.m != 0u)) {
+      // D:R24: cells next to an open face must tell wall links from open links; with exactly one non-periodic face
+      // at the cell (the usual case, one lane per row for x faces: keep it short) every link that leaves the box is open
+      const bool open_cell = touches_open<BC>(p, c);
+      const bool single = ((int)c.lo[0] + (int)c.hi[0] + (int)c.lo[1] + (int)c.hi[1] + (int)c.lo[2] + (int)c.hi[2]) == 1;
       static_for<0, Q>([&](auto A) {
         constexpr int a = decltype(A)::value;
         constexpr int o = Dir<Q, a>::opp;
         if constexpr (a != o) {
           // each +- pair is touched at most once: the condition excludes its mirror image
-          if (((c.m >> a) & 1u) && !((c.m >> o) & 1u)) f[a] = f[o];
+          if (((c.m >> a) & 1u) && !((c.m >> o) & 1u)) {
+            // link a arrives from x - e_a = x + e_o: open-resolved links are not wall links
+            bool open = false;
+            if (open_cell) open = single ? c.template leaves_box<Q, a, -1>() : open_resolved<Q, o, BC>(p, c);
+            if (!open) f[a] = f[o];
+          }
         }
       });
     }
@@ -573,8 +691,10 @@ __device__ __forceinline__ void nodal_replicate(T (&f)[Q], const Params& p, cons
 // would double.  A regular load of a wall link reads a slot nobody writes; the value is discarded.  The price
 // is Q wasted loads on an inactive node, which is right for the paper's workloads (an obstacle in a channel:
 // a fraction of a percent of the nodes are solid).  Returns false for an inactive node.
-template <int Q, int BC, typename T, typename LinkF, typename WallF, typename LoadF>
-__device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&& link, WallF&& wall, LoadF&& load) {
+struct NoMirror {};  // gather() without SYMMETRY faces (the in-place kernels: lbm_create refuses the combination)
+
+template <int Q, int BC, typename T, typename LinkF, typename WallF, typename LoadF, typename MirrorF = NoMirror>
+__device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&& link, WallF&& wall, LoadF&& load, MirrorF&& mirror = NoMirror{}, bool at_mirror = false) {
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     auto q = link(A);
@@ -592,6 +712,19 @@ __device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&
           if (c.template leaves<Q, a, -1>()) f[a] = load(A, wall(A));
         }
       });
+    }
+    // D:R25: links through SYMMETRY faces come from the mirror image (mirror(A) = its address, or NULL for every
+    // other link); the link bit says whether that node is active.  Only cells next to such a face get here.
+    if constexpr (!std::is_same<std::decay_t<MirrorF>, NoMirror>::value) {
+      if (at_mirror) {
+        static_for<0, Q>([&](auto A) {
+          constexpr int a = decltype(A)::value;
+          if constexpr (Dir<Q, a>::s > 0) {
+            auto q = mirror(A);
+            if (q && !c.template leaves<Q, a, -1>()) f[a] = load(A, q);
+          }
+        });
+      }
     }
   }
   return true;
@@ -628,9 +761,16 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   const CellFlags<BC> c(p, x, y, z, nb.ic);
   auto link = [&](auto A) { return plane<decltype(A)::value>(src, p.N) + nb.template at<Q, decltype(A)::value, -1>(); };
   auto wall = [&](auto A) { return plane<Dir<Q, decltype(A)::value>::opp>(src, p.N) + nb.ic; };  // t_a == t_abar: same shift
+  // D:R25: through SYMMETRY faces f_a comes from the mirror image (same speed class: same fp32 shift)
+  auto mirror = [&](auto A) -> const ST* {
+    int dir, idx;
+    if (!mirror_link<Q, decltype(A)::value, -1, BC>(p, c, nb, dir, idx)) return nullptr;
+    return src + (long long)dir * p.N + idx;
+  };
+  const bool at_mirror = touches_sym<BC>(p, c);
   if constexpr (sizeof(ST) == 4) {
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
-    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); })) return;
+    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); }, mirror, at_mirror)) return;
     nodal_replicate<Q, BC>(g, p, c);
     collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.ic, z, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
@@ -640,7 +780,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     });
   } else {
     double f[Q];
-    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); })) return;
+    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); }, mirror, at_mirror)) return;
     nodal_replicate<Q, BC>(f, p, c);
     collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
     static_for<0, Q>([&](auto A) {
@@ -730,6 +870,18 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
     }
     f[a] = ld_pop_rw<ST, Q, a>(q, 0);
   });
+  if constexpr (BC == BC_GEO && MODE == MODE_PULL) {
+    if (touches_sym<BC>(p, c)) {  // D:R25: links through SYMMETRY faces read the mirror image
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        if constexpr (Dir<Q, a>::s > 0) {
+          int dir, idx;
+          if (mirror_link<Q, a, -1, BC>(p, c, nb, dir, idx) && !c.template leaves<Q, a, -1>())
+            f[a] = ld_pop_rw<ST, Q, a>(buf + (long long)dir * p.N + idx, 0);
+        }
+      });
+    }
+  }
   nodal_replicate<Q, BC>(f, p, c);
 }
 
@@ -783,6 +935,12 @@ __global__ void __launch_bounds__(256) import_canonical(const double* __restrict
         q = plane<a>(in, p.N) + nb.template at<Q, a, 1>();
         if constexpr (BC != BC_PERIODIC) {
           if (c.template leaves<Q, a, 1>()) q = plane<o>(in, p.N) + i;
+        }
+        if constexpr (BC == BC_GEO && Dir<Q, a>::s > 0) {
+          // D:R25: a slot whose link leaves through SYMMETRY faces is read by the mirror image, as direction `dir`
+          int dir, idx;
+          if (p.any_sym && mirror_link<Q, a, 1, BC>(p, c, nb, dir, idx) && !c.template leaves<Q, a, 1>())
+            q = in + (long long)dir * p.N + idx;
         }
         // slab: the halo planes are filled here too (the canonical arrays of a slab carry the neighbour's
         // planes); a slot whose downstream node would lie beyond a halo plane is never read: leave it.
@@ -847,8 +1005,14 @@ __global__ void __launch_bounds__(256) build_links_kernel(const uint8_t* __restr
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       if constexpr (Dir<Q, a>::s > 0) {
-        bool none = c.template leaves_box<Q, a, -1>();
-        if (!none) none = active[nb.template at<Q, a, -1>()] == 0;
+        bool none;
+        int dir, idx;
+        if (p.any_sym && mirror_link<Q, a, -1, BC_WALLS>(p, c, nb, dir, idx)) {
+          none = active[idx] == 0;  // D:R25: the source is the mirror image
+        } else {
+          none = c.template leaves_box<Q, a, -1>();
+          if (!none) none = active[nb.template at<Q, a, -1>()] == 0;
+        }
         m |= none ? (1u << a) : 0u;
       }
     });

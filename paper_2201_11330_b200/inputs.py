@@ -19,7 +19,7 @@ import numpy as np
 
 SEED_BASE = 0x22011330
 
-FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE = 0, 1, 2, 3
+FACE_PERIODIC, FACE_BOUNCE, FACE_MOVING, FACE_PRESSURE, FACE_SYMMETRY = 0, 1, 2, 3, 4
 EQ_STANDARD, EQ_INCOMP = 0, 1
 WALL_HALFWAY, WALL_NODAL = 0, 1
 
@@ -140,7 +140,7 @@ class Workload:
     u0: float = 0.0
     noise: float = 0.0
     seed: int = 0
-    kind: str = "tgv"  # "tgv" | "rest"
+    kind: str = "tgv"  # "tgv" | "rest" | "channel" (parabolic inflow) | "inflow" (uniform inflow)
     eq: int = EQ_STANDARD
     wall_model: int = WALL_HALFWAY
     sphere: tuple | None = None  # (cx, cy, cz, r): nodes with |x - c| <= r are solid
@@ -186,6 +186,8 @@ class Workload:
             return taylor_green(self.nx, self.ny, self.nz, self.u0, self.noise, self.seed, box)
         rho = density_noise(self.nx, self.ny, self.nz, self.noise, self.seed, box)
         u = np.zeros((3, rho.size))
+        if self.kind == "inflow":
+            u[0] = self.inlet_umax  # the uniform inflow velocity everywhere
         if self.kind == "channel":
             # the inlet profile at every x ("steady-state inviscid flow with randomly distributed perturbation")
             b = box or ((0, self.nx), (0, self.ny), (0, self.nz))
@@ -243,4 +245,15 @@ def config(i: int) -> Workload:
                         face_kind=(FACE_MOVING, FACE_PRESSURE, FACE_BOUNCE, FACE_BOUNCE, FACE_PERIODIC, FACE_PERIODIC),
                         noise=1e-5, seed=SEED_BASE + i + 1, kind="channel", eq=EQ_INCOMP,
                         cylinder=(cx, (ny - 1) / 2.0, D / 2.0), face_rho=(1.0,) * 6, inlet_umax=U)
+    if i == 8:
+        # Not in BASELINE.json: the paper's sphere case with the boundaries P:468 names — "the back surface is inlet and
+        # the front surface is outlet, the left and right boundaries are symmetric, and the top and bottom boundaries
+        # are periodic": x- MOVING (uniform inflow U), x+ PRESSURE rho = 1, y-/y+ SYMMETRY, z periodic (R22,
+        # R24, R25); D3Q27, Eq. 5, nodal bounce-back on the sphere as in config 5.  U = 0.05 (Re = U D / nu = 43).
+        U = 0.05
+        return Workload("cfg8_q27_sphere_open512x128x128", 512, 128, 128, 27, 1.0 / 1.8, 6401,
+                        face_kind=(FACE_MOVING, FACE_PRESSURE, FACE_SYMMETRY, FACE_SYMMETRY, FACE_PERIODIC, FACE_PERIODIC),
+                        face_u=((U, 0.0, 0.0),) + tuple((0.0, 0.0, 0.0) for _ in range(5)),
+                        noise=1e-5, seed=SEED_BASE + 9, kind="inflow", eq=EQ_INCOMP, wall_model=WALL_NODAL,
+                        sphere=(64.0, 64.0, 64.0, 8.0), face_rho=(1.0,) * 6, inlet_umax=U)
     raise IndexError(i)

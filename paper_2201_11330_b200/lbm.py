@@ -17,7 +17,7 @@ LBM_D2Q9, LBM_D3Q19, LBM_D3Q27 = 9, 19, 27
 LBM_EQ_STANDARD, LBM_EQ_INCOMP = 0, 1 << 8
 LBM_SCHEME_AUTO, LBM_SCHEME_AB, LBM_SCHEME_AA = 0, 1 << 12, 2 << 12
 LBM_STORE_F64, LBM_STORE_F32 = 0, 1 << 16
-LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE = 0, 1, 2, 3
+LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE, LBM_FACE_SYMMETRY = 0, 1, 2, 3, 4
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
 

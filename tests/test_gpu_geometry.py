@@ -92,8 +92,6 @@ def test_random_populations_with_mask(lbm, scheme, model, faces, Q, eq, forced):
     dims = (37, 21, 13)
     N = dims[0] * dims[1] * dims[2]
     fk, fu = FACES[faces]
-    if model == WALL_NODAL and M in fk:
-        pytest.skip("nodal walls with a MOVING face are unsupported by both sides")
     geo = obstacle_mask(dims, seed=Q)
     F = (2e-4, -1e-4, 3e-4 if Q != 9 else 0.0) if forced else None
     o, s = make_pair(lbm, dims, Q, 0.77, geo, model, eq, scheme, fk, face_u_of(fu), F)
@@ -194,10 +192,8 @@ def test_returning_to_the_analytic_box(lbm):
 def test_geometry_argument_errors(lbm):
     s = lbm.Solver(8, 8, 8, 19, 0.8, face_kind=[B, B, B, B, B, M], face_u=face_u_of({5: (0.1, 0, 0)}))
     with pytest.raises(lbm.LBMError) as e:
-        s.set_geometry(None, lbm.LBM_WALL_NODAL)
-    assert e.value.code == lbm.LBM_EUNSUPPORTED
-    with pytest.raises(lbm.LBMError):
         s.set_geometry(None, 7)
+    assert e.value.code == lbm.LBM_EINVAL
     with pytest.raises(lbm.LBMError):
         s.boundary_force()  # no geometry
     s.set_geometry(torch.zeros(512, dtype=torch.uint8), lbm.LBM_WALL_HALFWAY)  # host pointer path

@@ -1,13 +1,14 @@
 """GPU parity for the open boundaries (R22; the paper's channel-cylinder example): FACE_PRESSURE
 (anti-bounce-back at a prescribed density) and FACE_MOVING with a per-cell wall-velocity profile (velocity inlet),
-through the C ABI (lbm_set_face_density, lbm_set_face_velocity) against the CPU oracle, element by element.
+through the C ABI (lbm_set_face_density, lbm_set_face_velocity); FACE_SYMMETRY mirror planes (R25; the sphere case's
+"symmetric" sides) and open faces next to the nodal wall model (R24) — against the CPU oracle, element by element.
 Tolerance: max |df| <= 1e-12 (BASELINE.json north_star); fp32 storage <= 2e-5 relative.  `pytest -m gpu` on a B200.
 """
 import numpy as np
 import pytest
 
 from oracle import Oracle
-from oracle.binding import EQ_INCOMP, EQ_STANDARD, WALL_HALFWAY
+from oracle.binding import EQ_INCOMP, EQ_STANDARD, WALL_HALFWAY, WALL_NODAL
 from paper_2201_11330_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -15,6 +16,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 TOL = 1e-12
 P, B, M, PR = inputs.FACE_PERIODIC, inputs.FACE_BOUNCE, inputs.FACE_MOVING, inputs.FACE_PRESSURE
+S = inputs.FACE_SYMMETRY
 
 
 @pytest.fixture(scope="module")
@@ -56,7 +58,7 @@ MIXES = {
 FACE_RHO = (1.02, 0.97, 1.01, 0.99, 1.03, 0.98)
 
 
-def make_pair(lbm, dims, Q, tau, fk, eq, scheme, store=0, force=None, seed=0, profiles=True, geo=None):
+def make_pair(lbm, dims, Q, tau, fk, eq, scheme, store=0, force=None, seed=0, profiles=True, geo=None, model=WALL_HALFWAY):
     nx, ny, nz = dims
     fu = np.zeros((6, 3))
     for k in range(6):
@@ -67,9 +69,9 @@ def make_pair(lbm, dims, Q, tau, fk, eq, scheme, store=0, force=None, seed=0, pr
                    scheme={"ab": lbm.LBM_SCHEME_AB, "aa": lbm.LBM_SCHEME_AA}[scheme], store=store,
                    face_kind=fk, face_u=fu, force=force)
     s.set_face_density(FACE_RHO)
-    if geo is not None:
-        o.set_geometry(geo, WALL_HALFWAY)
-        s.set_geometry(torch.from_numpy(np.ascontiguousarray(geo, dtype=np.uint8).reshape(-1)).cuda(), lbm.LBM_WALL_HALFWAY)
+    if geo is not None or model != WALL_HALFWAY:
+        o.set_geometry(geo, model)
+        s.set_geometry(None if geo is None else torch.from_numpy(np.ascontiguousarray(geo, dtype=np.uint8).reshape(-1)).cuda(), model)
     if profiles:
         # every second MOVING face gets a per-cell profile, the others keep the uniform face_u
         for j, k in enumerate([k for k in range(6) if fk[k] == M]):
@@ -213,8 +215,6 @@ def test_open_face_argument_checks(lbm):
         s.set_face_velocity(1, dev(np.zeros(3 * 64)))
     with pytest.raises(lbm.LBMError):
         s.set_face_velocity(6, None)
-    with pytest.raises(lbm.LBMError):  # the paper defines no open boundary for its nodal wall model
-        s.set_geometry(None, lbm.LBM_WALL_NODAL)
     with pytest.raises(lbm.LBMError):
         s.set_face_density([1.0, float("nan"), 1, 1, 1, 1])
     s.set_face_velocity(0, dev(np.zeros(3 * 64)))
@@ -222,6 +222,10 @@ def test_open_face_argument_checks(lbm):
     s.close()
     with pytest.raises(lbm.LBMError):  # PRESSURE on one face of an axis, periodic on the other
         lbm.Solver(8, 8, 8, 19, 0.8, face_kind=[PR, P, P, P, P, P])
+    with pytest.raises(lbm.LBMError):  # mirror planes need the A/B scheme
+        lbm.Solver(8, 8, 8, 19, 0.8, face_kind=[S, S, P, P, P, P], scheme=lbm.LBM_SCHEME_AA)
+    with pytest.raises(lbm.LBMError):  # and are not available on z-slabs
+        lbm.lbm_create_slab(8, 8, 4, 0, 8, 19, 0.8, lbm.make_bc([S, S, P, P, P, P]))
 
 
 # --------------------------------------------------------------------------- the paper's printed drag coefficients
@@ -266,3 +270,136 @@ def test_channel_cylinder_drag_matches_the_paper(lbm, golden_dir, case, cfg, ste
         assert h[:, 0].std() < 0.02 * cd
     else:
         assert h[:, 1].max() > 0.1 and h[:, 1].min() < -0.1   # von Karman street: the lift oscillates (Re > 47)
+
+
+# --------------------------------------------------------------------------- symmetry planes (R25), nodal + open (R24)
+SYM_MIXES = {
+    "sphere_case_faces": [M, PR, S, S, P, P],   # inlet, outlet, symmetric sides, periodic top / bottom
+    "duct_sym_walls": [M, PR, S, B, B, S],
+    "all_kinds": [S, PR, M, B, PR, S],
+    "sym_everywhere": [S] * 6,
+    "inlet_outlet_walls": [M, PR, B, B, P, P],  # the channel-cylinder faces: R24 under the nodal model
+}
+
+
+def lumps(dims):
+    """Solid lumps: one in the interior, one cut by the y- plane, one in the (0,0,0) corner, single nodes."""
+    nx, ny, nz = dims
+    g = np.zeros((nz, ny, nx), dtype=np.uint8)
+    g[nz // 2:nz // 2 + 2, ny // 2 - 1:ny // 2 + 2, nx // 3:nx // 3 + 3] = 1
+    g[:, 0:2, nx // 2:nx // 2 + 2] = 1
+    g[0, 0, 0] = 1
+    g[nz - 1, ny - 1, nx - 2:] = 1
+    g[nz - 1, ny // 2, 0] = 1
+    return g.reshape(-1)
+
+
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("model", [WALL_HALFWAY, WALL_NODAL], ids=["halfway", "nodal"])
+@pytest.mark.parametrize("Q,eq", [(9, EQ_INCOMP), (19, EQ_STANDARD), (27, EQ_INCOMP)])
+@pytest.mark.parametrize("mix", sorted(SYM_MIXES))
+def test_symmetry_and_nodal_open_faces_match_oracle(lbm, mix, Q, eq, model, store):
+    dims = (37, 11, 1 if Q == 9 else 6)
+    fk = list(SYM_MIXES[mix])
+    if Q == 9:
+        fk[4] = fk[5] = P
+    N = dims[0] * dims[1] * dims[2]
+    force = (1e-5, -2e-5, 0.0) if mix == "all_kinds" else None
+    o, s = make_pair(lbm, dims, Q, 0.62, fk, eq, "ab", store=lbm.LBM_STORE_F32 if store == "f32" else 0, force=force,
+                     seed=4, geo=lumps(dims), model=model)
+    if store == "f64":
+        f0 = random_f(Q, N, 8)
+        o.set_f(f0)
+        s.set_populations(dev(f0))
+        # set_populations makes the nodal state consistent with Eq. 10 on both sides
+        assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+        for n in (1, 4):
+            o.step(n)
+            s.step(n)
+            err = float(np.abs(s.get_populations().cpu().numpy() - o.get_f()).max())
+            assert err <= TOL, f"{mix} Q{Q} eq{eq} model{model}: max|df| = {err:.3e} after {s.time} steps"
+        rho_o, u_o, d_o = o.moments()
+        rho_g, u_g, d_g = s.moments()
+        assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= TOL
+        assert np.abs(u_g.cpu().numpy() - u_o).max() <= TOL
+        assert np.abs(s.boundary_force() - o.boundary_force()).max() <= TOL
+    else:
+        rho = 1.0 + 1e-3 * np.random.default_rng(2).uniform(-1, 1, N)
+        o.init_equilibrium(rho, None)
+        s.init_equilibrium(dev(rho), None)
+        o.step(12)
+        s.step(12)
+        ref = o.get_f()
+        assert np.abs(s.get_populations().cpu().numpy() - ref).max() / np.abs(ref).max() <= 2e-5
+    s.close()
+
+
+def test_uniform_flow_between_mirror_planes_stays_uniform(lbm):
+    """Free slip through the CUDA path: u = (U,0,0) between symmetry planes is a steady state (no wall friction)."""
+    s = lbm.Solver(64, 33, 5, 19, 0.7, face_kind=[P, P, S, S, S, S])
+    u = np.zeros((3, s.N))
+    u[0] = 0.05
+    s.init_equilibrium(None, dev(u.reshape(-1)))
+    f0 = s.get_populations().clone()
+    s.step(100)
+    assert float((s.get_populations() - f0).abs().max()) <= 1e-15
+    s.close()
+
+
+# --------------------------------------------------------------------------- the sphere case with the paper's boundaries
+def _oracle_of(w):
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, eq=w.eq, face_kind=w.face_kind, face_u=w.face_u, force=w.force, face_rho=w.face_rho)
+    if w.has_geometry:
+        o.set_geometry(w.geo(), w.wall_model)
+    for k, prof in w.face_profiles().items():
+        o.set_face_velocity(k, prof)
+    return o
+
+
+def test_sphere_case_open_quarter_size_point_A_history(lbm):
+    """inputs.config(8) — inlet, outlet, symmetric sides, periodic top / bottom, nodal sphere — with every length
+    divided by 4, 400 steps: the paper's own validation (Fig. 7: velocity and pressure at point A, CPU run against
+    GPU run, differences 1e-16..1e-17) repeated as oracle against CUDA path at the scaled point A = (18,18,18)."""
+    w = inputs.config(8).shrunk(4, steps=400)
+    rho, u = w.fields()
+    o = _oracle_of(w)
+    s = lbm.Solver.from_workload(w)
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    A = 18 + w.nx * (18 + w.ny * 18)
+    worst = 0.0
+    for _ in range(20):
+        o.step(20)
+        s.step(20)
+        ro, uo, _ = o.moments()
+        rg, ug, _ = s.moments()
+        worst = max(worst, abs(float(rg[A]) - ro[A]), float(np.abs(ug[:, A].cpu().numpy() - uo[:, A]).max()))
+    assert worst <= 1e-13, worst
+    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    assert np.abs(s.boundary_force() - o.boundary_force()).max() <= TOL
+    assert o.boundary_force()[0] > 0
+    s.close()
+
+
+def test_sphere_case_open_full_size_first_steps(lbm):
+    """inputs.config(8) at the paper's 512 x 128 x 128: every population after 6 steps, point A = (72,72,72), the force."""
+    w = inputs.config(8)
+    rho, u = w.fields()
+    o = _oracle_of(w)
+    s = lbm.Solver.from_workload(w)
+    o.init_equilibrium(rho, u)
+    s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
+    o.step(6)
+    s.step(6)
+    f = s.get_populations()
+    ref = o.get_f()
+    err = 0.0
+    for a in range(w.Q):  # plane by plane: no second 1.8 GB host copy
+        err = max(err, float(np.abs(f[a].cpu().numpy() - ref[a]).max()))
+    assert err <= TOL, err
+    A = 72 + w.nx * (72 + w.ny * 72)
+    ro, uo, _ = o.moments()
+    rg, ug, _ = s.moments()
+    assert abs(float(rg[A]) - ro[A]) <= 1e-14 and float(np.abs(ug[:, A].cpu().numpy() - uo[:, A]).max()) <= 1e-14
+    assert np.abs(s.boundary_force() - o.boundary_force()).max() <= TOL
+    s.close()
