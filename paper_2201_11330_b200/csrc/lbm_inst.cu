@@ -1,12 +1,12 @@
 // lbm_inst.cu — kernel instantiations.  Compiled once per (LBM_Q, LBM_PART) by build.py, in parallel:
 //   LBM_Q    9 | 19 | 27
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
-//            5 A/B step of a z-slab (fused halo push)
+//            5 A/B step of a z-slab (fused halo push)   6 A/B step with SYMMETRY faces (link mask + mirror links)
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..5"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..6"
 #endif
 
 namespace lbm {
@@ -60,10 +60,25 @@ constexpr int Q_ = LBM_Q;
 #if LBM_PART == 0
 template <>
 void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
+  if (c.p.any_sym) return launch_step_ab_sym<Q_>(c, src, dst);  // part 6
   dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
     using ST = decltype(st);
     stream_collide_ab<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
         <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+  });
+}
+#elif LBM_PART == 6
+template <>
+void launch_step_ab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
+  // D:R25: handles with SYMMETRY faces always carry the link mask (BC_GEO)
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_force(c, [&](auto force) {
+      dispatch_storage(c, [&](auto st) {
+        using ST = decltype(st);
+        stream_collide_ab<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, ST, false, true>
+            <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+      });
+    });
   });
 }
 #elif LBM_PART == 5

@@ -750,7 +750,9 @@ __device__ __forceinline__ void push_one(const Params& p, int z, int ixy, ST v) 
   }
 }
 
-template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB = false>
+// SYM (D:R25): the box has SYMMETRY faces (always BC_GEO).  A separate instantiation: the mirror fix-up costs the
+// link-mask kernels registers even where it never runs (sphere case 15.4 -> 15.0 GLUPS when it was compiled in).
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB = false, bool SYM = false>
 __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -767,10 +769,15 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     if (!mirror_link<Q, decltype(A)::value, -1, BC>(p, c, nb, dir, idx)) return nullptr;
     return src + (long long)dir * p.N + idx;
   };
-  const bool at_mirror = touches_sym<BC>(p, c);
+  const bool at_mirror = SYM ? touches_sym<BC>(p, c) : false;
+  auto pull = [&](auto& f) {
+    auto load = [](auto, const ST* q) { return LBM_LD_STREAM(q); };
+    if constexpr (SYM) return gather<Q, BC>(f, c, link, wall, load, mirror, at_mirror);
+    else return gather<Q, BC>(f, c, link, wall, load);
+  };
   if constexpr (sizeof(ST) == 4) {
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
-    if (!gather<Q, BC>(g, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); }, mirror, at_mirror)) return;
+    if (!pull(g)) return;
     nodal_replicate<Q, BC>(g, p, c);
     collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.ic, z, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
@@ -780,7 +787,7 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     });
   } else {
     double f[Q];
-    if (!gather<Q, BC>(f, c, link, wall, [](auto, const ST* q) { return LBM_LD_STREAM(q); }, mirror, at_mirror)) return;
+    if (!pull(f)) return;
     nodal_replicate<Q, BC>(f, p, c);
     collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
     static_for<0, Q>([&](auto A) {
