@@ -299,7 +299,7 @@ void make_state_consistent(Oracle& o) {
 // InitPDF: f(x, 0) = feq(rho0(x), u0(x)).  D:R17: under the NODAL model the state
 // is then made consistent with Eq. 10 on the wall nodes.
 void init_pdf(Oracle& o, const double* rho, const double* u /* SoA u[c*N+i] */) {
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (o.N >= 16384)  // tiny grids: a thread team costs more than the sweep
   for (int64_t i = 0; i < o.N; ++i) {
     const double r = rho ? rho[i] : 1.0;
     double uu[3] = {0.0, 0.0, 0.0};
@@ -317,7 +317,7 @@ void init_pdf(Oracle& o, const double* rho, const double* u /* SoA u[c*N+i] */) 
 void collision(Oracle& o) {
   const int Q = o.L.Q;
   const bool forced = (o.F[0] != 0.0 || o.F[1] != 0.0 || o.F[2] != 0.0);
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (o.N >= 16384)  // tiny grids: a thread team costs more than the sweep
   for (int64_t i = 0; i < o.N; ++i) {
     if (!o.active[i]) continue;  // the loop runs over `fluid_id` (here: the active nodes, D:R16)
     const double* fc = &o.f[i * Q];
@@ -359,7 +359,7 @@ void boundary_condition(Oracle&) {}
 // index (z+ > z- > y+ > y- > x+ > x-) is used.
 void propagation(Oracle& o) {
   const int Q = o.L.Q;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (o.N >= 16384)  // tiny grids: a thread team costs more than the sweep
   for (int z = 0; z < o.nz; ++z)
     for (int y = 0; y < o.ny; ++y)
       for (int x = 0; x < o.nx; ++x) {
