@@ -87,8 +87,8 @@ enum {
  *   node (specular reflection, free slip).  A link that leaves through SYMMETRY faces only connects the node with the
  *   mirror image: f_a(x,t+1) = f*_a'(x', t), x' = x - e_a on the axes not crossed, a' = e_a with the crossed components
  *   negated; if x' is not an active node the link is a wall link.  Together with a face of another kind, that kind
- *   decides.  Handles with a SYMMETRY face always use the link mask of lbm_set_geometry (+4 B per node and step); they
- *   need LBM_SCHEME_AB and are not available as z-slabs (LBM_EUNSUPPORTED).
+ *   decides.  Handles with a SYMMETRY face always use the link mask of lbm_set_geometry (+4 B per node and step) and
+ *   need LBM_SCHEME_AB (LBM_EUNSUPPORTED otherwise).
  * Under LBM_WALL_NODAL (D:R24) the MOVING / PRESSURE / SYMMETRY faces keep these link-wise rules; Eq. 10 acts on the
  *   wall links only (BOUNCE faces and solid nodes). */
 typedef struct {
@@ -202,8 +202,12 @@ int lbm_set_block(lbm_handle h, int bx, int by);
  * memory: NVLink between GPUs); there is no separate exchange pass and no host staging.  Ordering between
  * slabs is on the device: step t of a slab starts when both neighbours have finished step t-1 (a 64-bit
  * counter per side in the slab's own memory, written by the neighbour, waited for by the stream).
- * Restrictions: LBM_SCHEME_AB only; no lbm_set_geometry; every slab must be advanced by the same
- * number of steps; lbm_init_equilibrium / lbm_set_populations need all connected slabs idle. */
+ * Geometry on a slab: lbm_set_geometry takes the mask with TWO halo planes per side — nx*ny*(nz_local+4) bytes, plane
+ * index 2 + (z_global - z0), periodic wrap included, ignored beyond a non-periodic z face — because under
+ * LBM_WALL_NODAL the wall-node status of a halo node depends on the plane beyond it (D:R16).  lbm_boundary_force
+ * returns the part of Eq. 13 carried by the fluid nodes of the own planes: sum it over the slabs.
+ * Restrictions: LBM_SCHEME_AB only; every slab must be advanced by the same number of steps;
+ * lbm_init_equilibrium / lbm_set_populations / lbm_set_geometry need all connected slabs idle. */
 
 /* What a neighbour needs to know about a slab.  Plain data: pass it to another process as bytes. */
 typedef struct {

@@ -311,7 +311,6 @@ int alloc_geometry(lbm_handle_s* h) {
 
 // geo_dev: device pointer to N bytes (must not alias h->geo or h->active), or NULL (all fluid)
 int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
-  if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -414,9 +413,6 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   }
   if (p.any_sym && scheme == LBM_SCHEME_AA) {
     delete h; fail(LBM_EUNSUPPORTED, "lbm_create: LBM_FACE_SYMMETRY needs LBM_SCHEME_AB"); return nullptr;
-  }
-  if (p.any_sym && slab) {
-    delete h; fail(LBM_EUNSUPPORTED, "lbm_create_slab: LBM_FACE_SYMMETRY is not supported on z-slab handles (it needs the link mask)"); return nullptr;
   }
   p.z_lo = 0;
   p.z_hi = nz;
@@ -664,9 +660,13 @@ int lbm_set_geometry(lbm_handle h, const uint8_t* geo, int wall_model) {
   return do_set_geometry(h, geo, wall_model);
 }
 
+// bytes of the mask the caller passes: N, or on a z-slab two more planes (two halo planes per side, include/lbm.h)
+static size_t geo_input_bytes(const lbm_handle_s* h) {
+  return (size_t)h->N + (h->slab ? 2 * (size_t)h->nx * h->ny : 0);
+}
+
 int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model) {
   if (!h) return fail(LBM_EINVAL, "lbm_set_geometry_host: NULL handle");
-  if (h->slab) return fail(LBM_EUNSUPPORTED, "lbm_set_geometry: not supported on a z-slab handle");
   if (!geo_host) return do_set_geometry(h, nullptr, wall_model);
   if (wall_model != LBM_WALL_HALFWAY && wall_model != LBM_WALL_NODAL)
     return fail(LBM_EINVAL, "lbm_set_geometry: wall_model must be LBM_WALL_HALFWAY or LBM_WALL_NODAL");
@@ -675,9 +675,17 @@ int lbm_set_geometry_host(lbm_handle h, const uint8_t* geo_host, int wall_model)
     int rc = alloc_geometry(h);
     if (rc) return rc;
   }
-  // stage the host mask in the link-mask array (4N bytes, rebuilt last by do_set_geometry)
-  uint8_t* stage = (uint8_t*)h->links + (size_t)h->N * 3;
-  CUDA_TRY(cudaMemcpyAsync(stage, geo_host, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+  // stage the host mask in the tail of the link-mask array (4N bytes, rebuilt last by do_set_geometry); a slab's
+  // mask is two planes longer than N and goes to the scratch buffer instead
+  uint8_t* stage = nullptr;
+  if (h->slab) {
+    int rc = ensure_scratch(h, geo_input_bytes(h));
+    if (rc) return rc;
+    stage = (uint8_t*)h->scratch;
+  } else {
+    stage = (uint8_t*)h->links + (size_t)h->N * 3;
+  }
+  CUDA_TRY(cudaMemcpyAsync(stage, geo_host, geo_input_bytes(h), cudaMemcpyHostToDevice, h->stream));
   return do_set_geometry(h, stage, wall_model);
 }
 

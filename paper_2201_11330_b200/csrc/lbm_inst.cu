@@ -2,11 +2,12 @@
 //   LBM_Q    9 | 19 | 27
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
 //            5 A/B step of a z-slab (fused halo push)   6 A/B step with SYMMETRY faces (link mask + mirror links)
+//            7 A/B step of a z-slab with SYMMETRY faces
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..6"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..7"
 #endif
 
 namespace lbm {
@@ -84,17 +85,22 @@ void launch_step_ab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
 #elif LBM_PART == 5
 template <>
 void launch_step_ab_slab<Q_>(const Ctx& c, const void* src, void* dst) {
-  // z-slabs exist for the analytic box only (BC_PERIODIC / BC_WALLS): lbm_set_geometry refuses a slab handle
+  if (c.p.any_sym) return launch_step_ab_slab_sym<Q_>(c, src, dst);  // part 7
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    stream_collide_ab<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST, true>
+        <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+  });
+}
+#elif LBM_PART == 7
+template <>
+void launch_step_ab_slab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
   dispatch_eq(c, [&](auto eq) {
     dispatch_force(c, [&](auto force) {
       dispatch_storage(c, [&](auto st) {
         using ST = decltype(st);
-        if (c.bc == BC_PERIODIC)
-          stream_collide_ab<Q_, decltype(eq)::value, BC_PERIODIC, decltype(force)::value != 0, ST, true>
-              <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
-        else
-          stream_collide_ab<Q_, decltype(eq)::value, BC_WALLS, decltype(force)::value != 0, ST, true>
-              <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
+        stream_collide_ab<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, ST, true, true>
+            <<<c.grid, c.block, 0, c.stream>>>((const ST*)src, (ST*)dst, c.p);
       });
     });
   });
@@ -177,7 +183,7 @@ void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const ui
   });
 }
 #else
-#error "LBM_PART must be 0..5"
+#error "LBM_PART must be 0..7"
 #endif
 
 }  // namespace lbm

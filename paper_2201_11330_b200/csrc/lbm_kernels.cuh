@@ -983,23 +983,32 @@ __global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __r
 template <int Q>
 __global__ void __launch_bounds__(256) classify_nodes_kernel(const uint8_t* __restrict__ geo_in, uint8_t* __restrict__ geo, uint8_t* __restrict__ active,
                                                              int nodal, int bx, const __grid_constant__ Params p) {
-  // geo_in: the caller's mask (any device-readable memory; NULL = no solid nodes); geo: the library's 0/1 copy
+  // geo_in: the caller's mask (any device-readable memory; NULL = no solid nodes); geo: the library's 0/1 copy.
+  // z-slab (D:R21): geo_in carries TWO halo planes per side (nz + 2 planes, plane 1 + z of the handle's plane z), so
+  // that the halo nodes — whose wall-node status the own planes' links depend on — see all their neighbours.
+  const int pl = p.nx * p.ny;
+  const int zin = p.slab ? 1 : 0;
   for_each_cell(p, bx, [&](int x, int y, int z, int i) {
-    const bool solid = geo_in ? geo_in[i] != 0 : false;
+    const bool solid = geo_in ? geo_in[i + zin * pl] != 0 : false;
     bool a = !solid;
     if (solid && nodal) {
       const Neigh nb(p, x, y, z);
       const CellFlags<BC_WALLS> c(p, x, y, z, i);
       static_for<0, Q>([&](auto A) {
         constexpr int b = decltype(A)::value;
-        if constexpr (Dir<Q, b>::s > 0) {
-          if (!c.template leaves_box<Q, b, 1>()) a = a | (geo_in[nb.template at<Q, b, 1>()] == 0);
+        using D = Dir<Q, b>;
+        if constexpr (D::s > 0) {
+          if (!c.template leaves_box<Q, b, 1>()) {
+            // slab: no wrap along z inside the handle — the neighbouring planes are in geo_in as they are
+            const int j = p.slab ? nb.ox[1 + D::ex] + nb.oy[1 + D::ey] + (z + D::ez + zin) * pl : nb.template at<Q, b, 1>();
+            a = a | (geo_in[j] == 0);
+          }
         }
       });
     }
     geo[i] = solid ? 1 : 0;
     active[i] = a ? 1 : 0;
-  });
+  }, p.slab != 0);
 }
 
 template <int Q>
@@ -1024,7 +1033,8 @@ __global__ void __launch_bounds__(256) build_links_kernel(const uint8_t* __restr
       }
     });
     links[i] = m;
-  });
+  }, p.slab != 0);  // slab: the halo planes too (import_canonical fills their slots); bits of links that point
+                   // beyond a halo plane are meaningless and never used
 }
 
 // ---------------------------------------------------------------------------------------

@@ -24,6 +24,7 @@ struct Ctx {
 template <int Q> void launch_step_ab(const Ctx& c, const void* src, void* dst);
 template <int Q> void launch_step_ab_slab(const Ctx& c, const void* src, void* dst);
 template <int Q> void launch_step_ab_sym(const Ctx& c, const void* src, void* dst);
+template <int Q> void launch_step_ab_slab_sym(const Ctx& c, const void* src, void* dst);
 template <int Q> void launch_step_aa_even(const Ctx& c, void* buf);
 template <int Q> void launch_step_aa_odd(const Ctx& c, void* buf);
 template <int Q> void launch_export(const Ctx& c, int mode, const void* buf, double* out);

@@ -5,7 +5,7 @@ cross a cut once per step through host-staged MPI (P:165-169, P:286-294, P:395-3
 z only, the exchange is done by the fused step kernel itself (peer stores into the neighbour's halo plane)
 and the ordering between slabs is a device-side step counter; this module is the host-side plumbing:
 
-  partition / neighbours / halo_box / combine_diagnostics   pure functions (tested on CPU)
+  partition / neighbours / halo_box / slab_mask / combine_diagnostics   pure functions (tested on CPU)
   exchange_descriptors, all_reduce_diagnostics               torch.distributed (gloo on CPU, nccl on GPUs)
   SlabSolver                                                 one slab = one rank's share (one process per GPU)
   SlabGroup                                                  all slabs of a box in ONE process (one or more devices)
@@ -45,6 +45,23 @@ def halo_box(nx: int, ny: int, z0: int, nz_local: int):
     """Sub-box of the global grid that a slab's arrays cover: its own planes plus one halo plane on each side
     (inputs.Workload.fields(box=...) wraps the coordinates periodically)."""
     return ((0, nx), (0, ny), (z0 - 1, z0 + nz_local + 1))
+
+
+def slab_mask(geo, nx: int, ny: int, nz: int, z0: int, nz_local: int, periodic_z: bool):
+    """The solid mask a slab hands to lbm_set_geometry: its own planes plus TWO halo planes per side
+    (include/lbm.h: the wall-node status of a halo node depends on the plane beyond it), uint8[(nz_local+4)*ny*nx].
+    geo: uint8[nz*ny*nx] of the whole box or None.  Periodic z wraps; beyond a non-periodic z face the planes are 0."""
+    out = np.zeros((nz_local + 4, ny * nx), dtype=np.uint8)
+    if geo is None:
+        return out.reshape(-1)
+    g = np.asarray(geo, dtype=np.uint8).reshape(nz, ny * nx)
+    for k in range(nz_local + 4):
+        z = z0 - 2 + k
+        if periodic_z:
+            out[k] = g[z % nz]
+        elif 0 <= z < nz:
+            out[k] = g[z]
+    return out.reshape(-1)
 
 
 def combine_diagnostics(parts):
@@ -104,8 +121,6 @@ class Slab:
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2201_11330_b200 needs a CUDA device (no CPU fallback)")
-        if getattr(w, "has_geometry", False):
-            raise lbm.LBMError(lbm.LBM_EUNSUPPORTED, "z-slabs do not support lbm_set_geometry")
         self.w, self.z0, self.nz_local = w, int(z0), int(nz_local)
         self.nx, self.ny, self.Q = w.nx, w.ny, w.Q
         self.N = self.nx * self.ny * (self.nz_local + 2)
@@ -115,6 +130,11 @@ class Slab:
         eq = lbm.LBM_EQ_INCOMP if getattr(w, "eq", 0) else lbm.LBM_EQ_STANDARD
         self.bc = lbm.make_bc(w.face_kind, w.face_u, w.force, None if stream is None else stream.cuda_stream)
         self.h = lbm.lbm_create_slab(self.nx, self.ny, self.nz_local, self.z0, w.nz, int(w.Q) | eq | scheme | store, w.tau, self.bc)
+        # solid mask and wall model: the slab's planes of the whole-box mask + two halo planes per side
+        self.has_geometry = bool(getattr(w, "has_geometry", False))
+        if self.has_geometry:
+            m = slab_mask(w.geo(), self.nx, self.ny, w.nz, self.z0, self.nz_local, w.face_kind[4] == 0)
+            lbm.lbm_set_geometry(self.h, torch.from_numpy(m).cuda(), w.wall_model, m.size)
         # open boundaries (D:R22): every slab takes the density and the per-cell velocity of the WHOLE box faces
         if getattr(w, "face_rho", None) is not None:
             lbm.lbm_set_face_density(self.h, w.face_rho)
@@ -146,6 +166,10 @@ class Slab:
 
     def diagnostics(self):
         return lbm.lbm_moments(self.h, None, None, True)
+
+    def boundary_force(self):
+        """This slab's part of the momentum-exchange force (Eq. 13): the links of its own fluid nodes."""
+        return lbm.lbm_boundary_force(self.h)
 
     def moments(self):
         """(rho[N_own], u[3, N_own]) of the own planes (device tensors), diagnostics of the own planes."""
@@ -198,6 +222,15 @@ class SlabSolver(Slab):
     def global_diagnostics(self, device="cuda"):
         return all_reduce_diagnostics(self.diagnostics(), device)
 
+    def global_boundary_force(self, device="cuda"):
+        """Eq. 13 of the whole box: the slabs' parts summed over the process group."""
+        import torch
+        import torch.distributed as dist
+        F = torch.tensor(self.boundary_force(), dtype=torch.float64, device=device)
+        if dist.is_available() and dist.is_initialized():
+            dist.all_reduce(F, op=dist.ReduceOp.SUM)
+        return F.cpu().numpy()
+
 
 class SlabGroup:
     """All slabs of a box in one process: slab r on devices[r % len(devices)], each on its own stream.
@@ -246,6 +279,9 @@ class SlabGroup:
 
     def diagnostics(self):
         return combine_diagnostics(self._each(lambda s: s.diagnostics()))
+
+    def boundary_force(self):
+        return np.sum(self._each(lambda s: s.boundary_force()), axis=0)
 
     def get_populations(self):
         """Canonical populations of the whole box, [Q, N] (on the first device)."""

@@ -224,8 +224,6 @@ def test_open_face_argument_checks(lbm):
         lbm.Solver(8, 8, 8, 19, 0.8, face_kind=[PR, P, P, P, P, P])
     with pytest.raises(lbm.LBMError):  # mirror planes need the A/B scheme
         lbm.Solver(8, 8, 8, 19, 0.8, face_kind=[S, S, P, P, P, P], scheme=lbm.LBM_SCHEME_AA)
-    with pytest.raises(lbm.LBMError):  # and are not available on z-slabs
-        lbm.lbm_create_slab(8, 8, 4, 0, 8, 19, 0.8, lbm.make_bc([S, S, P, P, P, P]))
 
 
 # --------------------------------------------------------------------------- the paper's printed drag coefficients

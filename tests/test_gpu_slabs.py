@@ -192,7 +192,8 @@ def test_slab_argument_errors(mods):
         with pytest.raises(lbm.LBMError):
             lbm.lbm_slab_connect(h, lbm.lbm_slab_export(other), None)
         with pytest.raises(lbm.LBMError):
-            lbm.lbm_set_geometry(h, None, lbm.LBM_WALL_NODAL, 8 * 8 * 6)
+            lbm.lbm_set_geometry(h, None, 7, 8 * 8 * 8)  # unknown wall model
+        lbm.lbm_set_geometry(h, None, lbm.LBM_WALL_NODAL, 8 * 8 * 8)  # geometry on a slab is allowed (nz_local + 4 planes)
         plain = lbm.lbm_create(8, 8, 8, 19, 0.8)
         assert lbm.load().lbm_slab_export(plain, None) == lbm.LBM_EINVAL
         with pytest.raises(lbm.LBMError):
@@ -265,3 +266,100 @@ def test_two_processes_connected_through_cuda_ipc(mods, tmp_path):
     out = [json.loads(ln[3:]) for ln in r.stdout.splitlines() if ln.startswith("OUT")][-1]
     assert out["equal"], out
     assert out["mass_rel"] <= 1e-13 and out["umax_equal"]
+
+
+# --------------------------------------------------------------------------- solid masks, nodal walls, mirror planes on slabs
+def _oracle_geo_run(w, steps):
+    rho, u = w.fields()
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, eq=w.eq, face_kind=w.face_kind, face_u=w.face_u, force=w.force, face_rho=w.face_rho)
+    if w.has_geometry:
+        o.set_geometry(w.geo(), w.wall_model)
+    for k, prof in w.face_profiles().items():
+        o.set_face_velocity(k, prof)
+    o.init_equilibrium(rho, u)
+    o.step(steps)
+    out = o.get_f(), o.boundary_force() if w.has_geometry else None
+    o.close()
+    return out
+
+
+class _Lumpy(inputs.Workload):
+    """A workload whose mask has bodies next to every cut of a 2- / 3- / 4-slab split, on the z faces and single nodes."""
+
+    def geo(self):
+        nx, ny, nz = self.nx, self.ny, self.nz
+        g = inputs.sphere_mask(nx, ny, nz, (0.4 * nx, 0.5 * ny, 0.5 * nz), 0.3 * min(nx, ny, nz)).reshape(nz, ny, nx).copy()
+        g[0:2, 1:4, 2:5] = 1            # a block on the z- face
+        g[nz - 1, ny - 3:, nx - 4:] = 1  # a plate in the last plane
+        for z in range(nz):             # a thin diagonal rod through every plane
+            g[z, (2 + z) % ny, (nx - 2 - z) % nx] = 1
+        return g.reshape(-1)
+
+    @property
+    def has_geometry(self):
+        return True
+
+
+def _lumpy(dims, Q, tau, model, faces, eq=EQ_STANDARD, force=(0.0, 0.0, 0.0), steps=9):
+    S_, PR_ = inputs.FACE_SYMMETRY, inputs.FACE_PRESSURE
+    fu = np.zeros((6, 3))
+    for k in range(6):
+        if faces[k] == M:
+            fu[k] = (0.03, 0.0, 0.01 if k < 4 else 0.0)
+    return _Lumpy(f"lumpy_{Q}_{model}", dims[0], dims[1], dims[2], Q, tau, steps, face_kind=tuple(faces),
+                  face_u=tuple(map(tuple, fu)), force=tuple(force), noise=1e-3, seed=inputs.SEED_BASE + 91, kind="rest",
+                  eq=eq, wall_model=model, face_rho=(1.0, 0.99, 1.0, 1.0, 1.01, 0.98))
+
+
+_S, _PR = inputs.FACE_SYMMETRY, inputs.FACE_PRESSURE
+GEO_CASES = {
+    "periodic_q19_forced": dict(dims=(20, 12, 12), Q=19, tau=0.8, faces=[P] * 6, force=(1e-5, 0, 2e-6)),
+    "zwalls_q27": dict(dims=(14, 10, 13), Q=27, tau=0.7, faces=[P, P, P, P, B, B], force=(2e-5, 0, 0)),
+    "sphere_case_faces_q27": dict(dims=(22, 8, 12), Q=27, tau=0.6, faces=[M, _PR, _S, _S, P, P], eq=EQ_INCOMP),
+    "open_z_mirror_x_q19": dict(dims=(10, 9, 14), Q=19, tau=0.66, faces=[_S, _S, B, B, M, _PR]),
+}
+
+
+@pytest.mark.parametrize("nslabs", [2, 3, 4])
+@pytest.mark.parametrize("model", [inputs.WALL_HALFWAY, inputs.WALL_NODAL], ids=["halfway", "nodal"])
+@pytest.mark.parametrize("case", list(GEO_CASES))
+def test_slabs_with_geometry_equal_the_undivided_box(mods, case, model, nslabs):
+    """lbm_set_geometry on slab handles (mask with two halo planes per side): solid bodies across the cuts, nodal wall
+    nodes in the halo planes, mirror planes and open faces — bit-identical to the undivided CUDA run, 1e-12 from the
+    oracle, and the slabs' parts of Eq. 13 add up to the whole force."""
+    lbm, slabs = mods
+    w = _lumpy(model=model, **GEO_CASES[case])
+    ref, Fref = _oracle_geo_run(w, w.steps)
+    rho, u = w.fields()
+    s = lbm.Solver.from_workload(w)
+    s.init_equilibrium(torch.from_numpy(rho).cuda(), torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).cuda())
+    s.step(w.steps)
+    one = s.get_populations().clone()
+    F1 = s.boundary_force()
+    s.close()
+    assert float(np.abs(one.cpu().numpy() - ref).max()) <= TOL
+    g = slabs.SlabGroup(w, nslabs)
+    g.init_equilibrium()
+    g.step(w.steps)
+    f = g.get_populations()
+    F = g.boundary_force()
+    g.close()
+    assert torch.equal(f, one), f"{case}: slabs differ from the undivided CUDA run by {float((f - one).abs().max())}"
+    assert np.abs(F - F1).max() <= 1e-12 * max(1.0, np.abs(F1).max())
+    assert np.abs(F - Fref).max() <= 1e-12 * max(1.0, np.abs(Fref).max())
+
+
+def test_sphere_case_on_slabs(mods):
+    """inputs.config(8) (the paper's sphere case with its boundaries) shrunk by 4, cut into 4 slabs: the cut
+    at z = 16 goes through the sphere."""
+    lbm, slabs = mods
+    w = inputs.config(8).shrunk(4, steps=60)
+    ref, Fref = _oracle_geo_run(w, w.steps)
+    g = slabs.SlabGroup(w, 4)
+    g.init_equilibrium()
+    g.step(w.steps)
+    f = g.get_populations().cpu().numpy()
+    F = g.boundary_force()
+    g.close()
+    assert np.abs(f - ref).max() <= TOL
+    assert np.abs(F - Fref).max() <= 1e-12

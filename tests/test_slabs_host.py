@@ -129,3 +129,20 @@ def test_descriptor_exchange_and_diagnostics_gloo_world2(tmp_path):
         assert o["bufs"] == [1000, 1001] and o["nzl"] == [5, 4] and o["pids_differ"]
         assert (o["lo"], o["up"]) == ((1, 1) if o["rank"] == 0 else (0, 0))
         assert o["tot"] == [30.0, 1.0, -1.0, 2.0, 1.0, 0.02, 0.9, 1.0]
+
+
+def test_slab_mask_carries_two_halo_planes_per_side():
+    """include/lbm.h: on a slab lbm_set_geometry takes nz_local + 4 planes, plane 2 + (z - z0); periodic z wraps, planes
+    beyond a non-periodic z face are empty."""
+    nx, ny, nz = 4, 3, 7
+    geo = (np.arange(nx * ny * nz) % 3 == 0).astype(np.uint8)
+    g = geo.reshape(nz, ny * nx)
+    for z0, nzl in slabs.partition(nz, 3):
+        m = slabs.slab_mask(geo, nx, ny, nz, z0, nzl, True).reshape(nzl + 4, ny * nx)
+        for k in range(nzl + 4):
+            assert (m[k] == g[(z0 - 2 + k) % nz]).all()
+        m = slabs.slab_mask(geo, nx, ny, nz, z0, nzl, False).reshape(nzl + 4, ny * nx)
+        for k in range(nzl + 4):
+            z = z0 - 2 + k
+            assert (m[k] == (g[z] if 0 <= z < nz else 0)).all()
+    assert slabs.slab_mask(None, nx, ny, nz, 0, 3, True).sum() == 0
