@@ -374,7 +374,7 @@ def run_gpu_slabs(args, w):
     if rank != 0:
         replicas.finalize()
         return 0
-    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8)
+    bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8) + (4 if w.has_geometry else 0)
     peak, peak_src = measured_peak()
     achieved = bytes_per_cell * units / secs_max / 1e9 / world  # per GPU
     halo_dirs = sum(1 for ez in _EZ[w.Q] if ez == 1)
