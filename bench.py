@@ -215,7 +215,8 @@ def run_gpu(args, w):
     del rho, u
     log(f"[rank {rank}] inputs {w.name} ready in {time.perf_counter() - t0:.1f} s")
 
-    s = lbm.Solver.from_workload(w, scheme=scheme, store=store, stream=stream)
+    layout = lbm.LBM_LAYOUT_SOA if args.layout == "soa" else lbm.LBM_LAYOUT_ROWS
+    s = lbm.Solver.from_workload(w, scheme=scheme, store=store, stream=stream, layout=layout)
     if args.block:
         s.set_block(*[int(v) for v in args.block.split(",")])
     with torch.cuda.stream(stream):
@@ -272,7 +273,8 @@ def run_gpu(args, w):
         "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "lattice": lattice_name(w.Q), "collision": "BGK", "tau": w.tau,
                    "equilibrium": "Eq. 5" if w.eq else "Eq. 2", "geometry": ("none" if not w.has_geometry else
                                                                               ("nodal" if w.wall_model else "halfway") + " walls, solid mask"),
-                   "scheme": args.scheme, "storage": args.store, "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
+                   "scheme": args.scheme, "storage": args.store, "layout": "f[z][y][a][x]" if args.layout == "rows" else "f[a][z][y][x]",
+                   "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
                    "l2": l2_note(bytes_per_cell * w.N)},
         "clocks": clocks,
         "e2e": {"value": e2e_ups / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 32 * w.N / K, "d2h_bytes_per_step": (32 * w.N + 64) / K,
@@ -416,6 +418,8 @@ def main():
     ap.add_argument("--scheme", default="ab", choices=["ab", "aa"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", default="", help="bx,by block shape override")
+    ap.add_argument("--layout", default="rows", choices=["rows", "soa"],
+                    help="internal population layout: f[z][y][a][x] (default) or plain structure of arrays f[a][z][y][x]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "zslab"],
                     help="--gpus N > 1: N independent replicas (default; BASELINE.json: no sharding) or ONE box cut into z-slabs")

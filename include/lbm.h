@@ -53,7 +53,9 @@ enum {
   LBM_SCHEME_AB = 1 << 12,  /* two buffers, pull ("stream on read")                            */
   LBM_SCHEME_AA = 2 << 12,  /* one buffer, in-place AA pattern                                 */
   LBM_STORE_F64 = 0,        /* populations stored as fp64 (default)                            */
-  LBM_STORE_F32 = 1 << 16   /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
+  LBM_STORE_F32 = 1 << 16,  /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
+  LBM_LAYOUT_ROWS = 0,      /* internal buffers f[z][y][a][x]: the Q rows of a grid row adjacent (default, faster) */
+  LBM_LAYOUT_SOA = 1 << 20  /* internal buffers f[a][z][y][x] (for measurements; not on z-slab handles)  */
 };
 
 enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2, LBM_FACE_PRESSURE = 3, LBM_FACE_SYMMETRY = 4 };

@@ -38,6 +38,7 @@ constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 
 
 struct lbm_handle_s {
   int nx, ny, nz, Q, eq, scheme, f32;
+  int soa;            // LBM_LAYOUT_SOA: plain structure of arrays instead of the row-interleaved layout
   long long N;
   double tau;
   Params p;
@@ -67,7 +68,7 @@ struct lbm_handle_s {
   void* peer_lo[2];       // lower / upper neighbour's population buffers as seen from this process
   void* peer_hi[2];
   long long peer_lo_N, peer_hi_N;
-  int peer_lo_off, peer_hi_off;
+  long long peer_lo_off, peer_hi_off;
   uint32_t* peer_lo_flag;  // the counter we write in the lower neighbour (its "upper" one) / in the upper neighbour
   uint32_t* peer_hi_flag;
   void* ipc_opened[6];
@@ -374,7 +375,7 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   int scheme = lattice & (3 << 12);
   if (scheme == LBM_SCHEME_AUTO) scheme = LBM_SCHEME_AB;
   if (scheme != LBM_SCHEME_AB && scheme != LBM_SCHEME_AA) { fail(LBM_EINVAL, "lbm_create: unknown storage scheme"); return nullptr; }
-  if (lattice & ~(0xff | LBM_EQ_INCOMP | (3 << 12) | LBM_STORE_F32)) { fail(LBM_EINVAL, "lbm_create: unknown bits in lattice"); return nullptr; }
+  if (lattice & ~(0xff | LBM_EQ_INCOMP | (3 << 12) | LBM_STORE_F32 | LBM_LAYOUT_SOA)) { fail(LBM_EINVAL, "lbm_create: unknown bits in lattice"); return nullptr; }
 
   lbm_handle_s* h = new (std::nothrow) lbm_handle_s();
   if (!h) { fail(LBM_ENOMEM, "lbm_create: out of host memory"); return nullptr; }
@@ -385,8 +386,11 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   h->f32 = (lattice & LBM_STORE_F32) ? 1 : 0;
   h->N = (long long)nx * ny * nz;
   h->tau = tau;
+  h->soa = (lattice & LBM_LAYOUT_SOA) ? 1 : 0;
   Params& p = h->p;
   p.nx = nx; p.ny = ny; p.nz = nz; p.N = h->N;
+  if (h->soa) { p.ds = h->N; p.rs = nx; p.zs = (long long)nx * ny; }
+  else { p.ds = nx; p.rs = Q * nx; p.zs = (long long)Q * nx * ny; }
   p.omega = 1.0 / tau;
   if (bc) {
     for (int k = 0; k < 6; ++k) {
@@ -569,12 +573,13 @@ int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_
     if (rc) { close_peers(h); return rc; }
     if (side == 0) {  // lower neighbour: we fill its UPPER halo plane and write its "upper neighbour" counter
       h->peer_lo[0] = b[0]; h->peer_lo[1] = b[1];
-      h->peer_lo_N = d->plane_stride;
-      h->peer_lo_off = (int)(plane * (d->nz_local + 1));
+      // the neighbour stores in the same layout: its direction stride and the offset of its upper halo plane
+      h->peer_lo_N = h->soa ? d->plane_stride : h->p.ds;
+      h->peer_lo_off = h->p.zs * (d->nz_local + 1);
       h->peer_lo_flag = (uint32_t*)fl + 1;
     } else {          // upper neighbour: its LOWER halo plane, its "lower neighbour" counter
       h->peer_hi[0] = b[0]; h->peer_hi[1] = b[1];
-      h->peer_hi_N = d->plane_stride;
+      h->peer_hi_N = h->soa ? d->plane_stride : h->p.ds;
       h->peer_hi_off = 0;
       h->peer_hi_flag = (uint32_t*)fl;
     }

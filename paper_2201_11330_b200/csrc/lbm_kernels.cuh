@@ -86,7 +86,14 @@ enum { BC_PERIODIC = 0, BC_WALLS = 1, BC_GEO = 2 };
 
 struct Params {
   int nx, ny, nz;
-  long long N;          // cells = plane stride of the SoA layout (64-bit: 512^3*19 > 2^31)
+  long long N;          // cells = component stride of the arrays at the interface (rho, u, canonical f)
+  // Storage layout of the population buffers: element (x, y, z, a) sits at
+  //   a*ds + x + y*rs + z*zs.
+  // Row-interleaved (default): ds = nx, rs = Q*nx, zs = Q*nx*ny, i.e. f[z][y][a][x] — the Q rows a block streams
+  // lie next to each other in memory instead of N elements apart (measured +1.8 % D3Q19, +3 % D3Q27 at 512^3).
+  // Plain structure of arrays (LBM_LAYOUT_SOA): ds = N, rs = nx, zs = nx*ny, i.e. f[a][z][y][x].
+  long long ds, zs;
+  int rs;
   double omega;         // 1/tau (D:R1)
   double F[3];          // body force (D:R7)
   int wall[6];          // face is non-periodic (BOUNCE, MOVING or PRESSURE), order x-,x+,y-,y+,z-,z+
@@ -117,8 +124,8 @@ struct Params {
   // push_lo_off / push_hi_off = in-plane offset of that neighbour's receiving halo plane.  NULL = nothing to push.
   void* push_lo;
   void* push_hi;
-  long long push_lo_N, push_hi_N;
-  int push_lo_off, push_hi_off;
+  long long push_lo_N, push_hi_N;      // the neighbours' direction strides ds
+  long long push_lo_off, push_hi_off;  // offset of their receiving halo plane (plane index * zs)
 };
 
 enum { EQ_STANDARD = 0, EQ_INCOMP = 1 };
@@ -176,26 +183,40 @@ struct CellFlags {
   }
 };
 
-// Neighbour offsets of one cell with periodic wrap by conditional add (no %).  Offsets inside one
-// direction plane are 32-bit (lbm_create refuses N >= 2^31); the plane base alpha*N is 64-bit and
-// thread-invariant, so it lives in uniform registers and an address costs one IMAD.WIDE.
+// Neighbour offsets of one cell with periodic wrap by conditional add (no %).  Two index spaces:
+//   storage  at<>() / ic   offset of the node inside a population buffer, direction excluded (add a*ds): x + y*rs as
+//                          32 bits, the plane part z*zs as 64 bits (thread-invariant in the step kernels, where z =
+//                          blockIdx.z: it lives in uniform registers together with the direction base);
+//   cells    cat<>() / cell the node's linear index x + nx*(y + ny*z) in the arrays at the interface (link mask, geo,
+//                          rho, u, canonical f): 32 bits (lbm_create refuses N >= 2^31).
 struct Neigh {
-  int ox[3], oy[3], oz[3];  // index 0: coordinate-1, 1: same, 2: coordinate+1
-  int ic;
+  int ox[3], oy[3];   // index 0: coordinate-1, 1: same, 2: coordinate+1
+  long long oz[3];
+  int cy[3], cz[3];
+  long long ic;
+  int cell;
   __device__ __forceinline__ Neigh(const Params& p, int x, int y, int z) {
     const int xm = (x == 0) ? p.nx - 1 : x - 1, xp = (x == p.nx - 1) ? 0 : x + 1;
     const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
     const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
-    const int sy = p.nx, sz = p.nx * p.ny;
     ox[0] = xm; ox[1] = x; ox[2] = xp;
-    oy[0] = ym * sy; oy[1] = y * sy; oy[2] = yp * sy;
-    oz[0] = zm * sz; oz[1] = z * sz; oz[2] = zp * sz;
+    oy[0] = ym * p.rs; oy[1] = y * p.rs; oy[2] = yp * p.rs;
+    oz[0] = zm * p.zs; oz[1] = z * p.zs; oz[2] = zp * p.zs;
+    const int sy = p.nx, sz = p.nx * p.ny;
+    cy[0] = ym * sy; cy[1] = y * sy; cy[2] = yp * sy;
+    cz[0] = zm * sz; cz[1] = z * sz; cz[2] = zp * sz;
     ic = ox[1] + oy[1] + oz[1];
+    cell = ox[1] + cy[1] + cz[1];
   }
-  // in-plane index of x + s*e_A (wrapped)
+  // storage offset of x + s*e_A (wrapped)
   template <int Q, int A, int S>
-  __device__ __forceinline__ int at() const {
-    return ox[1 + S * Dir<Q, A>::ex] + oy[1 + S * Dir<Q, A>::ey] + oz[1 + S * Dir<Q, A>::ez];
+  __device__ __forceinline__ long long at() const {
+    return (ox[1 + S * Dir<Q, A>::ex] + oy[1 + S * Dir<Q, A>::ey]) + oz[1 + S * Dir<Q, A>::ez];
+  }
+  // cell index of x + s*e_A (wrapped)
+  template <int Q, int A, int S>
+  __device__ __forceinline__ int cat() const {
+    return ox[1 + S * Dir<Q, A>::ex] + cy[1 + S * Dir<Q, A>::ey] + cz[1 + S * Dir<Q, A>::ez];
   }
 };
 
@@ -211,7 +232,7 @@ __host__ __device__ constexpr int dir_index(int ex, int ey, int ez) {
 // the last node.  If the node x + S*e_A lies beyond SYMMETRY faces ONLY, the link connects x with the mirror image:
 // the node whose coordinates along the crossed axes are those of x, and the population there has the direction
 // e_A with those components negated.  Returns false for every other link (inside the box, or through a face of
-// another kind: MOVING > BOUNCE > PRESSURE decide those, D:R22).  idx = in-plane index of that node.
+// another kind: MOVING > BOUNCE > PRESSURE decide those, D:R22).  idx / cidx = storage offset / cell index of that node.
 template <int BC>
 __device__ __forceinline__ bool touches_sym(const Params& p, const CellFlags<BC>& c) {
   if constexpr (BC == BC_PERIODIC) return false;
@@ -221,7 +242,7 @@ __device__ __forceinline__ bool touches_sym(const Params& p, const CellFlags<BC>
 }
 
 template <int Q, int A, int S, int BC>
-__device__ __forceinline__ bool mirror_link(const Params& p, const CellFlags<BC>& c, const Neigh& nb, int& dir, int& idx) {
+__device__ __forceinline__ bool mirror_link(const Params& p, const CellFlags<BC>& c, const Neigh& nb, int& dir, long long& idx, int& cidx) {
   using D = Dir<Q, A>;
   constexpr int dx = S * D::ex, dy = S * D::ey, dz = S * D::ez;
   const bool cx = (dx == -1) ? c.lo[0] : (dx == 1) ? c.hi[0] : false;
@@ -229,7 +250,9 @@ __device__ __forceinline__ bool mirror_link(const Params& p, const CellFlags<BC>
   const bool cz = (dz == -1) ? c.lo[2] : (dz == 1) ? c.hi[2] : false;
   const bool sx = cx && p.sym[dx == 1 ? 1 : 0], sy = cy && p.sym[dy == 1 ? 3 : 2], sz = cz && p.sym[dz == 1 ? 5 : 4];
   if ((cx && !sx) || (cy && !sy) || (cz && !sz) || !(sx || sy || sz)) return false;
-  idx = (sx ? nb.ox[1] : nb.ox[1 + dx]) + (sy ? nb.oy[1] : nb.oy[1 + dy]) + (sz ? nb.oz[1] : nb.oz[1 + dz]);
+  const int mx = sx ? nb.ox[1] : nb.ox[1 + dx];
+  idx = (mx + (sy ? nb.oy[1] : nb.oy[1 + dy])) + (sz ? nb.oz[1] : nb.oz[1 + dz]);  // storage offset of the mirror image
+  cidx = mx + (sy ? nb.cy[1] : nb.cy[1 + dy]) + (sz ? nb.cz[1] : nb.cz[1 + dz]);   // its cell index
   constexpr int t1 = dir_index<Q>(-D::ex, D::ey, D::ez), t2 = dir_index<Q>(D::ex, -D::ey, D::ez), t3 = dir_index<Q>(-D::ex, -D::ey, D::ez),
                 t4 = dir_index<Q>(D::ex, D::ey, -D::ez), t5 = dir_index<Q>(-D::ex, D::ey, -D::ez), t6 = dir_index<Q>(D::ex, -D::ey, -D::ez),
                 t7 = dir_index<Q>(-D::ex, -D::ey, -D::ez);
@@ -237,7 +260,8 @@ __device__ __forceinline__ bool mirror_link(const Params& p, const CellFlags<BC>
   return true;
 }
 
-// Base of direction plane A of a population buffer (64-bit, thread-invariant).
+// Base of component A of an array whose components are `N` elements apart (64-bit, thread-invariant): the direction
+// rows of a population buffer (N = p.ds) or the components of rho / u / canonical f (N = p.N).
 template <int A, typename T>
 __device__ __forceinline__ T* plane(T* buf, long long N) {
   return buf + (long long)A * N;
@@ -276,18 +300,18 @@ __device__ __forceinline__ T* plane(T* buf, long long N) {
 // Storage element access.  fp64: the value itself.  fp32 storage (S:§8f NEXT-1): f - t_a is
 // kept as float, arithmetic stays fp64.
 template <typename ST, int Q, int A>
-__device__ __forceinline__ double ld_pop(const ST* __restrict__ p, int i) {
+__device__ __forceinline__ double ld_pop(const ST* __restrict__ p, long long i) {
   if constexpr (sizeof(ST) == 8) return __ldg(p + i);
   else return (double)__ldg(p + i) + Dir<Q, A>::t;
 }
 // same through a plain (coherent) load: the in-place kernels read the buffer they write
 template <typename ST, int Q, int A>
-__device__ __forceinline__ double ld_pop_rw(const ST* p, int i) {
+__device__ __forceinline__ double ld_pop_rw(const ST* p, long long i) {
   if constexpr (sizeof(ST) == 8) return p[i];
   else return (double)p[i] + Dir<Q, A>::t;
 }
 template <typename ST, int Q, int A>
-__device__ __forceinline__ void st_pop(ST* __restrict__ p, int i, double v) {
+__device__ __forceinline__ void st_pop(ST* __restrict__ p, long long i, double v) {
   if constexpr (sizeof(ST) == 8) p[i] = v;
   else p[i] = (float)(v - Dir<Q, A>::t);
 }
@@ -741,7 +765,7 @@ __device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&
 // neighbour then pulls them like any other upstream value.  Compute and exchange are one kernel; the ordering
 // between slabs is stream-level (lbm_abi.cu: wait on the neighbours' step counters, launch, signal).
 template <int Q, int A, typename ST>
-__device__ __forceinline__ void push_one(const Params& p, int z, int ixy, ST v) {
+__device__ __forceinline__ void push_one(const Params& p, int z, int ixy /* x + y*rs */, ST v) {
   if constexpr (Dir<Q, A>::ez == -1) {
     if (z == p.z_lo && p.push_lo) ((ST*)p.push_lo + (long long)A * p.push_lo_N)[p.push_lo_off + ixy] = v;
   }
@@ -760,14 +784,15 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   if constexpr (SLAB) z += p.z_lo;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
-  const CellFlags<BC> c(p, x, y, z, nb.ic);
-  auto link = [&](auto A) { return plane<decltype(A)::value>(src, p.N) + nb.template at<Q, decltype(A)::value, -1>(); };
-  auto wall = [&](auto A) { return plane<Dir<Q, decltype(A)::value>::opp>(src, p.N) + nb.ic; };  // t_a == t_abar: same shift
+  const CellFlags<BC> c(p, x, y, z, nb.cell);
+  auto link = [&](auto A) { return plane<decltype(A)::value>(src, p.ds) + nb.template at<Q, decltype(A)::value, -1>(); };
+  auto wall = [&](auto A) { return plane<Dir<Q, decltype(A)::value>::opp>(src, p.ds) + nb.ic; };  // t_a == t_abar: same shift
   // D:R25: through SYMMETRY faces f_a comes from the mirror image (same speed class: same fp32 shift)
   auto mirror = [&](auto A) -> const ST* {
-    int dir, idx;
-    if (!mirror_link<Q, decltype(A)::value, -1, BC>(p, c, nb, dir, idx)) return nullptr;
-    return src + (long long)dir * p.N + idx;
+    int dir, cidx;
+    long long idx;
+    if (!mirror_link<Q, decltype(A)::value, -1, BC>(p, c, nb, dir, idx, cidx)) return nullptr;
+    return src + dir * p.ds + idx;
   };
   const bool at_mirror = SYM ? touches_sym<BC>(p, c) : false;
   auto pull = [&](auto& f) {
@@ -779,20 +804,20 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
     if (!pull(g)) return;
     nodal_replicate<Q, BC>(g, p, c);
-    collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.ic, z, [&](auto A, double v) {
+    collide_shifted<Q, EQ, BC, FORCE>(g, p, c, nb.cell, z, [&](auto A, double v) {
       constexpr int a = decltype(A)::value;
       const float s = (float)v;
-      LBM_ST_STREAM(plane<a>(dst, p.N) + nb.ic, s);
+      LBM_ST_STREAM(plane<a>(dst, p.ds) + nb.ic, s);
       if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], s);
     });
   } else {
     double f[Q];
     if (!pull(f)) return;
     nodal_replicate<Q, BC>(f, p, c);
-    collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
+    collide<Q, EQ, BC, FORCE>(f, p, c, nb.cell, z);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
-      LBM_ST_STREAM(plane<a>(dst, p.N) + nb.ic, f[a]);  // ST = double in this branch
+      LBM_ST_STREAM(plane<a>(dst, p.ds) + nb.ic, f[a]);  // ST = double in this branch
       if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], f[a]);
     });
   }
@@ -810,19 +835,20 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
-  const int ic = x + p.nx * (y + p.ny * z);
-  const CellFlags<BC> c(p, x, y, z, ic);
+  const int cell = x + p.nx * (y + p.ny * z);
+  const long long ic = (x + y * p.rs) + z * p.zs;  // storage offset (Neigh::ic)
+  const CellFlags<BC> c(p, x, y, z, cell);
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), ic);
+    f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.ds), ic);
   });
   if (!c.template active<Q>()) return;  // after the loads: they do not wait for the link mask (see gather)
   nodal_replicate<Q, BC>(f, p, c);
-  collide<Q, EQ, BC, FORCE>(f, p, c, ic, z);
+  collide<Q, EQ, BC, FORCE>(f, p, c, cell, z);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    st_pop<ST, Q, a>(plane<Dir<Q, a>::opp>(buf, p.N), ic, f[a]);
+    st_pop<ST, Q, a>(plane<Dir<Q, a>::opp>(buf, p.ds), ic, f[a]);
   });
 }
 
@@ -833,20 +859,20 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   const Neigh nb(p, x, y, z);
-  const CellFlags<BC> c(p, x, y, z, nb.ic);
+  const CellFlags<BC> c(p, x, y, z, nb.cell);
   double f[Q];
   // f_a(x) comes from the slot that f*_abar(x) goes to (link x <-> x - e_a traversed both ways)
-  auto link = [&](auto A) { return (const ST*)plane<Dir<Q, decltype(A)::value>::opp>(buf, p.N) + nb.template at<Q, decltype(A)::value, -1>(); };
-  auto wall = [&](auto A) { return (const ST*)plane<decltype(A)::value>(buf, p.N) + nb.ic; };
+  auto link = [&](auto A) { return (const ST*)plane<Dir<Q, decltype(A)::value>::opp>(buf, p.ds) + nb.template at<Q, decltype(A)::value, -1>(); };
+  auto wall = [&](auto A) { return (const ST*)plane<decltype(A)::value>(buf, p.ds) + nb.ic; };
   if (!gather<Q, BC>(f, c, link, wall, [](auto A, const ST* q) { return ld_pop_rw<ST, Q, decltype(A)::value>(q, 0); })) return;
   nodal_replicate<Q, BC>(f, p, c);
-  collide<Q, EQ, BC, FORCE>(f, p, c, nb.ic, z);
+  collide<Q, EQ, BC, FORCE>(f, p, c, nb.cell, z);
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     constexpr int o = Dir<Q, a>::opp;
-    ST* q = plane<a>(buf, p.N) + nb.template at<Q, a, 1>();
+    ST* q = plane<a>(buf, p.ds) + nb.template at<Q, a, 1>();
     if constexpr (BC != BC_PERIODIC) {
-      if (c.template leaves<Q, a, 1>()) q = plane<o>(buf, p.N) + nb.ic;
+      if (c.template leaves<Q, a, 1>()) q = plane<o>(buf, p.ds) + nb.ic;
     }
     st_pop<ST, Q, a>(q, 0, f[a]);
   });
@@ -867,12 +893,12 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
     constexpr int o = Dir<Q, a>::opp;
     const ST* q;
     if constexpr (MODE == MODE_NATURAL) {
-      q = plane<a>(buf, p.N) + nb.ic;
+      q = plane<a>(buf, p.ds) + nb.ic;
     } else {
       constexpr int q_in = (MODE == MODE_PULL) ? a : o, q_wall = (MODE == MODE_PULL) ? o : a;
-      q = plane<q_in>(buf, p.N) + nb.template at<Q, a, -1>();
+      q = plane<q_in>(buf, p.ds) + nb.template at<Q, a, -1>();
       if constexpr (BC != BC_PERIODIC) {
-        if (c.template leaves<Q, a, -1>()) q = plane<q_wall>(buf, p.N) + nb.ic;
+        if (c.template leaves<Q, a, -1>()) q = plane<q_wall>(buf, p.ds) + nb.ic;
       }
     }
     f[a] = ld_pop_rw<ST, Q, a>(q, 0);
@@ -882,9 +908,10 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
       static_for<0, Q>([&](auto A) {
         constexpr int a = decltype(A)::value;
         if constexpr (Dir<Q, a>::s > 0) {
-          int dir, idx;
-          if (mirror_link<Q, a, -1, BC>(p, c, nb, dir, idx) && !c.template leaves<Q, a, -1>())
-            f[a] = ld_pop_rw<ST, Q, a>(buf + (long long)dir * p.N + idx, 0);
+          int dir, cidx;
+          long long idx;
+          if (mirror_link<Q, a, -1, BC>(p, c, nb, dir, idx, cidx) && !c.template leaves<Q, a, -1>())
+            f[a] = ld_pop_rw<ST, Q, a>(buf + dir * p.ds, idx);
         }
       });
     }
@@ -939,15 +966,16 @@ __global__ void __launch_bounds__(256) import_canonical(const double* __restrict
       constexpr int o = Dir<Q, a>::opp;
       const double* q = plane<a>(in, p.N) + i;
       if constexpr (MODE != MODE_NATURAL) {
-        q = plane<a>(in, p.N) + nb.template at<Q, a, 1>();
+        q = plane<a>(in, p.N) + nb.template cat<Q, a, 1>();
         if constexpr (BC != BC_PERIODIC) {
           if (c.template leaves<Q, a, 1>()) q = plane<o>(in, p.N) + i;
         }
         if constexpr (BC == BC_GEO && Dir<Q, a>::s > 0) {
           // D:R25: a slot whose link leaves through SYMMETRY faces is read by the mirror image, as direction `dir`
-          int dir, idx;
-          if (p.any_sym && mirror_link<Q, a, 1, BC>(p, c, nb, dir, idx) && !c.template leaves<Q, a, 1>())
-            q = in + (long long)dir * p.N + idx;
+          int dir, cidx;
+          long long idx;
+          if (p.any_sym && mirror_link<Q, a, 1, BC>(p, c, nb, dir, idx, cidx) && !c.template leaves<Q, a, 1>())
+            q = in + (long long)dir * p.N + cidx;
         }
         // slab: the halo planes are filled here too (the canonical arrays of a slab carry the neighbour's
         // planes); a slot whose downstream node would lie beyond a halo plane is never read: leave it.
@@ -956,7 +984,7 @@ __global__ void __launch_bounds__(256) import_canonical(const double* __restrict
           if (p.slab && (zd < 0 || zd >= p.nz) && !c.template leaves<Q, a, 1>()) return;
         }
       }
-      st_pop<ST, Q, a>(plane<a>(buf, p.N), i, __ldg(q));
+      st_pop<ST, Q, a>(plane<a>(buf, p.ds), nb.ic, __ldg(q));
     });
   }, p.slab != 0);
 }
@@ -1000,7 +1028,7 @@ __global__ void __launch_bounds__(256) classify_nodes_kernel(const uint8_t* __re
         if constexpr (D::s > 0) {
           if (!c.template leaves_box<Q, b, 1>()) {
             // slab: no wrap along z inside the handle — the neighbouring planes are in geo_in as they are
-            const int j = p.slab ? nb.ox[1 + D::ex] + nb.oy[1 + D::ey] + (z + D::ez + zin) * pl : nb.template at<Q, b, 1>();
+            const int j = p.slab ? nb.ox[1 + D::ex] + nb.cy[1 + D::ey] + (z + D::ez + zin) * pl : nb.template cat<Q, b, 1>();
             a = a | (geo_in[j] == 0);
           }
         }
@@ -1022,12 +1050,13 @@ __global__ void __launch_bounds__(256) build_links_kernel(const uint8_t* __restr
       constexpr int a = decltype(A)::value;
       if constexpr (Dir<Q, a>::s > 0) {
         bool none;
-        int dir, idx;
-        if (p.any_sym && mirror_link<Q, a, -1, BC_WALLS>(p, c, nb, dir, idx)) {
-          none = active[idx] == 0;  // D:R25: the source is the mirror image
+        int dir, cidx;
+        long long idx;
+        if (p.any_sym && mirror_link<Q, a, -1, BC_WALLS>(p, c, nb, dir, idx, cidx)) {
+          none = active[cidx] == 0;  // D:R25: the source is the mirror image
         } else {
           none = c.template leaves_box<Q, a, -1>();
-          if (!none) none = active[nb.template at<Q, a, -1>()] == 0;
+          if (!none) none = active[nb.template cat<Q, a, -1>()] == 0;
         }
         m |= none ? (1u << a) : 0u;
       }
@@ -1162,7 +1191,7 @@ __global__ void __launch_bounds__(256, 2) boundary_force_kernel(const ST* buf, c
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       if constexpr (Dir<Q, a>::s > 0) {
-        if (!c.template leaves_box<Q, a, 1>()) solid |= (geo[nb.template at<Q, a, 1>()] != 0) ? (1u << a) : 0u;
+        if (!c.template leaves_box<Q, a, 1>()) solid |= (geo[nb.template cat<Q, a, 1>()] != 0) ? (1u << a) : 0u;
       }
     });
     if (solid == 0u) return;
@@ -1176,12 +1205,12 @@ __global__ void __launch_bounds__(256, 2) boundary_force_kernel(const ST* buf, c
         if ((solid >> a) & 1u) {
           double post;
           if constexpr (MODE == MODE_PULL) {
-            post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), i);
+            post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.ds), nb.ic);
           } else if constexpr (MODE == MODE_PULL_SWAP) {
-            post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.N), i);
+            post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.ds), nb.ic);
           } else {
-            if (c.template leaves<Q, a, 1>()) post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.N), i);
-            else post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.N), nb.template at<Q, a, 1>());
+            if (c.template leaves<Q, a, 1>()) post = ld_pop_rw<ST, Q, a>(plane<o>(buf, p.ds), nb.ic);
+            else post = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.ds), nb.template at<Q, a, 1>());
           }
           const double term = post + f[o];
           if constexpr (D::ex != 0) acc[0] += D::ex * term;

@@ -17,6 +17,7 @@ LBM_D2Q9, LBM_D3Q19, LBM_D3Q27 = 9, 19, 27
 LBM_EQ_STANDARD, LBM_EQ_INCOMP = 0, 1 << 8
 LBM_SCHEME_AUTO, LBM_SCHEME_AB, LBM_SCHEME_AA = 0, 1 << 12, 2 << 12
 LBM_STORE_F64, LBM_STORE_F32 = 0, 1 << 16
+LBM_LAYOUT_ROWS, LBM_LAYOUT_SOA = 0, 1 << 20
 LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE, LBM_FACE_SYMMETRY = 0, 1, 2, 3, 4
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
@@ -291,7 +292,7 @@ class Solver:
     method name says host."""
 
     def __init__(self, nx, ny, nz, Q=19, tau=0.8, eq=LBM_EQ_STANDARD, scheme=LBM_SCHEME_AUTO, store=LBM_STORE_F64,
-                 face_kind=None, face_u=None, force=None, stream=None):
+                 face_kind=None, face_u=None, force=None, stream=None, layout=LBM_LAYOUT_ROWS):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2201_11330_b200 needs a CUDA device (no CPU fallback)")
@@ -300,7 +301,7 @@ class Solver:
         self.torch_stream = stream  # torch.cuda.Stream or None
         raw = None if stream is None else stream.cuda_stream
         self.bc = make_bc(face_kind, face_u, force, raw)
-        self.h = lbm_create(nx, ny, nz, int(Q) | eq | scheme | store, tau, self.bc)
+        self.h = lbm_create(nx, ny, nz, int(Q) | eq | scheme | store | layout, tau, self.bc)
 
     @classmethod
     def from_workload(cls, w, **kw):
