@@ -3,7 +3,8 @@
 // P:n = PAPER.md line n; D:Rk = DESIGN.md §2 reading k; S:§8 = SURVEY.md hot-path table.
 // Everything here is HBM-bound (S:§8d: 2*Q*8 B per lattice update, ~1 flop/B): no tensor
 // cores, no shared-memory staging; one thread owns one cell, the Q populations live in
-// registers, every per-direction stream is unit-stride in x (SoA f[a][z][y][x]).
+// registers, every per-direction stream is unit-stride in x (rows f[z][y][a][x]: the Q rows of one grid row are
+// adjacent).
 #pragma once
 #include <type_traits>
 #include <cstdint>
