@@ -414,7 +414,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3,
-                    help="index into BASELINE.json configs (default 3 = 512^3 headline); 5 = the paper's sphere case")
+                    help="index into BASELINE.json configs (default 3 = 512^3 headline); 5 / 8 = the paper's sphere case (periodic box / its own "
+                         "boundaries), 6 / 7 = its 2-D channel-cylinder cases")
     ap.add_argument("--scheme", default="ab", choices=["ab", "aa"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", default="", help="bx,by block shape override")
