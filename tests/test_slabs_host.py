@@ -2,6 +2,7 @@
 the neighbour map, the halo boxes of the seeded inputs, the combination of the per-slab diagnostics, and — with
 two gloo processes — the exchange of slab descriptors and the three all-reduces of the diagnostics."""
 import json
+import re
 import os
 import socket
 import subprocess
@@ -123,7 +124,8 @@ def test_descriptor_exchange_and_diagnostics_gloo_world2(tmp_path):
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), str(script)]
     r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=240)
     assert r.returncode == 0, r.stderr[-2000:]
-    outs = [json.loads(ln[3:]) for ln in r.stdout.splitlines() if ln.startswith("OUT")]
+    # the two ranks share one pipe: their lines can arrive glued together
+    outs = [json.loads(m) for m in re.findall(r"OUT(\{[^{}]*\})", r.stdout)]
     assert len(outs) == 2
     for o in outs:
         assert o["bufs"] == [1000, 1001] and o["nzl"] == [5, 4] and o["pids_differ"]
