@@ -487,3 +487,42 @@ def test_storage_layouts_give_identical_results(lbm, scheme):
             out.append((s.get_populations().clone(), s.moments()[0].clone()))
             s.close()
         assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_large_box_equals_its_periodic_tile(lbm, scheme):
+    """Maximum sizes: 640^3 D3Q19 (Q*N = 4.98e9 stored elements: offsets beyond 2^32, 40 GB per buffer) started from a
+    128^3 field tiled 5 x 5 x 5.  A periodic flow whose period divides the box evolves exactly like the small periodic
+    box (same arithmetic per cell), so after an odd number of steps rho and u of the large box are the small box's,
+    tile by tile, bit for bit — and the small box is compared with the oracle elsewhere in this file."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs 120 GB of free device memory")
+    n, k, steps = 128, 5, 7
+    w = inputs.config(1).scaled(n, steps=steps)
+    rho, u = w.fields()
+    rho_s = torch.from_numpy(rho).cuda()
+    u_s = torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).cuda()
+    sch = {"ab": lbm.LBM_SCHEME_AB, "aa": lbm.LBM_SCHEME_AA}[scheme]
+    s = lbm.Solver.from_workload(w, scheme=sch)
+    s.init_equilibrium(rho_s, u_s)
+    s.step(steps)
+    r_small, u_small, d_small = s.moments()
+    r_small, u_small = r_small.clone().view(n, n, n), u_small.clone().view(3, n, n, n)
+    s.close()
+    N = n * k
+    big = lbm.Solver(N, N, N, 19, w.tau, scheme=sch)
+    rho_b = rho_s.view(n, n, n).repeat(k, k, k).reshape(-1)
+    u_b = u_s.view(3, n, n, n).repeat(1, k, k, k).reshape(-1)
+    big.init_equilibrium(rho_b, u_b)
+    del rho_b, u_b
+    big.step(steps)
+    r_big, u_big, d_big = big.moments()
+    big.close()
+    r_big, u_big = r_big.view(N, N, N), u_big.view(3, N, N, N)
+    for tz, ty, tx in ((0, 0, 0), (k - 1, k - 1, k - 1), (2, 4, 1), (4, 0, 3)):
+        sl = (slice(tz * n, (tz + 1) * n), slice(ty * n, (ty + 1) * n), slice(tx * n, (tx + 1) * n))
+        assert torch.equal(r_big[sl], r_small)
+        assert torch.equal(u_big[(slice(None),) + sl], u_small)
+    assert d_big[7] == 0 and d_big[5] == d_small[5] and d_big[6] == d_small[6]
+    assert abs(d_big[0] - k**3 * d_small[0]) <= 1e-12 * d_big[0]
