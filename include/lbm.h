@@ -215,7 +215,7 @@ int lbm_set_block(lbm_handle h, int bx, int by);
 typedef struct {
   uint64_t buf[2];        /* device addresses of the two population buffers (valid in the owner process) */
   uint64_t flags;         /* device address of the two step counters {written by lower, by upper neighbour} */
-  int64_t plane_stride;   /* cells per direction plane = nx*ny*(nz_local+2)                              */
+  int64_t plane_stride;   /* cells of the handle = nx*ny*(nz_local+2) (checked by lbm_slab_connect)             */
   int32_t nz_local;
   int32_t device;         /* CUDA device ordinal of the owner                                           */
   int64_t pid;            /* owner process                                                              */
