@@ -263,7 +263,9 @@ def run_gpu(args, w):
     # link mask of the geometry variant)
     bytes_per_cell = 2 * w.Q * (4 if args.store == "f32" else 8) + (4 if w.has_geometry else 0)
     ms_per_launch = secs / launches * 1e3
-    achieved = bytes_per_cell * w.N / (secs / launches) / 1e9
+    # algorithmic bytes of the timed region / its duration (a launch covers K / launches time steps: 1 for the large
+    # grids, all K for the small ones that run in the persistent kernel)
+    achieved = bytes_per_cell * w.N * K / secs / 1e9
     peak, peak_src = measured_peak()
     traffic = ncu_traffic(w.name, args.scheme + ("" if args.store == "f64" else "_f32"))
     out = {
@@ -282,7 +284,7 @@ def run_gpu(args, w):
                 "seconds": e2e_max},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                     "kernel": "stream_collide_" + args.scheme, "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch,
+                     "kernel": "stream_collide_" + args.scheme + ("_persistent" if launches < K else ""), "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch, "steps_per_launch": K / launches,
                      "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
         "checks": {"mass_drift_rel": abs(d_end[0] - d_init[0]) / d_init[0], "nonfinite_cells": d_end[7],
                    "kinetic_energy_ratio": d_end[4] / d_init[4] if d_init[4] else None, "e2e_mass": d_e2e[0]},

@@ -183,6 +183,12 @@ int64_t lbm_time(lbm_handle h);
 /* Number of kernels this handle has launched so far (bookkeeping for benchmarks). */
 int64_t lbm_launch_count(lbm_handle h);
 
+/* Small grids (every block of the step kernel resident on the device at once, e.g. 32^3 or the paper's 512 x 128
+ * channel) are bound by the launch rate of one kernel per step; for them lbm_step(h, n) takes all n steps in ONE
+ * cooperative launch of a persistent kernel (a grid-wide barrier separates the steps; same arithmetic per cell, same
+ * results bit for bit).  on = 0 switches that off (one launch per step, as for every larger grid); default on. */
+int lbm_set_persistent(lbm_handle h, int on);
+
 /* Tuning knob for measurements: CUDA block shape (threads along x, along y) of the
  * stream-collide kernel; 0,0 restores the default.  bx*by must be <= 256 and a multiple of 32. */
 int lbm_set_block(lbm_handle h, int bx, int by);

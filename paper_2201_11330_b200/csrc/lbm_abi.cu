@@ -33,6 +33,7 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 SMs
+constexpr long long kPersistentMaxBlocks = 148 * 16;  // upper bound of what can be co-resident; the launcher checks exactly
 
 }  // namespace
 
@@ -73,6 +74,7 @@ struct lbm_handle_s {
   uint32_t* peer_hi_flag;
   void* ipc_opened[6];
   int n_ipc_opened;
+  int persistent;     // lbm_step may take all steps of a call in one cooperative launch (small grids; lbm_set_persistent)
   int bx, by;         // block shape of the fused kernel (lbm_set_block), 0,0 = default_block()
   int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
   size_t elem() const { return f32 ? 4 : 8; }
@@ -82,6 +84,12 @@ struct lbm_handle_s {
 namespace {
 
 // Q dispatch: the per-lattice launchers live in lbm_inst.cu (one object per lattice and part).
+#define LBM_Q_CALL_RET(h, ret, fn, ...)                 \
+  do {                                                  \
+    if ((h)->Q == 19) ret = fn<19>(__VA_ARGS__);        \
+    else if ((h)->Q == 27) ret = fn<27>(__VA_ARGS__);   \
+    else ret = fn<9>(__VA_ARGS__);                      \
+  } while (0)
 #define LBM_Q_CALL(h, fn, ...)                 \
   do {                                         \
     if ((h)->Q == 19) fn<19>(__VA_ARGS__);     \
@@ -447,6 +455,7 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   int bx = 32;
   while (bx < nx && bx < 256) bx *= 2;
   h->bx = h->by = 0;  // default_block() at launch time (it depends on the geometry)
+  h->persistent = 1;
   h->fbx = bx;
 
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
@@ -749,6 +758,20 @@ int lbm_step(lbm_handle h, int nsteps) {
   if (nsteps < 0) return fail(LBM_EINVAL, "lbm_step: nsteps must be >= 0");
   if (nsteps == 0) return LBM_OK;
   Ctx c = make_ctx(h);
+  // Small grids: all steps of this call in ONE cooperative launch (stream_collide_ab_persistent) when the whole grid
+  // is resident at once; otherwise, and for slabs / in-place AA, one launch per step.
+  if (h->persistent && h->scheme == LBM_SCHEME_AB && !h->slab && nsteps >= 2 &&
+      (long long)c.grid.x * c.grid.y * c.grid.z <= kPersistentMaxBlocks) {
+    bool ok = false;
+    LBM_Q_CALL_RET(h, ok, launch_step_ab_persistent, c, h->buf[h->cur], h->buf[h->cur ^ 1], nsteps);
+    if (ok) {
+      h->cur ^= (nsteps & 1);
+      h->time += nsteps;
+      ++h->launches;
+      h->stepped = true;
+      return check_launch("lbm_step");
+    }
+  }
   for (int s = 0; s < nsteps; ++s) {
     if (h->slab) {
       int rc = launch_step_slab(h, c);
@@ -814,6 +837,12 @@ int lbm_set_populations(lbm_handle h, const double* f) {
 
 int64_t lbm_time(lbm_handle h) { return h ? h->time : -1; }
 int64_t lbm_launch_count(lbm_handle h) { return h ? h->launches : -1; }
+
+int lbm_set_persistent(lbm_handle h, int on) {
+  if (!h) return fail(LBM_EINVAL, "lbm_set_persistent: NULL handle");
+  h->persistent = on ? 1 : 0;
+  return LBM_OK;
+}
 
 int lbm_set_block(lbm_handle h, int bx, int by) {
   if (!h) return fail(LBM_EINVAL, "lbm_set_block: NULL handle");

@@ -2,12 +2,12 @@
 //   LBM_Q    9 | 19 | 27
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
 //            5 A/B step of a z-slab (fused halo push)   6 A/B step with SYMMETRY faces (link mask + mirror links)
-//            7 A/B step of a z-slab with SYMMETRY faces
+//            7 A/B step of a z-slab with SYMMETRY faces   8 persistent A/B kernel (all steps of a call in one launch)
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..7"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..8"
 #endif
 
 namespace lbm {
@@ -81,6 +81,52 @@ void launch_step_ab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
       });
     });
   });
+}
+#elif LBM_PART == 8
+namespace {
+// cooperative launch of one instantiation if the whole grid can be resident at once; false = use the per-step kernels
+template <typename K>
+bool launch_persistent(K kernel, const Ctx& c, void* b0, void* b1, int nsteps) {
+  int per_sm = 0, dev = 0, sms = 0, coop = 0;
+  const int threads = c.block.x * c.block.y * c.block.z;
+  if (cudaGetDevice(&dev) != cudaSuccess) return false;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  const long long blocks = (long long)c.grid.x * c.grid.y * c.grid.z;
+  if (blocks > (long long)per_sm * sms) return false;
+  Params p = c.p;
+  void* args[] = {&b0, &b1, &nsteps, &p};
+  if (cudaLaunchCooperativeKernel((const void*)kernel, c.grid, c.block, args, 0, c.stream) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return true;
+}
+}  // namespace
+
+template <>
+bool launch_step_ab_persistent<Q_>(const Ctx& c, void* b0, void* b1, int nsteps) {
+  bool ok = false;
+  if (c.p.any_sym) {
+    dispatch_eq(c, [&](auto eq) {
+      dispatch_force(c, [&](auto force) {
+        dispatch_storage(c, [&](auto st) {
+          using ST = decltype(st);
+          ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, ST, true>, c, b0, b1, nsteps);
+        });
+      });
+    });
+    return ok;
+  }
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST, false>, c, b0, b1, nsteps);
+  });
+  return ok;
 }
 #elif LBM_PART == 5
 template <>
@@ -183,7 +229,7 @@ void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const ui
   });
 }
 #else
-#error "LBM_PART must be 0..7"
+#error "LBM_PART must be 0..8"
 #endif
 
 }  // namespace lbm

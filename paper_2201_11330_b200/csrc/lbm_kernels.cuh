@@ -9,6 +9,7 @@
 #include <type_traits>
 #include <cstdint>
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 
 namespace lbm {
 
@@ -777,13 +778,10 @@ __device__ __forceinline__ void push_one(const Params& p, int z, int ixy /* x + 
 
 // SYM (D:R25): the box has SYMMETRY faces (always BC_GEO).  A separate instantiation: the mirror fix-up costs the
 // link-mask kernels registers even where it never runs (sphere case 15.4 -> 15.0 GLUPS when it was compiled in).
-template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB = false, bool SYM = false>
-__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  int z = blockIdx.z;
-  if constexpr (SLAB) z += p.z_lo;
-  if (x >= p.nx || y >= p.ny) return;
+// One cell of the A/B step.  COHERENT: the loads go through L2 (ld.global.cg) instead of the non-coherent path — needed
+// by the persistent kernel below, whose source buffer was written by other SMs earlier in the SAME launch.
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB, bool SYM, bool COHERENT>
+__device__ __forceinline__ void ab_cell(const ST* src, ST* dst, const Params& p, int x, int y, int z) {
   const Neigh nb(p, x, y, z);
   const CellFlags<BC> c(p, x, y, z, nb.cell);
   auto link = [&](auto A) { return plane<decltype(A)::value>(src, p.ds) + nb.template at<Q, decltype(A)::value, -1>(); };
@@ -797,7 +795,10 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   };
   const bool at_mirror = SYM ? touches_sym<BC>(p, c) : false;
   auto pull = [&](auto& f) {
-    auto load = [](auto, const ST* q) { return LBM_LD_STREAM(q); };
+    auto load = [](auto, const ST* q) {
+      if constexpr (COHERENT) return __ldcg(q);
+      else return LBM_LD_STREAM(q);
+    };
     if constexpr (SYM) return gather<Q, BC>(f, c, link, wall, load, mirror, at_mirror);
     else return gather<Q, BC>(f, c, link, wall, load);
   };
@@ -821,6 +822,37 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
       LBM_ST_STREAM(plane<a>(dst, p.ds) + nb.ic, f[a]);  // ST = double in this branch
       if constexpr (SLAB) push_one<Q, a, ST>(p, z, nb.ox[1] + nb.oy[1], f[a]);
     });
+  }
+}
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SLAB = false, bool SYM = false>
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) stream_collide_ab(const ST* __restrict__ src, ST* __restrict__ dst, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  int z = blockIdx.z;
+  if constexpr (SLAB) z += p.z_lo;
+  if (x >= p.nx || y >= p.ny) return;
+  ab_cell<Q, EQ, BC, FORCE, ST, SLAB, SYM, false>(src, dst, p, x, y, z);
+}
+
+// Small grids (every block of the grid resident at once: <= 148 SMs x blocks/SM x 256 cells, e.g. 32^3 or the paper's
+// 512 x 128 channel) are bound by the launch rate of one kernel per step (4-5 us), and CUDA-graph replay is slower
+// still.  This persistent kernel takes all the steps of one lbm_step call in ONE cooperative
+// launch: every thread keeps its cell, the two buffers swap roles each step, a grid-wide barrier separates the steps
+// (stores fenced before it, loads through L2 after it), and the populations never leave the L2.  Compiled for two
+// blocks per SM (128 registers: no spills): a grid that fits at all is far from filling the device.
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SYM = false>
+__global__ void __launch_bounds__(256, 2) stream_collide_ab_persistent(ST* b0, ST* b1, int nsteps, const __grid_constant__ Params p) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  const bool inside = x < p.nx && y < p.ny;
+  for (int s = 0; s < nsteps; ++s) {
+    const ST* src = (s & 1) ? b1 : b0;
+    ST* dst = (s & 1) ? b0 : b1;
+    if (inside) ab_cell<Q, EQ, BC, FORCE, ST, false, SYM, true>(src, dst, p, x, y, z);
+    if (s + 1 < nsteps) grid.sync();
   }
 }
 
