@@ -49,7 +49,7 @@ enum {
   LBM_D3Q27 = 27,           /* domain (use nz = 1 for one)                                      */
   LBM_EQ_STANDARD = 0,      /* Eq. 2, weakly compressible (default)                            */
   LBM_EQ_INCOMP = 1 << 8,   /* Eq. 5, incompressible model with rho0 = 1               */
-  LBM_SCHEME_AUTO = 0,      /* = LBM_SCHEME_AB                                                 */
+  LBM_SCHEME_AUTO = 0,      /* LBM_SCHEME_AB, except LBM_SCHEME_AA where one buffer fits the L2 and two do not */
   LBM_SCHEME_AB = 1 << 12,  /* two buffers, pull ("stream on read")                            */
   LBM_SCHEME_AA = 2 << 12,  /* one buffer, in-place AA pattern                                 */
   LBM_STORE_F64 = 0,        /* populations stored as fp64 (default)                            */
