@@ -453,8 +453,8 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
     p.z_hi = nz - 1;
     // the z faces of the box act only on the slab that owns them; elsewhere the cut is an ordinary interior plane
     const bool owns_lo = z0 == 0, owns_hi = z0 + h->nz_local == nz_global;
-    if (!owns_lo) { p.wall[4] = 0; p.open[4] = 0; p.kind[4] = LBM_FACE_PERIODIC; }
-    if (!owns_hi) { p.wall[5] = 0; p.open[5] = 0; p.kind[5] = LBM_FACE_PERIODIC; }
+    if (!owns_lo) { p.wall[4] = 0; p.open[4] = 0; p.sym[4] = 0; p.kind[4] = LBM_FACE_PERIODIC; }
+    if (!owns_hi) { p.wall[5] = 0; p.open[5] = 0; p.sym[5] = 0; p.kind[5] = LBM_FACE_PERIODIC; }
     p.any_open = 0;
     for (int k = 0; k < 6; ++k) p.any_open |= p.open[k];
     p.zg_off = z0 - 1;
