@@ -33,7 +33,6 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 SMs
-constexpr long long kPersistentMaxBlocks = 148 * 16;  // upper bound of what can be co-resident; the launcher checks exactly
 
 }  // namespace
 
@@ -74,6 +73,7 @@ struct lbm_handle_s {
   uint32_t* peer_hi_flag;
   void* ipc_opened[6];
   int n_ipc_opened;
+  int l2_bytes;       // L2 cache size of the device (0 = unknown)
   int persistent;     // lbm_step may take all steps of a call in one cooperative launch (small grids; lbm_set_persistent)
   int bx, by;         // block shape of the fused kernel (lbm_set_block), 0,0 = default_block()
   int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
@@ -468,6 +468,11 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   while (bx < nx && bx < 256) bx *= 2;
   h->bx = h->by = 0;  // default_block() at launch time (it depends on the geometry)
   h->persistent = 1;
+  {
+    int dev = 0, l2 = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) == cudaSuccess) h->l2_bytes = l2;
+    cudaGetLastError();
+  }
   h->fbx = bx;
 
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
@@ -770,10 +775,10 @@ int lbm_step(lbm_handle h, int nsteps) {
   if (nsteps < 0) return fail(LBM_EINVAL, "lbm_step: nsteps must be >= 0");
   if (nsteps == 0) return LBM_OK;
   Ctx c = make_ctx(h);
-  // Small grids: all steps of this call in ONE cooperative launch (stream_collide_ab_persistent) when the whole grid
-  // is resident at once; otherwise, and for slabs / in-place AA, one launch per step.
-  if (h->persistent && h->scheme == LBM_SCHEME_AB && !h->slab && nsteps >= 2 &&
-      (long long)c.grid.x * c.grid.y * c.grid.z <= kPersistentMaxBlocks) {
+  // Small grids (both buffers fit the L2): all steps of this call in ONE cooperative launch of the persistent kernel;
+  // otherwise, and for slabs / in-place AA, one launch per step.
+  if (h->persistent && h->scheme == LBM_SCHEME_AB && !h->slab && nsteps >= 2 && h->l2_bytes > 0 &&
+      2.0 * (double)h->buf_bytes() <= 0.8 * h->l2_bytes) {
     bool ok = false;
     LBM_Q_CALL_RET(h, ok, launch_step_ab_persistent, c, h->buf[h->cur], h->buf[h->cur ^ 1], nsteps);
     if (ok) {

@@ -96,11 +96,22 @@ bool launch_persistent(K kernel, const Ctx& c, void* b0, void* b1, int nsteps) {
     cudaGetLastError();
     return false;
   }
-  const long long blocks = (long long)c.grid.x * c.grid.y * c.grid.z;
-  if (blocks > (long long)per_sm * sms) return false;
+  // as many layers of blocks along z (then along y) as can be resident at once; the kernel strides over the rest
+  const long long capacity = (long long)per_sm * sms;
+  dim3 grid = c.grid;
+  if ((long long)grid.x > capacity) return false;
+  if ((long long)grid.x * grid.y * grid.z > capacity) {
+    const long long zl = capacity / ((long long)grid.x * grid.y);
+    if (zl >= 1) {
+      grid.z = (unsigned)zl;
+    } else {
+      grid.z = 1;
+      grid.y = (unsigned)(capacity / grid.x);
+    }
+  }
   Params p = c.p;
   void* args[] = {&b0, &b1, &nsteps, &p};
-  if (cudaLaunchCooperativeKernel((const void*)kernel, c.grid, c.block, args, 0, c.stream) != cudaSuccess) {
+  if (cudaLaunchCooperativeKernel((const void*)kernel, grid, c.block, args, 0, c.stream) != cudaSuccess) {
     cudaGetLastError();
     return false;
   }

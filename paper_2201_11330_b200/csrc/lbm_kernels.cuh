@@ -835,9 +835,8 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   ab_cell<Q, EQ, BC, FORCE, ST, SLAB, SYM, false>(src, dst, p, x, y, z);
 }
 
-// Small grids (every block of the grid resident at once: <= 148 SMs x blocks/SM x 256 cells, e.g. 32^3 or the paper's
-// 512 x 128 channel) are bound by the launch rate of one kernel per step (4-5 us), and CUDA-graph replay is slower
-// still.  This persistent kernel takes all the steps of one lbm_step call in ONE cooperative
+// Small grids (both buffers resident in the L2: 32^3, 64^3, the paper's 512 x 128 channel) are bound by the launch
+// rate of one kernel per step (4-5 us), and CUDA-graph replay is slower still.  This persistent kernel takes all the steps of one lbm_step call in ONE cooperative
 // launch: every thread keeps its cell, the two buffers swap roles each step, a grid-wide barrier separates the steps
 // (stores fenced before it, loads through L2 after it), and the populations never leave the L2.  Compiled for two
 // blocks per SM (128 registers: no spills): a grid that fits at all is far from filling the device.
@@ -845,13 +844,16 @@ template <int Q, int EQ, int BC, bool FORCE, typename ST, bool SYM = false>
 __global__ void __launch_bounds__(256, 2) stream_collide_ab_persistent(ST* b0, ST* b1, int nsteps, const __grid_constant__ Params p) {
   cooperative_groups::grid_group grid = cooperative_groups::this_grid();
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
-  const bool inside = x < p.nx && y < p.ny;
+  const int y0 = blockIdx.y * blockDim.y + threadIdx.y, ystep = gridDim.y * blockDim.y;
   for (int s = 0; s < nsteps; ++s) {
     const ST* src = (s & 1) ? b1 : b0;
     ST* dst = (s & 1) ? b0 : b1;
-    if (inside) ab_cell<Q, EQ, BC, FORCE, ST, false, SYM, true>(src, dst, p, x, y, z);
+    if (x < p.nx) {
+      // the launcher gives the grid as many layers of blocks along z (then y) as fit the device at once; a block takes
+      // every gridDim.z-th plane and every gridDim.y-th group of rows
+      for (int z = blockIdx.z; z < p.nz; z += gridDim.z)
+        for (int y = y0; y < p.ny; y += ystep) ab_cell<Q, EQ, BC, FORCE, ST, false, SYM, true>(src, dst, p, x, y, z);
+    }
     if (s + 1 < nsteps) grid.sync();
   }
 }
