@@ -789,6 +789,18 @@ int lbm_step(lbm_handle h, int nsteps) {
       return check_launch("lbm_step");
     }
   }
+  if (h->persistent && h->scheme == LBM_SCHEME_AA && nsteps >= 2 && h->l2_bytes > 0 &&
+      (double)h->buf_bytes() <= 0.8 * h->l2_bytes) {
+    bool ok = false;
+    LBM_Q_CALL_RET(h, ok, launch_step_aa_persistent, c, h->buf[0], nsteps, h->phase);
+    if (ok) {
+      h->phase ^= (nsteps & 1);
+      h->time += nsteps;
+      ++h->launches;
+      h->stepped = true;
+      return check_launch("lbm_step");
+    }
+  }
   for (int s = 0; s < nsteps; ++s) {
     if (h->slab) {
       int rc = launch_step_slab(h, c);

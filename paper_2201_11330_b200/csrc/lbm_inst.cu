@@ -3,11 +3,12 @@
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
 //            5 A/B step of a z-slab (fused halo push)   6 A/B step with SYMMETRY faces (link mask + mirror links)
 //            7 A/B step of a z-slab with SYMMETRY faces   8 persistent A/B kernel (all steps of a call in one launch)
+//            9 persistent in-place AA kernel
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..8"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..9"
 #endif
 
 namespace lbm {
@@ -58,6 +59,43 @@ void dispatch_mode(int mode, F&& f) {
 
 constexpr int Q_ = LBM_Q;
 
+#if LBM_PART == 8 || LBM_PART == 9
+namespace {
+// cooperative launch of one instantiation with as many layers of blocks along z (then along y) as can be resident at
+// once (the kernel strides over the rest); false = not even one layer fits, or no cooperative launch: use the per-step kernels
+template <typename K>
+bool launch_cooperative(K kernel, const Ctx& c, void** args, bool allow_stride) {
+  int per_sm = 0, dev = 0, sms = 0, coop = 0;
+  const int threads = c.block.x * c.block.y * c.block.z;
+  if (cudaGetDevice(&dev) != cudaSuccess) return false;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  const long long capacity = (long long)per_sm * sms;
+  dim3 grid = c.grid;
+  if ((long long)grid.x > capacity) return false;
+  if ((long long)grid.x * grid.y * grid.z > capacity) {
+    if (!allow_stride) return false;
+    const long long zl = capacity / ((long long)grid.x * grid.y);
+    if (zl >= 1) {
+      grid.z = (unsigned)zl;
+    } else {
+      grid.z = 1;
+      grid.y = (unsigned)(capacity / grid.x);
+    }
+  }
+  if (cudaLaunchCooperativeKernel((const void*)kernel, grid, c.block, args, 0, c.stream) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return true;
+}
+}  // namespace
+#endif
+
 #if LBM_PART == 0
 template <>
 void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
@@ -84,38 +122,14 @@ void launch_step_ab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
 }
 #elif LBM_PART == 8
 namespace {
-// cooperative launch of one instantiation if the whole grid can be resident at once; false = use the per-step kernels
 template <typename K>
 bool launch_persistent(K kernel, const Ctx& c, void* b0, void* b1, int nsteps) {
-  int per_sm = 0, dev = 0, sms = 0, coop = 0;
-  const int threads = c.block.x * c.block.y * c.block.z;
-  if (cudaGetDevice(&dev) != cudaSuccess) return false;
-  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess) {
-    cudaGetLastError();
-    return false;
-  }
-  // as many layers of blocks along z (then along y) as can be resident at once; the kernel strides over the rest
-  const long long capacity = (long long)per_sm * sms;
-  dim3 grid = c.grid;
-  if ((long long)grid.x > capacity) return false;
-  if ((long long)grid.x * grid.y * grid.z > capacity) {
-    const long long zl = capacity / ((long long)grid.x * grid.y);
-    if (zl >= 1) {
-      grid.z = (unsigned)zl;
-    } else {
-      grid.z = 1;
-      grid.y = (unsigned)(capacity / grid.x);
-    }
-  }
   Params p = c.p;
   void* args[] = {&b0, &b1, &nsteps, &p};
-  if (cudaLaunchCooperativeKernel((const void*)kernel, grid, c.block, args, 0, c.stream) != cudaSuccess) {
-    cudaGetLastError();
-    return false;
-  }
-  return true;
+  // With inlet / outlet on the x faces single lanes run long ("One lane per row"): a grid that has to
+  // stride then waits for them at every barrier (512^2 D2Q9 channel-cylinder x0.95, 128x32x32 sphere case x0.81), so
+  // such grids must be resident in one pass; without open faces striding pays (64^3 cavity x1.14, 48^3 D3Q27 channel x1.23).
+  return launch_cooperative(kernel, c, args, !(c.p.open[0] || c.p.open[1]));
 }
 }  // namespace
 
@@ -136,6 +150,19 @@ bool launch_step_ab_persistent<Q_>(const Ctx& c, void* b0, void* b1, int nsteps)
   dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
     using ST = decltype(st);
     ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST, false>, c, b0, b1, nsteps);
+  });
+  return ok;
+}
+#elif LBM_PART == 9
+template <>
+bool launch_step_aa_persistent<Q_>(const Ctx& c, void* buf, int nsteps, int phase) {
+  bool ok = false;
+  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
+    using ST = decltype(st);
+    Params p = c.p;
+    void* args[] = {&buf, &nsteps, &phase, &p};
+    // in place: only grids resident in one pass (striding is neutral at best: 1200 x 1100 D2Q9 x0.92, 80^3 x0.99)
+    ok = launch_cooperative(stream_collide_aa_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>, c, args, false);
   });
   return ok;
 }
@@ -240,7 +267,7 @@ void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const ui
   });
 }
 #else
-#error "LBM_PART must be 0..8"
+#error "LBM_PART must be 0..9"
 #endif
 
 }  // namespace lbm

@@ -864,19 +864,26 @@ __global__ void __launch_bounds__(256, 2) stream_collide_ab_persistent(ST* b0, S
 // after which the buffer is in natural layout again.  Each thread reads and writes exactly its
 // own set of Q slots (the odd phase writes f*_a where it read f_abar), so there is no
 // inter-thread hazard in either phase.
-template <int Q, int EQ, int BC, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_even(ST* buf, const __grid_constant__ Params p) {
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
-  if (x >= p.nx || y >= p.ny) return;
+// COHERENT: loads through L2 (ld.global.cg) for the persistent kernel, as in ab_cell.
+template <bool COHERENT, typename ST, int Q, int A>
+__device__ __forceinline__ double ld_pop_aa(const ST* q) {
+  if constexpr (COHERENT) {
+    if constexpr (sizeof(ST) == 8) return __ldcg(q);
+    else return (double)__ldcg(q) + Dir<Q, A>::t;
+  } else {
+    return ld_pop_rw<ST, Q, A>(q, 0);
+  }
+}
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool COHERENT>
+__device__ __forceinline__ void aa_even_cell(ST* buf, const Params& p, int x, int y, int z) {
   const int cell = x + p.nx * (y + p.ny * z);
   const long long ic = (x + y * p.rs) + z * p.zs;  // storage offset (Neigh::ic)
   const CellFlags<BC> c(p, x, y, z, cell);
   double f[Q];
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
-    f[a] = ld_pop_rw<ST, Q, a>(plane<a>(buf, p.ds), ic);
+    f[a] = ld_pop_aa<COHERENT, ST, Q, a>(plane<a>(buf, p.ds) + ic);
   });
   if (!c.template active<Q>()) return;  // after the loads: they do not wait for the link mask (see gather)
   nodal_replicate<Q, BC>(f, p, c);
@@ -887,19 +894,15 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   });
 }
 
-template <int Q, int EQ, int BC, bool FORCE, typename ST>
-__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_odd(ST* buf, const __grid_constant__ Params p) {
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
-  if (x >= p.nx || y >= p.ny) return;
+template <int Q, int EQ, int BC, bool FORCE, typename ST, bool COHERENT>
+__device__ __forceinline__ void aa_odd_cell(ST* buf, const Params& p, int x, int y, int z) {
   const Neigh nb(p, x, y, z);
   const CellFlags<BC> c(p, x, y, z, nb.cell);
   double f[Q];
   // f_a(x) comes from the slot that f*_abar(x) goes to (link x <-> x - e_a traversed both ways)
   auto link = [&](auto A) { return (const ST*)plane<Dir<Q, decltype(A)::value>::opp>(buf, p.ds) + nb.template at<Q, decltype(A)::value, -1>(); };
   auto wall = [&](auto A) { return (const ST*)plane<decltype(A)::value>(buf, p.ds) + nb.ic; };
-  if (!gather<Q, BC>(f, c, link, wall, [](auto A, const ST* q) { return ld_pop_rw<ST, Q, decltype(A)::value>(q, 0); })) return;
+  if (!gather<Q, BC>(f, c, link, wall, [](auto A, const ST* q) { return ld_pop_aa<COHERENT, ST, Q, decltype(A)::value>(q); })) return;
   nodal_replicate<Q, BC>(f, p, c);
   collide<Q, EQ, BC, FORCE>(f, p, c, nb.cell, z);
   static_for<0, Q>([&](auto A) {
@@ -911,6 +914,43 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
     }
     st_pop<ST, Q, a>(q, 0, f[a]);
   });
+}
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_even(ST* buf, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= p.nx || y >= p.ny) return;
+  aa_even_cell<Q, EQ, BC, FORCE, ST, false>(buf, p, x, y, z);
+}
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collide_aa_odd(ST* buf, const __grid_constant__ Params p) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= p.nx || y >= p.ny) return;
+  aa_odd_cell<Q, EQ, BC, FORCE, ST, false>(buf, p, x, y, z);
+}
+
+// The in-place scheme in one cooperative launch per lbm_step call, for grids whose ONE buffer fits the L2 (where
+// LBM_SCHEME_AUTO picks this scheme): phases alternate from `phase` on, a grid-wide barrier after each step.
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256, 2) stream_collide_aa_persistent(ST* buf, int nsteps, int phase, const __grid_constant__ Params p) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y0 = blockIdx.y * blockDim.y + threadIdx.y, ystep = gridDim.y * blockDim.y;
+  for (int s = 0; s < nsteps; ++s, phase ^= 1) {
+    if (x < p.nx) {
+      for (int z = blockIdx.z; z < p.nz; z += gridDim.z)
+        for (int y = y0; y < p.ny; y += ystep) {
+          if (phase == 0) aa_even_cell<Q, EQ, BC, FORCE, ST, true>(buf, p, x, y, z);
+          else aa_odd_cell<Q, EQ, BC, FORCE, ST, true>(buf, p, x, y, z);
+        }
+    }
+    if (s + 1 < nsteps) grid.sync();
+  }
 }
 
 // ---------------------------------------------------------------------------------------

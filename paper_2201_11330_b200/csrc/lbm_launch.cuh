@@ -27,6 +27,7 @@ template <int Q> void launch_step_ab_sym(const Ctx& c, const void* src, void* ds
 template <int Q> void launch_step_ab_slab_sym(const Ctx& c, const void* src, void* dst);
 // all nsteps in one cooperative launch (b0 = current buffer); false = the grid does not fit the device at once
 template <int Q> bool launch_step_ab_persistent(const Ctx& c, void* b0, void* b1, int nsteps);
+template <int Q> bool launch_step_aa_persistent(const Ctx& c, void* buf, int nsteps, int phase);
 template <int Q> void launch_step_aa_even(const Ctx& c, void* buf);
 template <int Q> void launch_step_aa_odd(const Ctx& c, void* buf);
 template <int Q> void launch_export(const Ctx& c, int mode, const void* buf, double* out);
