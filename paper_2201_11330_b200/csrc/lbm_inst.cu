@@ -135,34 +135,36 @@ bool launch_persistent(K kernel, const Ctx& c, void* b0, void* b1, int nsteps) {
 
 template <>
 bool launch_step_ab_persistent<Q_>(const Ctx& c, void* b0, void* b1, int nsteps) {
+  // fp64 storage only: grids this small have no use for the fp32-storage variant, and it would double the build
+  if (c.f32) return false;
   bool ok = false;
-  if (c.p.any_sym) {
-    dispatch_eq(c, [&](auto eq) {
-      dispatch_force(c, [&](auto force) {
-        dispatch_storage(c, [&](auto st) {
-          using ST = decltype(st);
-          ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, ST, true>, c, b0, b1, nsteps);
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_force(c, [&](auto force) {
+      if (c.p.any_sym) {
+        ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, double, true>, c, b0, b1, nsteps);
+      } else {
+        dispatch_bc(c, [&](auto bc) {
+          ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, double, false>, c, b0, b1, nsteps);
         });
-      });
+      }
     });
-    return ok;
-  }
-  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
-    using ST = decltype(st);
-    ok = launch_persistent(stream_collide_ab_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST, false>, c, b0, b1, nsteps);
   });
   return ok;
 }
 #elif LBM_PART == 9
 template <>
 bool launch_step_aa_persistent<Q_>(const Ctx& c, void* buf, int nsteps, int phase) {
+  if (c.f32) return false;  // fp64 storage only, as above
   bool ok = false;
-  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
-    using ST = decltype(st);
-    Params p = c.p;
-    void* args[] = {&buf, &nsteps, &phase, &p};
-    // in place: only grids resident in one pass (striding is neutral at best: 1200 x 1100 D2Q9 x0.92, 80^3 x0.99)
-    ok = launch_cooperative(stream_collide_aa_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>, c, args, false);
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_bc(c, [&](auto bc) {
+      dispatch_force(c, [&](auto force) {
+        Params p = c.p;
+        void* args[] = {&buf, &nsteps, &phase, &p};
+        // in place: only grids resident in one pass (striding is neutral at best: 1200 x 1100 D2Q9 x0.92, 80^3 x0.99)
+        ok = launch_cooperative(stream_collide_aa_persistent<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, double>, c, args, false);
+      });
+    });
   });
   return ok;
 }
