@@ -526,3 +526,33 @@ def test_large_box_equals_its_periodic_tile(lbm, scheme):
         assert torch.equal(u_big[(slice(None),) + sl], u_small)
     assert d_big[7] == 0 and d_big[5] == d_small[5] and d_big[6] == d_small[6]
     assert abs(d_big[0] - k**3 * d_small[0]) <= 1e-12 * d_big[0]
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
+    """lbm_step(n) on a small grid runs in ONE cooperative launch of the persistent kernel (all n steps, a grid-wide
+    barrier between them); with lbm_set_persistent(0) it is n launches.  Same cell code: identical bits — periodic,
+    cavity with lid, inlet / outlet with a solid mask under the nodal model, odd and even step counts."""
+    sch = {"ab": lbm.LBM_SCHEME_AB, "aa": lbm.LBM_SCHEME_AA}[scheme]
+    dims = (48, 20, 12)
+    N = dims[0] * dims[1] * dims[2]
+    rng = np.random.default_rng(9)
+    f0 = torch.from_numpy(np.full((19, 1), 1.0 / 19) * (1.0 + 0.1 * rng.uniform(-1, 1, (19, N)))).cuda().reshape(-1)
+    geo = torch.from_numpy((rng.uniform(size=N) < 0.03).astype(np.uint8)).cuda()
+    lid = dict(face_kind=[1, 1, 1, 1, 1, 2], face_u=[[0, 0, 0]] * 5 + [[0.1, 0, 0]])
+    openx = dict(face_kind=[2, 3, 1, 1, 0, 0], face_u=[[0.03, 0, 0]] + [[0, 0, 0]] * 5, force=(1e-5, 0, 0))
+    for case, use_geo in ((dict(), False), (lid, False), (openx, True)):
+        out = []
+        for on in (1, 0):
+            s = lbm.Solver(*dims, 19, 0.7, scheme=sch, **case)
+            s.set_persistent(on)
+            if use_geo:
+                s.set_geometry(geo, lbm.LBM_WALL_NODAL)
+            s.set_populations(f0)
+            l0 = s.launches
+            s.step(7)
+            s.step(10)
+            out.append((s.get_populations().clone(), s.launches - l0))
+            s.close()
+        assert torch.equal(out[0][0], out[1][0])
+        assert out[1][1] - out[0][1] == 15, out  # 17 step launches became 2
