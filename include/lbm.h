@@ -208,7 +208,7 @@ int lbm_set_block(lbm_handle h, int bx, int by);
  * Per step the fused kernel also stores the 5 (D3Q19) / 9 (D3Q27) / 0 (D2Q9) populations per cell of
  * its first and last plane that cross the cut directly into the neighbouring slab's halo plane (peer
  * memory: NVLink between GPUs); there is no separate exchange pass and no host staging.  Ordering between
- * slabs is on the device: step t of a slab starts when both neighbours have finished step t-1 (a 64-bit
+ * slabs is on the device: step t of a slab starts when both neighbours have finished step t-1 (a 32-bit step
  * counter per side in the slab's own memory, written by the neighbour, waited for by the stream).
  * Geometry on a slab: lbm_set_geometry takes the mask with TWO halo planes per side — nx*ny*(nz_local+4) bytes, plane
  * index 2 + (z_global - z0), periodic wrap included, ignored beyond a non-periodic z face — because under
