@@ -719,8 +719,33 @@ __device__ __forceinline__ void nodal_replicate(T (&f)[Q], const Params& p, cons
 // a fraction of a percent of the nodes are solid).  Returns false for an inactive node.
 struct NoMirror {};  // gather() without SYMMETRY faces (the in-place kernels: lbm_create refuses the combination)
 
-template <int Q, int BC, typename T, typename LinkF, typename WallF, typename LoadF, typename MirrorF = NoMirror>
-__device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&& link, WallF&& wall, LoadF&& load, MirrorF&& mirror = NoMirror{}, bool at_mirror = false) {
+template <int Q, int BC, bool PREFETCH_FACES = false, typename T, typename LinkF, typename WallF, typename LoadF, typename MirrorF = NoMirror>
+__device__ __forceinline__ bool gather(T (&f)[Q], const CellFlags<BC>& c, LinkF&& link, WallF&& wall, LoadF&& load, MirrorF&& mirror = NoMirror{}, bool at_mirror = false,
+                                       const Params* pp = nullptr /* PREFETCH_FACES only */) {
+  if constexpr (BC == BC_GEO && PREFETCH_FACES) {
+    // Cells in a first / last plane of a non-periodic face know their box-face wall links from the coordinates: they
+    // prefetch those slots now (no destination register, no hazard), so that the re-read below — which has to wait for
+    // the link mask — finds them in L1 instead of making a second trip to DRAM.  With an inlet / outlet on the x faces
+    // that cell is ONE lane of a warp the rest of its block waits for (ncu, sphere case: 37 % of the divergent-lane
+    // stall samples sat on that second trip).
+    if (c.lo[0] | c.hi[0] | c.lo[1] | c.hi[1] | c.lo[2] | c.hi[2]) {
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        if constexpr (Dir<Q, a>::s > 0) {
+          // (links through SYMMETRY faces are no wall links: their value comes from the mirror image, below)
+          using D = Dir<Q, a>;
+          bool w = false;
+          if constexpr (D::ex == 1) w = w | (c.lo[0] & !pp->sym[0]);
+          if constexpr (D::ex == -1) w = w | (c.hi[0] & !pp->sym[1]);
+          if constexpr (D::ey == 1) w = w | (c.lo[1] & !pp->sym[2]);
+          if constexpr (D::ey == -1) w = w | (c.hi[1] & !pp->sym[3]);
+          if constexpr (D::ez == 1) w = w | (c.lo[2] & !pp->sym[4]);
+          if constexpr (D::ez == -1) w = w | (c.hi[2] & !pp->sym[5]);
+          if (w) asm volatile("prefetch.global.L1 [%0];" ::"l"(wall(A)));
+        }
+      });
+    }
+  }
   static_for<0, Q>([&](auto A) {
     constexpr int a = decltype(A)::value;
     auto q = link(A);
@@ -799,8 +824,9 @@ __device__ __forceinline__ void ab_cell(const ST* src, ST* dst, const Params& p,
       if constexpr (COHERENT) return __ldcg(q);
       else return LBM_LD_STREAM(q);
     };
+    // (no prefetch in the SYM instantiation: measured slower there, 609 -> 625 us on the sphere case)
     if constexpr (SYM) return gather<Q, BC>(f, c, link, wall, load, mirror, at_mirror);
-    else return gather<Q, BC>(f, c, link, wall, load);
+    else return gather<Q, BC, true>(f, c, link, wall, load, NoMirror{}, false, &p);
   };
   if constexpr (sizeof(ST) == 4) {
     float g[Q];  // packed: stays fp32 in registers until used (collide_shifted)
