@@ -21,6 +21,9 @@
 //   moving wall (Ladd) ........ pinned: planar Couette exact linear profile, cavity mass
 //   Guo forcing ............... pinned: momentum gain F*N per step, Poiseuille
 //   indexing .................. pinned: independent brute-force gather on 4^3 (long double)
+//   moments + diagnostics[8] .. pinned: fields by closed forms (Couette, Poiseuille); all eight diagnostics against a
+//                               direct NumPy evaluation of their definition (random f, solid mask, both wall models,
+//                               F/2 shift, Eq. 5 weighting), NaN / Inf cells counted and left out of the sums
 //   D3Q27 ..................... pinned only through the same invariants and closed forms;
 //                               no D3Q27-specific printed value exists in the paper.
 //   D2Q9 ...................... pinned: the table is Eq. 3-4 as printed; dynamics by 2-D isotropy, brute-force

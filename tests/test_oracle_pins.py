@@ -484,3 +484,82 @@ def test_sweeps_are_the_papers_four(golden_dir):
     f1 = b.get_f().reshape(19, n, n, n)  # [alpha, z, y, x]
     for q in range(19):
         assert (f1[q] == np.roll(fb[q], shift=(e[q, 2], e[q, 1], e[q, 0]), axis=(0, 1, 2))).all()
+
+
+# ---------------------------------------------------------------------------- diagnostics (Monitor)
+def _direct_diagnostics(f, act, E, F, eq):
+    """The 8 diagnostics of include/lbm.h:161-166 evaluated from their definition on f[Q, N] (NumPy, no oracle code):
+    { sum rho, sum rho u (3), 1/2 sum rho |u|^2, max |u|, min rho, non-finite cells } over the active nodes, non-finite
+    cells excluded from the other seven; u = (sum e f + F/2) / rho (Eq. 8-9, D:R7), under Eq. 5 divided by and weighted
+    with rho0 = 1 (D:R5); 3-component magnitude (D:R13)."""
+    E = np.asarray(E, dtype=np.float64)
+    with np.errstate(invalid="ignore", divide="ignore", over="ignore"):
+        rho = f.sum(axis=0)
+        m = E.T @ f + 0.5 * np.asarray(F, dtype=np.float64)[:, None]
+        u = m / rho if eq == EQ_STANDARD else m.copy()
+        usq = (u * u).sum(axis=0)
+        ok = act.astype(bool) & np.isfinite(rho) & np.isfinite(usq)
+    bad = int((act.astype(bool) & ~ok).sum())
+    w = rho[ok] if eq == EQ_STANDARD else np.ones(int(ok.sum()))
+    import math
+    d = [math.fsum(rho[ok])] + [math.fsum(w * u[c][ok]) for c in range(3)]
+    d += [0.5 * math.fsum(w * usq[ok]), float(np.sqrt(usq[ok]).max()), float(rho[ok].min()), float(bad)]
+    return np.array(d), rho, u
+
+
+@pytest.mark.parametrize("wall_model", [0, 1])
+@pytest.mark.parametrize("Q,eq,forced", [(19, EQ_STANDARD, False), (19, EQ_STANDARD, True), (19, EQ_INCOMP, True),
+                                         (27, EQ_STANDARD, True), (27, EQ_INCOMP, False), (9, EQ_STANDARD, True)])
+def test_all_eight_diagnostics_equal_their_definition(Q, eq, forced, wall_model):
+    """Every entry of post_processing's diagnostics[8] against a direct NumPy evaluation of its definition from the
+    same populations: random non-equilibrium f, a solid mask (so inactive nodes exist and must be left out), both wall
+    models, with and without the F/2 shift.  Catches a wrong constant (the 1/2 of the energy), a 2-component magnitude
+    (P:415 as printed), rho vs rho0 weighting under Eq. 5, sums over inactive nodes."""
+    if Q == 19:
+        E = _E19
+    else:
+        E = [e for e in itertools.product((-1, 0, 1), repeat=3) if Q == 27 or e[2] == 0]
+    dims = (9, 8, 7 if Q != 9 else 2)
+    nx, ny, nz = dims
+    N = nx * ny * nz
+    F = (3e-3, -2e-3, 1e-3 if Q != 9 else 0.0) if forced else (0.0, 0.0, 0.0)
+    o = Oracle(nx, ny, nz, Q, 0.7, eq=eq, force=F, face_kind=[FACE_PERIODIC] * 4 + ([FACE_BOUNCE] * 2 if Q != 9 else [FACE_PERIODIC] * 2))
+    geo = np.zeros((nz, ny, nx), dtype=np.uint8)
+    geo[: (4 if Q != 9 else nz), 2:6, 2:7] = 1  # a block on the z- wall: under the nodal model its skin becomes wall nodes, its core stays inactive
+    o.set_geometry(geo.reshape(-1), wall_model)
+    rng = np.random.default_rng(77 + Q + eq + wall_model)
+    f0 = (1.0 / Q) * (1.0 + 0.4 * rng.uniform(-1, 1, (Q, N)))
+    o.set_f(f0)
+    f, act = o.get_f(), o.active()
+    assert 0 < act.sum() < N
+    rho_o, u_o, d_o = o.moments()
+    d, rho, u = _direct_diagnostics(f, act, E, F, eq)
+    np.testing.assert_allclose(d_o[:5], d[:5], rtol=1e-13, atol=1e-13)
+    assert d_o[5] == pytest.approx(d[5], rel=1e-14) and d_o[6] == pytest.approx(d[6], rel=1e-14) and d_o[7] == d[7] == 0
+    a = act.astype(bool)
+    assert np.abs(rho_o[a] - rho[a]).max() <= 1e-14 and np.abs(u_o[:, a] - u[:, a]).max() <= 1e-14
+    assert (rho_o[~a] == 0).all() and (u_o[:, ~a] == 0).all()
+    # the energy really carries the factor 1/2 and all three components (not only its slope, as the Taylor-Green pin)
+    assert d_o[4] == pytest.approx(0.5 * ((rho[a] if eq == EQ_STANDARD else 1.0) * (u[:, a] * u[:, a]).sum(axis=0)).sum(), rel=1e-12)
+
+
+@pytest.mark.parametrize("eq", [EQ_STANDARD, EQ_INCOMP])
+def test_nonfinite_cells_are_counted_and_left_out(eq):
+    """One NaN and one Inf planted through set_f: diagnostics[7] = 2, the other seven finite and equal to the sums over
+    the remaining cells (include/lbm.h: 'non-finite cells are excluded from the sums')."""
+    nx, ny, nz, Q = 6, 5, 4, 19
+    N = nx * ny * nz
+    o = Oracle(nx, ny, nz, Q, 0.8, eq=eq, force=(1e-3, 0, 0))
+    rng = np.random.default_rng(5)
+    f0 = (1.0 / Q) * (1.0 + 0.3 * rng.uniform(-1, 1, (Q, N)))
+    f0[3, 17] = np.nan
+    f0[11, 60] = np.inf
+    o.set_f(f0)
+    _, _, d_o = o.moments()
+    d, _, _ = _direct_diagnostics(f0, np.ones(N, dtype=np.uint8), _E19, (1e-3, 0, 0), eq)
+    assert d_o[7] == 2 and d[7] == 2
+    assert np.isfinite(d_o[:7]).all()
+    np.testing.assert_allclose(d_o[:5], d[:5], rtol=1e-13, atol=1e-13)
+    assert d_o[5] == pytest.approx(d[5], rel=1e-14) and d_o[6] == pytest.approx(d[6], rel=1e-14)
+    clean = np.delete(f0, [17, 60], axis=1)
+    assert d_o[0] == pytest.approx(clean.sum(), rel=1e-13)
