@@ -54,8 +54,11 @@ enum {
   LBM_SCHEME_AA = 2 << 12,  /* one buffer, in-place AA pattern                                 */
   LBM_STORE_F64 = 0,        /* populations stored as fp64 (default)                            */
   LBM_STORE_F32 = 1 << 16,  /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
-  LBM_LAYOUT_ROWS = 0,      /* internal buffers f[z][y][a][x]: the Q rows of a grid row adjacent (default, faster) */
-  LBM_LAYOUT_SOA = 1 << 20  /* internal buffers f[a][z][y][x] (for measurements; not on z-slab handles)  */
+  LBM_LAYOUT_ROWS = 0,      /* internal buffers f[z][y][a][x]: the Q rows of a grid row adjacent (default, faster);
+                               a grid with Q*nx*ny >= 2^31 (e.g. D2Q9 16384^2) is stored as LBM_LAYOUT_SOA instead,
+                               because in-plane offsets are 32-bit — same results bit for bit                    */
+  LBM_LAYOUT_SOA = 1 << 20  /* internal buffers f[a][z][y][x] (for measurements; also accepted on z-slab handles,
+                               all connected slabs must then use it)                                            */
 };
 
 enum { LBM_FACE_PERIODIC = 0, LBM_FACE_BOUNCE = 1, LBM_FACE_MOVING = 2, LBM_FACE_PRESSURE = 3, LBM_FACE_SYMMETRY = 4 };
@@ -100,7 +103,8 @@ typedef struct {
   void* stream;        /* cudaStream_t to run on (NULL = legacy default stream); caller-owned   */
 } lbm_bc_t;
 
-/* Create a solver on the current CUDA device.  nx >= 1, 1 <= ny, nz <= 65535; tau > 0.5; bc may be NULL
+/* Create a solver on the current CUDA device.  nx >= 1, 1 <= ny, nz <= 65535, nx*ny*nz < 2^31 (LBM_EUNSUPPORTED
+ * beyond: cell indices are 32-bit); tau > 0.5; bc may be NULL
  * (all periodic, no force, default stream).  Allocates the population buffers (Q*N doubles,
  * twice for LBM_SCHEME_AB).  Populations are undefined until lbm_init_equilibrium or
  * lbm_set_populations.  Returns NULL on failure. */
@@ -150,7 +154,10 @@ int lbm_boundary_force(lbm_handle h, double* F);
  * rho: N doubles or NULL (= 1 everywhere); u: 3N doubles or NULL (= 0).  Device pointers.
  * Under LBM_WALL_NODAL the wall nodes then satisfy Eq. 10 (D:R17). */
 int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u);
-/* Same with HOST pointers; the fields are copied to the device on the handle's stream. */
+/* Same with HOST pointers (pinned memory recommended).  The fields are copied in z-chunks on an internal copy stream
+ * and chunk k is initialised on the handle's stream while chunk k+1 is still on the bus; the handle's stream waits for
+ * every copy, so synchronising it (or any later synchronising call) also means the host arrays have been read.  On a
+ * z-slab handle only the own planes of the arrays are read. */
 int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host);
 
 /* Advance nsteps >= 0 time steps: per step and cell, pull-stream (Eq. 7) with wall links
@@ -165,7 +172,10 @@ int lbm_step(lbm_handle h, int nsteps);
  * from the sums; under LBM_EQ_INCOMP "rho u" means rho0 u (D:R5); with forcing u includes the
  * F/2 shift (D:R7).  Synchronises the stream only if diagnostics != NULL. */
 int lbm_moments(lbm_handle h, double* rho, double* u, double* diagnostics);
-/* Same with HOST output pointers for the fields (either may be NULL); always synchronises. */
+/* Same with HOST output pointers for the fields (either may be NULL); always synchronises.  The moments are
+ * computed in z-chunks and chunk k travels to the host while chunk k+1 is computed.  The fields are staged in the idle
+ * A/B buffer (in a scratch allocation for LBM_SCHEME_AA and on z-slab handles, whose idle buffer's halo planes belong
+ * to the neighbours' next step); on a z-slab handle only the own planes of the host arrays are written. */
 int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* diagnostics);
 
 /* Canonical populations f[a*N+i] (Q*N doubles, device): export / import.  Not on the hot path
@@ -214,8 +224,12 @@ int lbm_set_block(lbm_handle h, int bx, int by);
  * index 2 + (z_global - z0), periodic wrap included, ignored beyond a non-periodic z face — because under
  * LBM_WALL_NODAL the wall-node status of a halo node depends on the plane beyond it (D:R16).  lbm_boundary_force
  * returns the part of Eq. 13 carried by the fluid nodes of the own planes: sum it over the slabs.
- * Restrictions: LBM_SCHEME_AB only; every slab must be advanced by the same number of steps;
- * lbm_init_equilibrium / lbm_set_populations / lbm_set_geometry need all connected slabs idle. */
+ * Restrictions: LBM_SCHEME_AB only; every slab must be advanced by the same number of steps; connected slabs of one
+ * process need a stream each (lbm_slab_connect returns LBM_EINVAL otherwise: on a shared stream the second step of one
+ * slab would wait for a step of the other that is queued behind it); lbm_init_equilibrium(_host) /
+ * lbm_set_populations / lbm_set_geometry need all connected slabs idle (they rewrite halo planes the neighbours
+ * store into); lbm_moments(_host) / lbm_get_populations may be called between unsynchronised steps (they wait for
+ * the neighbours' last step on the device and touch no memory a neighbour writes).  SYMMETRY faces are supported. */
 
 /* What a neighbour needs to know about a slab.  Plain data: pass it to another process as bytes. */
 typedef struct {
@@ -225,6 +239,11 @@ typedef struct {
   int32_t nz_local;
   int32_t device;         /* CUDA device ordinal of the owner                                           */
   int64_t pid;            /* owner process                                                              */
+  int32_t Q;              /* lattice, bytes per stored population (8 / 4) and internal layout (1 = LBM_LAYOUT_SOA):  */
+  int32_t elem_bytes;     /*   lbm_slab_connect refuses a neighbour that differs in any of them (LBM_EINVAL)    */
+  int32_t layout_soa;
+  int32_t reserved;
+  uint64_t stream;        /* the owner's cudaStream_t (compared only within one process)                */
   uint8_t ipc_buf[2][64]; /* cudaIpcMemHandle_t of buf[0], buf[1]                                        */
   uint8_t ipc_flags[64];  /* cudaIpcMemHandle_t of flags                                                 */
 } lbm_slab_peer_t;

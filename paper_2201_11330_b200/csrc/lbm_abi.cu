@@ -33,6 +33,8 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 SMs
+constexpr int kMaxChunks = 16;          // z-chunks of the host entry points (copy of chunk k+1 overlaps the kernel of chunk k)
+constexpr size_t kChunkBytes = 64u << 20;  // ... each at least this many bytes of rho, u (smaller grids: one chunk)
 
 }  // namespace
 
@@ -59,6 +61,9 @@ struct lbm_handle_s {
   double* diag_pinned;  // 8, host
   void* scratch;
   size_t scratch_bytes;
+  cudaStream_t copy_stream;          // host entry points: the copies run here, the kernels on `stream` (created on first use)
+  cudaEvent_t chunk_ev[kMaxChunks];  // chunk k has landed (init) / has been computed (moments)
+  cudaEvent_t fence_ev;              // orders the two streams at the start and at the end of a host call
   // z-slab of a decomposed box (D:R21)
   bool slab;
   int z0, nz_global, nz_local;
@@ -236,39 +241,56 @@ int ensure_scratch(lbm_handle_s* h, size_t bytes) {
   return LBM_OK;
 }
 
-// A canonical fp64 Q*N staging area that is free while no step is in flight: the idle A/B buffer
-// when populations are stored as fp64, else the lazily allocated scratch.
-int canonical_staging(lbm_handle_s* h, double** out) {
-  if (h->scheme == LBM_SCHEME_AB && !h->f32) {
-    *out = (double*)h->buf[h->cur ^ 1];
-    return LBM_OK;
-  }
-  int rc = ensure_scratch(h, (size_t)h->N * h->Q * sizeof(double));
-  if (rc) return rc;
-  *out = (double*)h->scratch;
-  return LBM_OK;
-}
-
 int check_launch(const char* what) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(e, what);
   return LBM_OK;
 }
 
-int do_init(lbm_handle_s* h, const double* rho, const double* u) {
-  if (h->slab) h->cur = 0;  // connected slabs must agree on which buffer is current
-  double* nat = nullptr;
-  int rc = canonical_staging(h, &nat);
-  if (rc) return rc;
-  const Ctx c = make_ctx(h);
-  LBM_Q_CALL(h, launch_init, c, rho, u, nat);
-  ++h->launches;
-  if (h->scheme != LBM_SCHEME_AB) h->cur = 0;
-  do_import(h, nat, h->cur);
+// rows r = y + ny*z of the planes this handle updates, and the blocks of a row-wise sweep over `nrows` of them
+int rows_begin(const lbm_handle_s* h) { return h->ny * h->p.z_lo; }
+int rows_end(const lbm_handle_s* h) { return h->ny * h->p.z_hi; }
+int grid_for_rows(const lbm_handle_s* h, long long nrows) {
+  const long long by = 256 / h->fbx, b = (nrows + by - 1) / by;
+  return (int)(b < 1 ? 1 : b < kReduceBlocks ? b : kReduceBlocks);
+}
+
+// storage buffer and mode an initialisation writes (always an even phase); connected slabs must agree on the buffer
+int init_target(lbm_handle_s* h) {
+  if (h->slab || h->scheme != LBM_SCHEME_AB) h->cur = 0;
+  return h->scheme == LBM_SCHEME_AB ? MODE_PULL : MODE_NATURAL;
+}
+
+void finish_init(lbm_handle_s* h) {
   h->phase = 0;
   h->time = 0;
   h->stepped = false;
+}
+
+// InitPDF on rows [r0, r1): ONE kernel, feq straight into the storage buffer (init_equilibrium_kernel)
+void launch_init_rows(lbm_handle_s* h, const Ctx& c, int mode, const double* rho, const double* u, int r0, int r1) {
+  LBM_Q_CALL(h, launch_init, c, mode, rho, u, h->buf[h->cur], r0, r1, grid_for_rows(h, r1 - r0));
+  ++h->launches;
+}
+
+int do_init(lbm_handle_s* h, const double* rho, const double* u) {
+  const int mode = init_target(h);
+  const Ctx c = make_ctx(h);
+  launch_init_rows(h, c, mode, rho, u, rows_begin(h), rows_end(h));
+  finish_init(h);
   return check_launch("init_equilibrium");
+}
+
+// diagnostics: reduce the `nblocks` block partials, copy the 8 doubles to the host, synchronise
+int finish_diagnostics(lbm_handle_s* h, int nblocks, double* diagnostics) {
+  reduce_final_kernel<><<<1, 256, 0, h->stream>>>(h->partials, nblocks, h->diag_dev);
+  ++h->launches;
+  int rc = check_launch("moments");
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(h->diag_pinned, h->diag_dev, kDiag * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  std::memcpy(diagnostics, h->diag_pinned, kDiag * sizeof(double));
+  return LBM_OK;
 }
 
 int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
@@ -277,19 +299,60 @@ int do_moments(lbm_handle_s* h, double* rho, double* u, double* diagnostics) {
     if (rc) return rc;
   }
   const Ctx c = make_ctx(h);
-  double* partials = diagnostics ? h->partials : nullptr;
-  LBM_Q_CALL(h, launch_moments, c, read_mode(h), h->buf[h->cur], rho, u, partials);
+  const int grid = grid_for_rows(h, rows_end(h) - rows_begin(h));
+  LBM_Q_CALL(h, launch_moments, c, read_mode(h), h->buf[h->cur], rho, u, diagnostics ? h->partials : nullptr, rows_begin(h), rows_end(h), grid);
   ++h->launches;
-  if (diagnostics) {
-    reduce_final_kernel<><<<1, 256, 0, h->stream>>>(h->partials, c.flat_grid, h->diag_dev);
-    ++h->launches;
+  if (diagnostics) return finish_diagnostics(h, grid, diagnostics);
+  return check_launch("moments");
+}
+
+// ---- host entry points: z-chunked so that the PCIe copies overlap the kernels ----------------------------------
+// Device staging for the 4N doubles of rho, u: the idle A/B buffer (Q*elem >= 32 B per cell for every lattice), else —
+// in-place scheme, or a z-slab, whose idle buffer's halo planes belong to the neighbours' next step — the scratch buffer.
+int host_staging(lbm_handle_s* h, double** out) {
+  if (h->scheme == LBM_SCHEME_AB && !h->slab) {
+    *out = (double*)h->buf[h->cur ^ 1];
+    return LBM_OK;
   }
-  int rc = check_launch("moments");
+  int rc = ensure_scratch(h, (size_t)h->N * 4 * sizeof(double));
   if (rc) return rc;
-  if (diagnostics) {
-    CUDA_TRY(cudaMemcpyAsync(h->diag_pinned, h->diag_dev, kDiag * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    std::memcpy(diagnostics, h->diag_pinned, kDiag * sizeof(double));
+  *out = (double*)h->scratch;
+  return LBM_OK;
+}
+
+int ensure_copy_stream(lbm_handle_s* h) {
+  if (h->copy_stream) return LBM_OK;
+  CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  for (int k = 0; k < kMaxChunks; ++k) CUDA_TRY(cudaEventCreateWithFlags(&h->chunk_ev[k], cudaEventDisableTiming));
+  CUDA_TRY(cudaEventCreateWithFlags(&h->fence_ev, cudaEventDisableTiming));
+  return LBM_OK;
+}
+
+// plane ranges [zc[k], zc[k+1]) of the updated planes, k < n
+int plane_chunks(const lbm_handle_s* h, int* zc) {
+  const int planes = h->p.z_hi - h->p.z_lo;
+  const size_t plane_bytes = (size_t)h->nx * h->ny * 4 * sizeof(double);
+  long long n = (long long)(plane_bytes * planes / kChunkBytes);
+  n = n < 1 ? 1 : n > kMaxChunks ? kMaxChunks : n;
+  if (n > planes) n = planes;
+  for (int k = 0; k <= n; ++k) zc[k] = h->p.z_lo + (int)((long long)planes * k / n);
+  return (int)n;
+}
+
+// one chunk of rho / u between host and device staging (planes [z0, z1) of each component)
+int copy_chunk(lbm_handle_s* h, double* dev_rho, double* dev_u, double* host_rho, double* host_u, int z0, int z1, bool to_device) {
+  const size_t off = (size_t)h->nx * h->ny * z0, n = (size_t)h->nx * h->ny * (z1 - z0) * sizeof(double);
+  const cudaMemcpyKind kind = to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
+  if (host_rho) {
+    if (to_device) CUDA_TRY(cudaMemcpyAsync(dev_rho + off, host_rho + off, n, kind, h->copy_stream));
+    else CUDA_TRY(cudaMemcpyAsync(host_rho + off, dev_rho + off, n, kind, h->copy_stream));
+  }
+  if (host_u) {
+    for (int d = 0; d < 3; ++d) {
+      const size_t o = (size_t)h->N * d + off;
+      if (to_device) CUDA_TRY(cudaMemcpyAsync(dev_u + o, host_u + o, n, kind, h->copy_stream));
+      else CUDA_TRY(cudaMemcpyAsync(host_u + o, dev_u + o, n, kind, h->copy_stream));
+    }
   }
   return LBM_OK;
 }
@@ -377,7 +440,7 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   const int Q = lattice & 0xff;
   if (Q != 9 && Q != 19 && Q != 27) { fail(LBM_EINVAL, "lbm_create: lattice must be LBM_D2Q9, LBM_D3Q19 or LBM_D3Q27"); return nullptr; }
   if (nx < 1 || ny < 1 || nz < 1) { fail(LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1"); return nullptr; }
-  if ((long long)nx * ny * nz >= (1LL << 31)) { fail(LBM_EUNSUPPORTED, "lbm_create: nx*ny*nz must be < 2^31 (in-plane offsets are 32-bit)"); return nullptr; }
+  if ((long long)nx * ny * nz >= (1LL << 31)) { fail(LBM_EUNSUPPORTED, "lbm_create: nx*ny*nz must be < 2^31 (cell indices are 32-bit)"); return nullptr; }
   if (nz > 65535 || ny > 65535) { fail(LBM_EINVAL, "lbm_create: ny or nz exceeds the launch grid limits"); return nullptr; }
   if (!(tau > 0.5) || !std::isfinite(tau)) { fail(LBM_EINVAL, "lbm_create: tau must be finite and > 0.5"); return nullptr; }
   int scheme = lattice & (3 << 12);
@@ -396,6 +459,10 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   h->N = (long long)nx * ny * nz;
   h->tau = tau;
   h->soa = (lattice & LBM_LAYOUT_SOA) ? 1 : 0;
+  // In-plane storage offsets x + y*rs are 32-bit in the kernels.  Row-interleaved: rs = Q*nx, so the bound is
+  // Q*nx*ny < 2^31; a plane beyond it (a 16384^2 D2Q9 grid) is stored as a plain structure of arrays, whose in-plane
+  // bound nx*ny < 2^31 holds for every grid accepted above.  The layout is internal: results are identical bit for bit.
+  if (!h->soa && (long long)Q * nx * ny >= (1LL << 31)) h->soa = 1;
   Params& p = h->p;
   p.nx = nx; p.ny = ny; p.nz = nz; p.N = h->N;
   if (h->soa) { p.ds = h->N; p.rs = nx; p.zs = (long long)nx * ny; }
@@ -478,7 +545,7 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
   cudaError_t e = cudaSuccess;
   for (int b = 0; b < nbuf && e == cudaSuccess; ++b) e = cudaMalloc(&h->buf[b], h->buf_bytes());
-  if (e == cudaSuccess) e = cudaMalloc((void**)&h->partials, (size_t)kReduceBlocks * kDiag * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->partials, (size_t)kMaxChunks * kReduceBlocks * kDiag * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc((void**)&h->diag_dev, kDiag * sizeof(double));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&h->diag_pinned, kDiag * sizeof(double));
   if (e == cudaSuccess && slab) {
@@ -528,6 +595,10 @@ int lbm_slab_export(lbm_handle h, lbm_slab_peer_t* out) {
   out->flags = (uint64_t)h->flags;
   out->plane_stride = h->N;
   out->nz_local = h->nz_local;
+  out->Q = h->Q;
+  out->elem_bytes = (int32_t)h->elem();
+  out->layout_soa = h->soa;
+  out->stream = (uint64_t)h->stream;
   int dev = 0;
   CUDA_TRY(cudaGetDevice(&dev));
   out->device = dev;
@@ -591,6 +662,17 @@ int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_
     if (!d) continue;
     if (d->plane_stride != plane * (d->nz_local + 2) || d->nz_local < 1)
       { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: neighbour descriptor does not match this slab's nx, ny"); }
+    // the halo stores write the neighbour's buffer in THIS slab's lattice, element type and layout
+    if (d->Q != h->Q || d->elem_bytes != (int32_t)h->elem() || d->layout_soa != h->soa)
+      { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: neighbour has another lattice, storage type or layout"); }
+    // two different slabs of one process on ONE stream: the second step of one waits (in the stream) for the first step
+    // of the other, which is queued behind that wait
+    if (d->pid == (int64_t)getpid() && d->buf[0] != (uint64_t)h->buf[0] && d->stream == (uint64_t)h->stream) {
+      int dev = 0;
+      cudaGetDevice(&dev);
+      if (d->device == dev)
+        { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: connected slabs of one process need a stream each (lbm_bc_t.stream)"); }
+    }
     void* b[2] = {nullptr, nullptr};
     void* fl = nullptr;
     int rc = map_peer(h, d, d->buf[0], d->ipc_buf[0], &b[0]);
@@ -632,6 +714,12 @@ void lbm_destroy(lbm_handle h) {
   if (h->diag_dev) cudaFree(h->diag_dev);
   if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
   if (h->scratch) cudaFree(h->scratch);
+  if (h->copy_stream) {
+    cudaStreamSynchronize(h->copy_stream);
+    for (int k = 0; k < kMaxChunks; ++k) cudaEventDestroy(h->chunk_ev[k]);
+    cudaEventDestroy(h->fence_ev);
+    cudaStreamDestroy(h->copy_stream);
+  }
   for (int k = 0; k < 6; ++k)
     if (h->p.face_prof[k]) cudaFree((void*)h->p.face_prof[k]);
   free_geometry(h);
@@ -744,30 +832,31 @@ int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u) {
 
 int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host) {
   if (!h) return fail(LBM_EINVAL, "lbm_init_equilibrium_host: NULL handle");
-  if (h->slab) h->cur = 0;  // as do_init will (the staging below depends on it)
-  // Stage the 4N doubles in device memory that do_init does not write before it has read them:
-  // the CURRENT storage buffer for fp64 A/B (do_init writes the idle one first), else scratch.
+  if (!rho_host && !u_host) return do_init(h, nullptr, nullptr);
+  const int mode = init_target(h);  // fixes h->cur: the staging below is the OTHER buffer
   double* stage = nullptr;
-  const size_t need = (size_t)h->N * 4 * sizeof(double);
-  if (h->scheme == LBM_SCHEME_AB && !h->f32) {
-    stage = (double*)h->buf[h->cur];
-  } else {
-    // scratch holds the canonical staging (Q*N doubles) followed by the 4N input doubles
-    int rc = ensure_scratch(h, (size_t)h->N * h->Q * sizeof(double) + need);
+  int rc = host_staging(h, &stage);
+  if (!rc) rc = ensure_copy_stream(h);
+  if (rc) return rc;
+  double* d_rho = rho_host ? stage : nullptr;
+  double* d_u = u_host ? stage + h->N : nullptr;
+  const Ctx c = make_ctx(h);
+  int zc[kMaxChunks + 1];
+  const int n = plane_chunks(h, zc);
+  // the copies may start once everything queued on the handle's stream has left the staging buffer
+  CUDA_TRY(cudaEventRecord(h->fence_ev, h->stream));
+  CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->fence_ev, 0));
+  for (int k = 0; k < n; ++k) {
+    // the kernel of a chunk reads rho, u of its own cells only (it pushes f_a towards the upstream slot), so chunk k
+    // is initialised while chunk k+1 is still on the bus
+    rc = copy_chunk(h, d_rho, d_u, const_cast<double*>(rho_host), const_cast<double*>(u_host), zc[k], zc[k + 1], true);
     if (rc) return rc;
-    stage = (double*)h->scratch + (size_t)h->N * h->Q;
+    CUDA_TRY(cudaEventRecord(h->chunk_ev[k], h->copy_stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->stream, h->chunk_ev[k], 0));
+    launch_init_rows(h, c, mode, d_rho, d_u, h->ny * zc[k], h->ny * zc[k + 1]);
   }
-  double* d_rho = nullptr;
-  double* d_u = nullptr;
-  if (rho_host) {
-    d_rho = stage;
-    CUDA_TRY(cudaMemcpyAsync(d_rho, rho_host, (size_t)h->N * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-  }
-  if (u_host) {
-    d_u = stage + h->N;
-    CUDA_TRY(cudaMemcpyAsync(d_u, u_host, (size_t)h->N * 3 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-  }
-  return do_init(h, d_rho, d_u);
+  finish_init(h);
+  return check_launch("init_equilibrium_host");
 }
 
 int lbm_step(lbm_handle h, int nsteps) {
@@ -823,22 +912,35 @@ int lbm_moments(lbm_handle h, double* rho, double* u, double* diagnostics) {
 int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* diagnostics) {
   if (!h) return fail(LBM_EINVAL, "lbm_moments_host: NULL handle");
   if (!rho_host && !u_host && !diagnostics) return LBM_OK;
+  if (!rho_host && !u_host) return do_moments(h, nullptr, nullptr, diagnostics);
   double* stage = nullptr;
-  if (rho_host || u_host) {
-    if (h->scheme == LBM_SCHEME_AB && !h->f32) {
-      stage = (double*)h->buf[h->cur ^ 1];
-    } else {
-      int rc = ensure_scratch(h, (size_t)h->N * 4 * sizeof(double));
-      if (rc) return rc;
-      stage = (double*)h->scratch;
-    }
-  }
+  int rc = host_staging(h, &stage);
+  if (!rc) rc = ensure_copy_stream(h);
+  if (!rc) rc = slab_wait_neighbours(h);  // the pull reads the halo planes
+  if (rc) return rc;
   double* d_rho = rho_host ? stage : nullptr;
   double* d_u = u_host ? stage + h->N : nullptr;
-  int rc = do_moments(h, d_rho, d_u, diagnostics);
+  const Ctx c = make_ctx(h);
+  int zc[kMaxChunks + 1];
+  const int n = plane_chunks(h, zc);
+  int nblocks = 0;
+  for (int k = 0; k < n; ++k) {
+    // chunk k goes to the host while chunk k+1 is being computed; every chunk keeps its own block partials
+    const int r0 = h->ny * zc[k], r1 = h->ny * zc[k + 1], grid = grid_for_rows(h, r1 - r0);
+    LBM_Q_CALL(h, launch_moments, c, read_mode(h), h->buf[h->cur], d_rho, d_u, diagnostics ? h->partials + (size_t)nblocks * kDiag : nullptr, r0, r1, grid);
+    ++h->launches;
+    nblocks += grid;
+    CUDA_TRY(cudaEventRecord(h->chunk_ev[k], h->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->chunk_ev[k], 0));
+    rc = copy_chunk(h, d_rho, d_u, rho_host, u_host, zc[k], zc[k + 1], false);
+    if (rc) return rc;
+  }
+  rc = check_launch("moments_host");
   if (rc) return rc;
-  if (rho_host) CUDA_TRY(cudaMemcpyAsync(rho_host, d_rho, (size_t)h->N * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  if (u_host) CUDA_TRY(cudaMemcpyAsync(u_host, d_u, (size_t)h->N * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  // whatever the handle's stream runs next (a step overwrites the staging buffer) comes after the copies
+  CUDA_TRY(cudaEventRecord(h->fence_ev, h->copy_stream));
+  CUDA_TRY(cudaStreamWaitEvent(h->stream, h->fence_ev, 0));
+  if (diagnostics) return finish_diagnostics(h, nblocks, diagnostics);  // synchronises the stream, hence the copies
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LBM_OK;
 }

@@ -100,6 +100,21 @@ bool launch_cooperative(K kernel, const Ctx& c, void** args, bool allow_stride) 
 template <>
 void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
   if (c.p.any_sym) return launch_step_ab_sym<Q_>(c, src, dst);  // part 6
+  if (c.f32 && c.bc != BC_GEO && c.p.nx % 2 == 0 && !c.p.slab) {
+    // fp32 storage: two cells per thread, one row per block (stream_collide_ab_f32x2)
+    int bx = 32;
+    while (bx < 128 && 2 * bx < c.p.nx) bx *= 2;
+    const dim3 block(bx, 1, 1), grid((c.p.nx / 2 + bx - 1) / bx, c.p.ny, c.p.nz);
+    dispatch_eq(c, [&](auto eq) {
+      dispatch_force(c, [&](auto force) {
+        if (c.bc == BC_WALLS)
+          stream_collide_ab_f32x2<Q_, decltype(eq)::value, BC_WALLS, decltype(force)::value != 0><<<grid, block, 0, c.stream>>>((const float*)src, (float*)dst, c.p);
+        else
+          stream_collide_ab_f32x2<Q_, decltype(eq)::value, BC_PERIODIC, decltype(force)::value != 0><<<grid, block, 0, c.stream>>>((const float*)src, (float*)dst, c.p);
+      });
+    });
+    return;
+  }
   dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
     using ST = decltype(st);
     stream_collide_ab<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
@@ -234,9 +249,17 @@ void launch_import<Q_>(const Ctx& c, int mode, const double* in, void* buf) {
   });
 }
 template <>
-void launch_init<Q_>(const Ctx& c, const double* rho, const double* u, double* out) {
+void launch_init<Q_>(const Ctx& c, int mode, const double* rho, const double* u, void* buf, int r0, int r1, int grid) {
   dispatch_eq(c, [&](auto eq) {
-    init_equilibrium_kernel<Q_, decltype(eq)::value><<<c.flat_grid, 256, 0, c.stream>>>(rho, u, out, c.fbx, c.p);
+    dispatch_bc(c, [&](auto bc) {
+      dispatch_storage(c, [&](auto st) {
+        using ST = decltype(st);
+        if (mode == MODE_PULL)
+          init_equilibrium_kernel<Q_, decltype(eq)::value, decltype(bc)::value, MODE_PULL, ST><<<grid, 256, 0, c.stream>>>(rho, u, (ST*)buf, c.fbx, r0, r1, c.p);
+        else
+          init_equilibrium_kernel<Q_, decltype(eq)::value, decltype(bc)::value, MODE_NATURAL, ST><<<grid, 256, 0, c.stream>>>(rho, u, (ST*)buf, c.fbx, r0, r1, c.p);
+      });
+    });
   });
 }
 template <>
@@ -246,14 +269,14 @@ void launch_geometry<Q_>(const Ctx& c, const uint8_t* geo_in, uint8_t* geo, uint
 }
 #elif LBM_PART == 4
 template <>
-void launch_moments<Q_>(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials) {
+void launch_moments<Q_>(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials, int r0, int r1, int grid) {
   dispatch_mode(mode, [&](auto m) {
     dispatch_eq(c, [&](auto eq) {
       dispatch_bc(c, [&](auto bc) {
         dispatch_storage(c, [&](auto st) {
           using ST = decltype(st);
           moments_kernel<Q_, decltype(eq)::value, decltype(bc)::value, decltype(m)::value, ST>
-              <<<c.flat_grid, 256, 0, c.stream>>>((const ST*)buf, rho, u, partials, c.fbx, c.p);
+              <<<grid, 256, 0, c.stream>>>((const ST*)buf, rho, u, partials, c.fbx, r0, r1, c.p);
         });
       });
     });

@@ -69,13 +69,8 @@ __device__ __forceinline__ void static_for(F&& f) {
 // Measured on B200: the A/B D3Q19 kernels fit 80 registers without spilling and need the third block;
 // the fp32-storage A/B kernel keeps its populations packed (collide_shifted) and fits 64 registers, which
 // buys the fourth block its half-size loads need; the forced and in-place variants and D3Q27 spill below 128.
-#ifdef LBM_MB_OVERRIDE  // tuning hook for occupancy sweeps (python -m paper_2201_11330_b200.build --force -DLBM_MB_OVERRIDE=n)
-template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
-constexpr int kMinBlocks = LBM_MB_OVERRIDE;
-#else
 template <int Q, bool FORCE, bool INPLACE, int STBYTES = 8>
 constexpr int kMinBlocks = (Q == 9) ? (FORCE || INPLACE ? 3 : 4) : (Q == 27 && STBYTES == 4 && !INPLACE) ? 3 : (Q == 19 && STBYTES == 4 && !INPLACE) ? (FORCE ? 3 : 4) : (Q == 19 && !FORCE && !INPLACE) ? 3 : 2;
-#endif
 
 // ---------------------------------------------------------------------------------------
 // How a cell finds out that a link has no upstream node (template parameter BC):
@@ -269,34 +264,11 @@ __device__ __forceinline__ T* plane(T* buf, long long N) {
   return buf + (long long)A * N;
 }
 
-// Cache policy of the population streams of the A/B step kernel (tuning hooks; defaults chosen by measurement,
-// DESIGN.md section 6): every population is read once and written once per step, nothing is re-used.
-//   LBM_LD_POLICY 0 ld.global.nc (__ldg)  1 .cs (streaming)  2 .cg (L2 only)  3 .lu (last use)
-//   LBM_ST_POLICY 0 plain st.global       1 .cs              2 .cg            3 .wt
-#ifndef LBM_LD_POLICY
-#define LBM_LD_POLICY 0
-#endif
-#ifndef LBM_ST_POLICY
-#define LBM_ST_POLICY 0
-#endif
-#if LBM_LD_POLICY == 1
-#define LBM_LD_STREAM(q) __ldcs(q)
-#elif LBM_LD_POLICY == 2
-#define LBM_LD_STREAM(q) __ldcg(q)
-#elif LBM_LD_POLICY == 3
-#define LBM_LD_STREAM(q) __ldlu(q)
-#else
+// The population streams of the A/B step kernel: every value is read once and written once per step, nothing is
+// re-used.  Loads take the non-coherent path (ld.global.nc), stores are plain: every other cache policy measured the
+// same or slower (profiles/cache_policy_r01d.txt).
 #define LBM_LD_STREAM(q) __ldg(q)
-#endif
-#if LBM_ST_POLICY == 1
-#define LBM_ST_STREAM(q, v) __stcs(q, v)
-#elif LBM_ST_POLICY == 2
-#define LBM_ST_STREAM(q, v) __stcg(q, v)
-#elif LBM_ST_POLICY == 3
-#define LBM_ST_STREAM(q, v) __stwt(q, v)
-#else
 #define LBM_ST_STREAM(q, v) (*(q) = (v))
-#endif
 
 // ---------------------------------------------------------------------------------------
 // Storage element access.  fp64: the value itself.  fp32 storage (S:§8f NEXT-1): f - t_a is
@@ -861,6 +833,76 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
   ab_cell<Q, EQ, BC, FORCE, ST, SLAB, SYM, false>(src, dst, p, x, y, z);
 }
 
+// fp32 storage, two cells per thread (S:§8f NEXT-1).  With half the bytes per cell the one-cell kernel above is bound by
+// issue slots, not by DRAM (ncu, 512^3 D3Q19: 576 instructions per cell, 165 of them integer address arithmetic, issue
+// 61 %, DRAM 81 %, and under the power cap of a sustained run the SM clock falls to ~1.6 GHz, where the issue rate
+// is the limit).  Here a thread owns the x-adjacent cells (x, x+1), x even, of a row that is uniform per block (the
+// block is bx x 1, y = blockIdx.y, z = blockIdx.z): the Q row bases are block-invariant and live in uniform registers,
+// the nine e_x = 0 streams are read and ALL Q streams are written as aligned 8-byte float2 accesses, and the address
+// arithmetic is paid once per pair.  Same arithmetic per cell as ab_cell (collide_shifted): bit-identical results.
+// A/B, BC_PERIODIC / BC_WALLS, even nx; everything else (link mask, z-slabs, odd nx) stays with the one-cell kernel.
+#ifndef LBM_F32X2_MB
+#define LBM_F32X2_MB 6
+#endif
+template <int Q, int EQ, int BC, bool FORCE>
+__global__ void __launch_bounds__(128, LBM_F32X2_MB) stream_collide_ab_f32x2(const float* __restrict__ src, float* __restrict__ dst, const __grid_constant__ Params p) {
+  static_assert(BC != BC_GEO, "the link-mask kernels keep one cell per thread");
+  const int x = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int y = blockIdx.y, z = blockIdx.z;
+  if (x >= p.nx) return;
+  // Addresses = one per-thread pointer per z-plane (the cell pair's x in row 0 of that plane) + a block-uniform
+  // in-plane offset (direction row + y row, periodic wrap by conditional add as in Neigh; uniform datapath): one 64-bit
+  // add per direction and pair.  The odd element of a shifted stream sits one float before / after the pair, except
+  // in the two lanes of a row where the pull wraps around in x: a per-thread element offset dm / dp covers both.
+  const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
+  // (byte addresses as integers: a plain 64-bit add per access; element indices would be scaled and added to the
+  // base one access at a time)
+  typedef unsigned long long addr_t;
+  const long long oyb[3] = {4LL * ym * p.rs, 4LL * y * p.rs, 4LL * yp * p.rs};
+  const addr_t xb = (addr_t)__cvta_generic_to_global(src) + 4ull * x;
+  const addr_t P[3] = {xb + 4ull * (zm * p.zs), xb + 4ull * (z * p.zs), xb + 4ull * (zp * p.zs)};
+  const long long dsb = 4LL * p.ds;
+  const long long dm = (x == 0) ? 4LL * (p.nx - 1) : -4LL;  // cell 0's x - 1, in bytes relative to x
+  const long long dp = (x + 2 == p.nx) ? -4LL * x : 8LL;    // cell 1's x + 1
+  const int cell0 = x + p.nx * (y + p.ny * z);
+  const CellFlags<BC> c0(p, x, y, z, cell0), c1(p, x + 1, y, z, cell0 + 1);
+  float g0[Q], g1[Q];
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    using D = Dir<Q, a>;
+    constexpr int o = D::opp;
+    // pair base in the row of the upstream node (x - e_a), and in the wall slot's row (own row, opposite direction;
+    // t_a == t_abar: same shift)
+    const addr_t up = P[1 - D::ez] + (addr_t)(a * dsb + oyb[1 - D::ey]);
+    if constexpr (D::ex == 0) {
+      addr_t q = up;
+      if constexpr (BC == BC_WALLS && D::s > 0) {
+        if (c0.template leaves<Q, a, -1>()) q = P[1] + (addr_t)(o * dsb + oyb[1]);  // depends on y, z only: the same for both cells
+      }
+      asm("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(g0[a]), "=f"(g1[a]) : "l"(q));
+    } else {
+      // e_x = +1 pulls from (x-1, x), e_x = -1 from (x+1, x+2)
+      addr_t q0 = up + (addr_t)(D::ex == 1 ? dm : 4LL);
+      addr_t q1 = up + (addr_t)(D::ex == 1 ? 0LL : dp);
+      if constexpr (BC == BC_WALLS) {
+        const addr_t wl = P[1] + (addr_t)(o * dsb + oyb[1]);
+        if (c0.template leaves<Q, a, -1>()) q0 = wl;
+        if (c1.template leaves<Q, a, -1>()) q1 = wl + 4;
+      }
+      asm("ld.global.nc.f32 %0, [%1];" : "=f"(g0[a]) : "l"(q0));
+      asm("ld.global.nc.f32 %0, [%1];" : "=f"(g1[a]) : "l"(q1));
+    }
+  });
+  const addr_t O = (addr_t)__cvta_generic_to_global(dst) + 4ull * (z * p.zs + x) + (addr_t)oyb[1];
+  // cell 0 in place (its results wait in g0 for their partners), then cell 1, stored as pairs
+  collide_shifted<Q, EQ, BC, FORCE>(g0, p, c0, cell0, z, [&](auto A, double v) { g0[decltype(A)::value] = (float)v; });
+  collide_shifted<Q, EQ, BC, FORCE>(g1, p, c1, cell0 + 1, z, [&](auto A, double v) {
+    constexpr int a = decltype(A)::value;
+    asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(O + (addr_t)(a * dsb)), "f"(g0[a]), "f"((float)v) : "memory");
+  });
+}
+
 // Small grids (both buffers resident in the L2: 32^3, 64^3, the paper's 512 x 128 channel) are bound by the launch
 // rate of one kernel per step (4-5 us), and CUDA-graph replay is slower still.  This persistent kernel takes all the steps of one lbm_step call in ONE cooperative
 // launch: every thread keeps its cell, the two buffers swap roles each step, a grid-wide barrier separates the steps
@@ -1025,13 +1067,16 @@ __device__ __forceinline__ void load_canonical(double (&f)[Q], const ST* buf, co
 // One 32-bit division per row, none per cell; x stays the coalesced direction.
 // The rows are those of the updated planes [z_lo, z_hi), or of every plane (the halo planes of a slab too).
 template <typename F>
-__device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body, bool with_halo = false) {
+__device__ __forceinline__ void for_each_cell_in_rows(const Params& p, int bx, int r0, int rows, F&& body) {
   const int tx = threadIdx.x & (bx - 1), ty = threadIdx.x / bx, by = blockDim.x / bx;
-  const int r0 = with_halo ? 0 : p.ny * p.z_lo, rows = with_halo ? p.ny * p.nz : p.ny * p.z_hi;
   for (int r = r0 + blockIdx.x * by + ty; r < rows; r += gridDim.x * by) {
     const int z = r / p.ny, y = r - z * p.ny;
     for (int x = tx; x < p.nx; x += bx) body(x, y, z, x + p.nx * r);
   }
+}
+template <typename F>
+__device__ __forceinline__ void for_each_cell(const Params& p, int bx, F&& body, bool with_halo = false) {
+  for_each_cell_in_rows(p, bx, with_halo ? 0 : p.ny * p.z_lo, with_halo ? p.ny * p.nz : p.ny * p.z_hi, body);
 }
 
 // lbm_get_populations: canonical f[a*N+i] (always fp64) out of the storage buffer; inactive nodes report 0.
@@ -1090,19 +1135,51 @@ __global__ void __launch_bounds__(256) import_canonical(const double* __restrict
   }, p.slab != 0);
 }
 
-// InitPDF: canonical f_a(x) = feq_a(rho(x), u(x)), natural fp64 layout.
-template <int Q, int EQ>
-__global__ void __launch_bounds__(256) init_equilibrium_kernel(const double* __restrict__ rho, const double* __restrict__ u, double* __restrict__ out, int bx, const __grid_constant__ Params p) {
-  for_each_cell(p, bx, [&](int, int, int, int i) {
+// InitPDF: f_a(x, 0) = feq_a(rho(x), u(x)), written straight into the storage buffer in the layout the
+// scheme wants at an even phase (S:§8c-S: "f^eq evaluated at the downstream cell") — one pass, 32 B read + Q stored
+// elements per cell, instead of a canonical array that is written, read back and written again.
+//   NATURAL (AA):  slot(x, a) = f_a(x).
+//   PULL (A/B):    B = S^-1 f as a PUSH from the cell that owns the value: f_a(x) goes where the pull of x will look for
+//                  it — slot(x - e_a, a) if the link has an active upstream node, the wall slot(x, abar) otherwise, the
+//                  mirror image's slot through SYMMETRY faces (D:R25).  Every slot the first step reads is written by
+//                  exactly one cell (S is a bijection on the slots); shifted stores stay unit-stride in x.
+// Eq. 10 at t = 0 (D:R17) needs nothing here: the pull replicates f_abar into the wall links of a nodal wall node
+// every time it gathers, so what their wall slots hold is never used.  A z-slab pushes from its own planes only: the
+// slots of its halo planes that the first step reads are exactly the ones its first / last plane push into.
+// Rows [r0, r1) of the grid (r = y + ny*z): the host entry point initialises z-chunks as their rho, u arrive.
+template <int Q, int EQ, int BC, int MODE, typename ST>
+__global__ void __launch_bounds__(256, 2) init_equilibrium_kernel(const double* __restrict__ rho, const double* __restrict__ u, ST* __restrict__ buf, int bx,
+                                                               int r0, int r1, const __grid_constant__ Params p) {
+  static_assert(MODE != MODE_PULL_SWAP, "initialisation always lands in an even phase");
+  for_each_cell_in_rows(p, bx, r0, r1, [&](int x, int y, int z, int i) {
+    const Neigh nb(p, x, y, z);
+    const CellFlags<BC> c(p, x, y, z, i);
+    if (!c.template active<Q>()) return;
     const double r = rho ? rho[i] : 1.0;
     const double ux = u ? u[i] : 0.0, uy = u ? plane<1>(u, p.N)[i] : 0.0, uz = u ? plane<2>(u, p.N)[i] : 0.0;
     double feq[Q];
     equilibrium<Q, EQ>(feq, r, ux, uy, uz);
+    const bool at_mirror = (BC == BC_GEO) ? touches_sym<BC>(p, c) : false;
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
-      plane<a>(out, p.N)[i] = feq[a];
+      constexpr int o = Dir<Q, a>::opp;
+      ST* q = plane<a>(buf, p.ds) + nb.ic;
+      if constexpr (MODE == MODE_PULL && Dir<Q, a>::s > 0) {
+        q = plane<a>(buf, p.ds) + nb.template at<Q, a, -1>();
+        if constexpr (BC != BC_PERIODIC) {
+          if (c.template leaves<Q, a, -1>()) q = plane<o>(buf, p.ds) + nb.ic;
+        }
+        if constexpr (BC == BC_GEO) {
+          if (at_mirror) {
+            int dir, cidx;
+            long long idx;
+            if (mirror_link<Q, a, -1, BC>(p, c, nb, dir, idx, cidx) && !c.template leaves<Q, a, -1>()) q = buf + dir * p.ds + idx;
+          }
+        }
+      }
+      st_pop<ST, Q, a>(q, 0, feq[a]);
     });
-  }, p.slab != 0);
+  });
 }
 
 // ---------------------------------------------------------------------------------------
@@ -1218,9 +1295,10 @@ __device__ __forceinline__ void block_reduce_diag(double (&acc)[kDiag], double* 
 // The F/2 shift of D:R7 is always applied (adding 0.5*0 is exact), so there is no FORCE variant here.
 template <int Q, int EQ, int BC, int MODE, typename ST>
 __global__ void __launch_bounds__(256, 2) moments_kernel(const ST* buf, double* __restrict__ rho_out, double* __restrict__ u_out,
-                                                      double* __restrict__ partials, int bx, const __grid_constant__ Params p) {
+                                                      double* __restrict__ partials, int bx, int r0, int r1, const __grid_constant__ Params p) {
+  // rows [r0, r1) of the grid (r = y + ny*z): lbm_moments_host sweeps z-chunks so that their copies to the host overlap
   double acc[kDiag] = {0, 0, 0, 0, 0, 0, INFINITY, 0};
-  for_each_cell(p, bx, [&](int x, int y, int z, int i) {
+  for_each_cell_in_rows(p, bx, r0, r1, [&](int x, int y, int z, int i) {
     const Neigh nb(p, x, y, z);
     const CellFlags<BC> c(p, x, y, z, i);
     if (!c.template active<Q>()) {  // Monitor runs over the fluid nodes; inactive nodes report 0

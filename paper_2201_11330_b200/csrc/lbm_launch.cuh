@@ -32,8 +32,9 @@ template <int Q> void launch_step_aa_even(const Ctx& c, void* buf);
 template <int Q> void launch_step_aa_odd(const Ctx& c, void* buf);
 template <int Q> void launch_export(const Ctx& c, int mode, const void* buf, double* out);
 template <int Q> void launch_import(const Ctx& c, int mode, const double* in, void* buf);
-template <int Q> void launch_init(const Ctx& c, const double* rho, const double* u, double* out);
-template <int Q> void launch_moments(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials);
+// rows [r0, r1) of the grid (r = y + ny*z) on `grid` blocks: the host entry points work through z-chunks
+template <int Q> void launch_init(const Ctx& c, int mode, const double* rho, const double* u, void* buf, int r0, int r1, int grid);
+template <int Q> void launch_moments(const Ctx& c, int mode, const void* buf, double* rho, double* u, double* partials, int r0, int r1, int grid);
 template <int Q> void launch_geometry(const Ctx& c, const uint8_t* geo_in, uint8_t* geo, uint8_t* active, uint32_t* links, int nodal);
 template <int Q> void launch_boundary_force(const Ctx& c, int mode, const void* buf, const uint8_t* geo, double* partials);
 

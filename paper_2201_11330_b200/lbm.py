@@ -22,8 +22,7 @@ LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE, LBM_FACE
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
 
-# LBM_B200_LIB points at another build of the same library (occupancy sweeps); it must exist just the same
-LIB_PATH = os.environ.get("LBM_B200_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
@@ -54,6 +53,11 @@ class lbm_slab_peer_t(C.Structure):
         ("nz_local", C.c_int32),
         ("device", C.c_int32),
         ("pid", C.c_int64),
+        ("Q", C.c_int32),
+        ("elem_bytes", C.c_int32),
+        ("layout_soa", C.c_int32),
+        ("reserved", C.c_int32),
+        ("stream", C.c_uint64),
         ("ipc_buf", (C.c_uint8 * 64) * 2),
         ("ipc_flags", C.c_uint8 * 64),
     ]
