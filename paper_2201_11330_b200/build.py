@@ -27,6 +27,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo", "--fmad=true",
     "-Xcompiler", "-fPIC", "-diag-suppress", "177",
+    "-Xfatbin", "-compress-all",  # 145 MB -> 36 MB of device code (the .so travels to the GPU box with every call)
 ]
 
 

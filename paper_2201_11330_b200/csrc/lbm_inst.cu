@@ -100,10 +100,10 @@ bool launch_cooperative(K kernel, const Ctx& c, void** args, bool allow_stride) 
 template <>
 void launch_step_ab<Q_>(const Ctx& c, const void* src, void* dst) {
   if (c.p.any_sym) return launch_step_ab_sym<Q_>(c, src, dst);  // part 6
-  if (c.f32 && c.bc != BC_GEO && c.p.nx % 2 == 0 && !c.p.slab) {
+  if constexpr (Q_ != 27) if (c.f32 && c.bc != BC_GEO && c.p.nx % 2 == 0 && !c.p.slab) {
     // fp32 storage: two cells per thread, one row per block (stream_collide_ab_f32x2)
     int bx = 32;
-    while (bx < 128 && 2 * bx < c.p.nx) bx *= 2;
+    while (bx < kF32x2Threads && 2 * bx < c.p.nx) bx *= 2;
     const dim3 block(bx, 1, 1), grid((c.p.nx / 2 + bx - 1) / bx, c.p.ny, c.p.nz);
     dispatch_eq(c, [&](auto eq) {
       dispatch_force(c, [&](auto force) {

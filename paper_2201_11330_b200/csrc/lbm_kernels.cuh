@@ -594,37 +594,46 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
     k = 1.0 - 0.5 * om;
     uF3 = 3.0 * (ux * p.F[0] + uy * p.F[1] + uz * p.F[2]);
   }
-  // open faces (D:R6, D:R22): what an outgoing wall link keeps in its slot; identity on every other cell
-  const bool touch = touches_open<BC>(p, c);
-  CellState st{A, ux, uy, uz, usq15, ic, z, -1, 0, 0.0, 0.0, 0.0, 1.0};
-  if (touch) classify_open_cell<BC>(st, p, c);
-  auto open = [&](auto BB, double v) -> double {
-    constexpr int b = decltype(BB)::value;
-    if constexpr (BC != BC_PERIODIC && Dir<Q, b>::s > 0) {
-      if (touch) return open_link<Q, EQ, BC, b, true>(v, p, c, st);
-    }
-    return v;
-  };
-  static_for<0, (Q + 1) / 2>([&](auto AA) {
-    constexpr int a = decltype(AA)::value;
-    using D = Dir<Q, a>;
-    if constexpr (a == D::opp) {
-      double gq = (om * D::t) * base;
-      if constexpr (FORCE) gq -= (k * D::t) * uF3;
-      store(IC<a>{}, fma(om1, (double)g[a], gq));
-    } else {
-      const double eu = edot<Q, a>(ux, uy, uz);
-      double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
-      double d = (3.0 * om * D::t) * (A * eu);
-      if constexpr (FORCE) {
-        const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
-        s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
-        d = fma(3.0 * k * D::t, eF, d);
+  // open faces (D:R6, D:R22): what an outgoing wall link keeps in its slot; identity on every other cell.  The cells
+  // next to such a face take their own copy of the relaxation loop, so that every other cell runs it without a test per
+  // direction (ncu, 256^3 cavity with fp32 storage: 624 -> instructions per cell as in the periodic kernel, and the hot
+  // path fits the instruction cache again).
+  auto relax = [&](auto OPEN, const CellState& st) {
+    auto open = [&](auto BB, double v) -> double {
+      constexpr int b = decltype(BB)::value;
+      if constexpr (decltype(OPEN)::value != 0 && BC != BC_PERIODIC && Dir<Q, b>::s > 0) return open_link<Q, EQ, BC, b, true>(v, p, c, st);
+      else return v;
+    };
+    static_for<0, (Q + 1) / 2>([&](auto AA) {
+      constexpr int a = decltype(AA)::value;
+      using D = Dir<Q, a>;
+      if constexpr (a == D::opp) {
+        double gq = (om * D::t) * base;
+        if constexpr (FORCE) gq -= (k * D::t) * uF3;
+        store(IC<a>{}, fma(om1, (double)g[a], gq));
+      } else {
+        const double eu = edot<Q, a>(ux, uy, uz);
+        double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
+        double d = (3.0 * om * D::t) * (A * eu);
+        if constexpr (FORCE) {
+          const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
+          s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
+          d = fma(3.0 * k * D::t, eF, d);
+        }
+        store(IC<a>{}, open(IC<a>{}, fma(om1, (double)g[a], s + d)));
+        store(IC<D::opp>{}, open(IC<D::opp>{}, fma(om1, (double)g[D::opp], s - d)));
       }
-      store(IC<a>{}, open(IC<a>{}, fma(om1, (double)g[a], s + d)));
-      store(IC<D::opp>{}, open(IC<D::opp>{}, fma(om1, (double)g[D::opp], s - d)));
+    });
+  };
+  CellState st{A, ux, uy, uz, usq15, ic, z, -1, 0, 0.0, 0.0, 0.0, 1.0};
+  if constexpr (BC != BC_PERIODIC) {
+    if (touches_open<BC>(p, c)) {
+      classify_open_cell<BC>(st, p, c);
+      relax(IC<1>{}, st);
+      return;
     }
-  });
+  }
+  relax(IC<0>{}, st);
 }
 
 // D:R24: true if the outgoing link B of this cell (node x + e_B) is resolved by an open face — it crosses a MOVING
@@ -834,31 +843,33 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, false, sizeof(ST)>) 
 }
 
 // fp32 storage, two cells per thread (S:§8f NEXT-1).  With half the bytes per cell the one-cell kernel above is bound by
-// issue slots, not by DRAM (ncu, 512^3 D3Q19: 576 instructions per cell, 165 of them integer address arithmetic, issue
-// 61 %, DRAM 81 %, and under the power cap of a sustained run the SM clock falls to ~1.6 GHz, where the issue rate
-// is the limit).  Here a thread owns the x-adjacent cells (x, x+1), x even, of a row that is uniform per block (the
-// block is bx x 1, y = blockIdx.y, z = blockIdx.z): the Q row bases are block-invariant and live in uniform registers,
-// the nine e_x = 0 streams are read and ALL Q streams are written as aligned 8-byte float2 accesses, and the address
-// arithmetic is paid once per pair.  Same arithmetic per cell as ab_cell (collide_shifted): bit-identical results.
-// A/B, BC_PERIODIC / BC_WALLS, even nx; everything else (link mask, z-slabs, odd nx) stays with the one-cell kernel.
-#ifndef LBM_F32X2_MB
-#define LBM_F32X2_MB 6
-#endif
+// instruction issue and by POWER, not by DRAM: ncu (512^3 D3Q19) shows 576 instructions per cell, 165 of them integer
+// address arithmetic; under the 1 kW cap of a sustained run the SM clock falls to ~1.6 GHz and the kernel to 0.91 of
+// the copy bandwidth although one launch at full clock is DRAM-bound.  Here a thread owns the x-adjacent cells
+// (x, x+1), x even, of a row that is uniform per block (the block is bx x 1, y = blockIdx.y, z = blockIdx.z): the Q
+// row bases are block-invariant (uniform datapath), the e_x = 0 streams are read and ALL streams are written as aligned
+// 8-byte vectors, and the address arithmetic — byte addresses as integers, one 64-bit add per access — is paid once
+// per pair: 400 instructions per cell.  Same arithmetic per cell as ab_cell (collide_shifted): bit-identical results.
+// A/B, D3Q19 / D2Q9, BC_PERIODIC / BC_WALLS, even nx; everything else (link mask, z-slabs, odd nx, and D3Q27, whose
+// pair needs 168 registers) stays with the one-cell kernel.
+// Measured, 512^3 D3Q19 sustained: 39.1 -> 42.0-42.3 GLUPS (0.98 of the copy bandwidth); one launch at full clock
+// (ncu) 3.01 ms = 44.6 GLUPS = 1.036, DRAM-bound — in the sustained run the power cap (sw_power_cap, ~1.65 GHz) is the
+// limit, i.e. energy per cell.  Tried and not kept: four cells per thread with 16-byte vectors and shuffles for the
+// shifted streams (306 instructions per cell, but 168 registers = 12 warps per SM and ptxas serialises the loads
+// through a few registers: 21-30 GLUPS); the collision in +- pair sums / differences (6 fp64 operations fewer per
+// cell, more spills: 41.0 vs 42.0 GLUPS).
+constexpr int kF32x2Threads = 128;  // D3Q19: 5 blocks per SM = 96 registers (44 B of spills; 128 registers, no spills: the same MLUPS)
 template <int Q, int EQ, int BC, bool FORCE>
-__global__ void __launch_bounds__(128, LBM_F32X2_MB) stream_collide_ab_f32x2(const float* __restrict__ src, float* __restrict__ dst, const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(kF32x2Threads, 5) stream_collide_ab_f32x2(const float* __restrict__ src, float* __restrict__ dst, const __grid_constant__ Params p) {
   static_assert(BC != BC_GEO, "the link-mask kernels keep one cell per thread");
+  typedef unsigned long long addr_t;
   const int x = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int y = blockIdx.y, z = blockIdx.z;
   if (x >= p.nx) return;
-  // Addresses = one per-thread pointer per z-plane (the cell pair's x in row 0 of that plane) + a block-uniform
-  // in-plane offset (direction row + y row, periodic wrap by conditional add as in Neigh; uniform datapath): one 64-bit
-  // add per direction and pair.  The odd element of a shifted stream sits one float before / after the pair, except
-  // in the two lanes of a row where the pull wraps around in x: a per-thread element offset dm / dp covers both.
+  // the thread's x in row 0 of each of the three z-planes + a block-uniform in-plane offset (direction row + y row;
+  // periodic wrap by conditional add as in Neigh)
   const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
   const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
-  // (byte addresses as integers: a plain 64-bit add per access; element indices would be scaled and added to the
-  // base one access at a time)
-  typedef unsigned long long addr_t;
   const long long oyb[3] = {4LL * ym * p.rs, 4LL * y * p.rs, 4LL * yp * p.rs};
   const addr_t xb = (addr_t)__cvta_generic_to_global(src) + 4ull * x;
   const addr_t P[3] = {xb + 4ull * (zm * p.zs), xb + 4ull * (z * p.zs), xb + 4ull * (zp * p.zs)};
