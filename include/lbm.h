@@ -193,6 +193,20 @@ int64_t lbm_time(lbm_handle h);
 /* Number of kernels this handle has launched so far (bookkeeping for benchmarks). */
 int64_t lbm_launch_count(lbm_handle h);
 
+/* Debug aids that work on the production kernels at any grid size (stand-ins for compute-sanitizer's memcheck /
+ * initcheck, which is not available on every pool).  Every device array a handle owns is allocated between two 64 KB
+ * guard zones filled with all-ones bytes (a NaN as fp64 and as fp32: a load that strays into a guard zone and is USED
+ * poisons the result like an uninitialised slot does).
+ *   lbm_debug_arm    rewrites the guard patterns and, poison != 0, fills every population / moment / scratch array of
+ *                    the handle with all-ones bytes (a NaN as fp64 and as fp32) — call it before lbm_init_equilibrium /
+ *                    lbm_set_populations: whatever the kernels then compute from a slot nobody wrote is NaN and shows up
+ *                    in diagnostics[7] and in every comparison (geometry, face profiles, slab counters are left alone).
+ *   lbm_debug_check  synchronises and returns the number of guard bytes that no longer hold the pattern: 0 = no store
+ *                    of the library's kernels landed within 64 KB outside an array; negative = LBM_E* error.
+ * Both synchronise the stream; neither costs anything between the two calls. */
+int lbm_debug_arm(lbm_handle h, int poison);
+int64_t lbm_debug_check(lbm_handle h);
+
 /* Small grids (every block of the step kernel resident on the device at once, e.g. 32^3 or the paper's 512 x 128
  * channel) are bound by the launch rate of one kernel per step; for them lbm_step(h, n) takes all n steps in ONE
  * cooperative launch of a persistent kernel (a grid-wide barrier separates the steps; same arithmetic per cell, same

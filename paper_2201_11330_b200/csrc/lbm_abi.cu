@@ -33,6 +33,9 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 constexpr int kReduceBlocks = 148 * 8;  // one wave of 256-thread blocks on 148 SMs
+constexpr size_t kGuard = 64u << 10;    // bytes of guard zone before and after every device array of a handle
+constexpr int kGuardByte = 0xFF;        // all-ones: a NaN as fp64 / fp32, so that an out-of-bounds READ that is used shows up too
+constexpr int kMaxOwned = 24;
 constexpr int kMaxChunks = 16;          // z-chunks of the host entry points (copy of chunk k+1 overlaps the kernel of chunk k)
 constexpr size_t kChunkBytes = 64u << 20;  // ... each at least this many bytes of rho, u (smaller grids: one chunk)
 
@@ -61,6 +64,10 @@ struct lbm_handle_s {
   double* diag_pinned;  // 8, host
   void* scratch;
   size_t scratch_bytes;
+  // debug aids (lbm_debug_arm / lbm_debug_check): every device array is allocated with a guard zone on both sides
+  struct { void* p; size_t bytes; bool floating; } owned[kMaxOwned];
+  int n_owned;
+  unsigned long long* guard_bad;     // device counter of guard bytes that lost their pattern
   cudaStream_t copy_stream;          // host entry points: the copies run here, the kernels on `stream` (created on first use)
   cudaEvent_t chunk_ev[kMaxChunks];  // chunk k has landed (init) / has been computed (moments)
   cudaEvent_t fence_ev;              // orders the two streams at the start and at the end of a host call
@@ -224,15 +231,51 @@ void do_import(lbm_handle_s* h, const double* in, int dst_idx) {
   ++h->launches;
 }
 
+// Device arrays of a handle: `bytes` usable bytes between two guard zones filled with kGuardByte (lbm_debug_check counts
+// the guard bytes that changed: an out-of-bounds store of the library's kernels that lands within 64 KB of an array).
+// floating: holds populations / moments (what lbm_debug_arm may poison with NaNs).
+cudaError_t gmalloc(lbm_handle_s* h, void** out, size_t bytes, bool floating) {
+  *out = nullptr;
+  if (h->n_owned >= kMaxOwned) return cudaErrorMemoryAllocation;
+  char* raw = nullptr;
+  cudaError_t e = cudaMalloc((void**)&raw, bytes + 2 * kGuard);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(raw, kGuardByte, kGuard, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(raw + kGuard + bytes, kGuardByte, kGuard, h->stream);
+  if (e != cudaSuccess) { cudaFree(raw); return e; }
+  *out = raw + kGuard;
+  h->owned[h->n_owned].p = *out;
+  h->owned[h->n_owned].bytes = bytes;
+  h->owned[h->n_owned].floating = floating;
+  ++h->n_owned;
+  return cudaSuccess;
+}
+void gfree(lbm_handle_s* h, void* p) {
+  if (!p) return;
+  for (int k = 0; k < h->n_owned; ++k)
+    if (h->owned[k].p == p) {
+      h->owned[k] = h->owned[h->n_owned - 1];
+      --h->n_owned;
+      break;
+    }
+  cudaFree((char*)p - kGuard);
+}
+
+__global__ void guard_count_kernel(const unsigned char* __restrict__ g, size_t n, unsigned long long* bad) {
+  unsigned long long c = 0;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) c += g[i] != kGuardByte;
+  if (c) atomicAdd(bad, c);
+}
+
 int ensure_scratch(lbm_handle_s* h, size_t bytes) {
   if (h->scratch_bytes >= bytes) return LBM_OK;
   if (h->scratch) {
     cudaStreamSynchronize(h->stream);
-    cudaFree(h->scratch);
+    gfree(h, h->scratch);
     h->scratch = nullptr;
     h->scratch_bytes = 0;
   }
-  cudaError_t e = cudaMalloc(&h->scratch, bytes);
+  cudaError_t e = gmalloc(h, &h->scratch, bytes, true);
   if (e != cudaSuccess) {
     cudaGetLastError();
     return fail(LBM_ENOMEM, "out of device memory for the scratch buffer");
@@ -358,9 +401,9 @@ int copy_chunk(lbm_handle_s* h, double* dev_rho, double* dev_u, double* host_rho
 }
 
 void free_geometry(lbm_handle_s* h) {
-  if (h->geo) cudaFree(h->geo);
-  if (h->active) cudaFree(h->active);
-  if (h->links) cudaFree(h->links);
+  gfree(h, h->geo);
+  gfree(h, h->active);
+  gfree(h, h->links);
   h->geo = h->active = nullptr;
   h->links = nullptr;
   h->has_geo = false;
@@ -371,9 +414,9 @@ void free_geometry(lbm_handle_s* h) {
 
 int alloc_geometry(lbm_handle_s* h) {
   if (h->geo) return LBM_OK;
-  cudaError_t e = cudaMalloc((void**)&h->geo, (size_t)h->N);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&h->active, (size_t)h->N);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&h->links, (size_t)h->N * sizeof(uint32_t));
+  cudaError_t e = gmalloc(h, (void**)&h->geo, (size_t)h->N, false);
+  if (e == cudaSuccess) e = gmalloc(h, (void**)&h->active, (size_t)h->N, false);
+  if (e == cudaSuccess) e = gmalloc(h, (void**)&h->links, (size_t)h->N * sizeof(uint32_t), false);
   if (e != cudaSuccess) {
     cudaGetLastError();
     free_geometry(h);
@@ -404,7 +447,11 @@ int do_set_geometry(lbm_handle_s* h, const uint8_t* geo_dev, int wall_model) {
   LBM_Q_CALL(h, launch_geometry, c, geo_dev, h->geo, h->active, h->links, h->p.nodal);
   h->launches += 2;
   h->stepped = false;
-  return check_launch("lbm_set_geometry");
+  int rc = check_launch("lbm_set_geometry");
+  if (rc) return rc;
+  // the caller's mask has been read when the call returns (it may be a temporary)
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBM_OK;
 }
 
 }  // namespace
@@ -544,12 +591,13 @@ static lbm_handle create_impl(int nx, int ny, int nz, int lattice, double tau, c
 
   const int nbuf = scheme == LBM_SCHEME_AB ? 2 : 1;
   cudaError_t e = cudaSuccess;
-  for (int b = 0; b < nbuf && e == cudaSuccess; ++b) e = cudaMalloc(&h->buf[b], h->buf_bytes());
-  if (e == cudaSuccess) e = cudaMalloc((void**)&h->partials, (size_t)kMaxChunks * kReduceBlocks * kDiag * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&h->diag_dev, kDiag * sizeof(double));
+  for (int b = 0; b < nbuf && e == cudaSuccess; ++b) e = gmalloc(h, &h->buf[b], h->buf_bytes(), true);
+  if (e == cudaSuccess) e = gmalloc(h, (void**)&h->partials, (size_t)kMaxChunks * kReduceBlocks * kDiag * sizeof(double), true);
+  if (e == cudaSuccess) e = gmalloc(h, (void**)&h->diag_dev, kDiag * sizeof(double), true);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->guard_bad, sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&h->diag_pinned, kDiag * sizeof(double));
   if (e == cudaSuccess && slab) {
-    e = cudaMalloc((void**)&h->flags, 2 * sizeof(uint32_t));
+    e = gmalloc(h, (void**)&h->flags, 2 * sizeof(uint32_t), false);
     if (e == cudaSuccess) e = cudaMemset(h->flags, 0, 2 * sizeof(uint32_t));
   }
   if (e != cudaSuccess) {
@@ -609,7 +657,8 @@ int lbm_slab_export(lbm_handle h, lbm_slab_peer_t* out) {
   uint8_t* dsts[3] = {out->ipc_buf[0], out->ipc_buf[1], out->ipc_flags};
   for (int k = 0; k < 3; ++k) {
     // without IPC support the descriptor still serves slabs of the same process
-    if (cudaIpcGetMemHandle(&ih, ptrs[k]) == cudaSuccess) std::memcpy(dsts[k], &ih, sizeof(ih));
+    // (the handle names the whole allocation, guard zone included: map_peer adds kGuard to what it opens)
+    if (cudaIpcGetMemHandle(&ih, (char*)ptrs[k] - kGuard) == cudaSuccess) std::memcpy(dsts[k], &ih, sizeof(ih));
     else cudaGetLastError();
   }
   return LBM_OK;
@@ -638,7 +687,7 @@ int map_peer(lbm_handle_s* h, const lbm_slab_peer_t* d, uint64_t addr, const uin
   cudaError_t e = cudaIpcOpenMemHandle(&ptr, ih, cudaIpcMemLazyEnablePeerAccess);
   if (e != cudaSuccess) return cuda_fail(e, "cudaIpcOpenMemHandle");
   if (h->n_ipc_opened < 6) h->ipc_opened[h->n_ipc_opened++] = ptr;
-  *out = ptr;
+  *out = (char*)ptr + kGuard;
   return LBM_OK;
 }
 
@@ -707,13 +756,13 @@ void lbm_destroy(lbm_handle h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
   if (h->slab) close_peers(h);
-  if (h->flags) cudaFree(h->flags);
-  for (int b = 0; b < 2; ++b)
-    if (h->buf[b]) cudaFree(h->buf[b]);
-  if (h->partials) cudaFree(h->partials);
-  if (h->diag_dev) cudaFree(h->diag_dev);
+  gfree(h, h->flags);
+  for (int b = 0; b < 2; ++b) gfree(h, h->buf[b]);
+  gfree(h, h->partials);
+  gfree(h, h->diag_dev);
+  if (h->guard_bad) cudaFree(h->guard_bad);
   if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
-  if (h->scratch) cudaFree(h->scratch);
+  gfree(h, h->scratch);
   if (h->copy_stream) {
     cudaStreamSynchronize(h->copy_stream);
     for (int k = 0; k < kMaxChunks; ++k) cudaEventDestroy(h->chunk_ev[k]);
@@ -721,7 +770,7 @@ void lbm_destroy(lbm_handle h) {
     cudaStreamDestroy(h->copy_stream);
   }
   for (int k = 0; k < 6; ++k)
-    if (h->p.face_prof[k]) cudaFree((void*)h->p.face_prof[k]);
+    gfree(h, (void*)h->p.face_prof[k]);
   free_geometry(h);
   cudaGetLastError();
   delete h;
@@ -741,14 +790,14 @@ static int set_face_velocity_impl(lbm_handle h, int face, const double* u, cudaM
   if (owns && h->p.kind[face] != LBM_FACE_MOVING) return fail(LBM_EINVAL, std::string(who) + ": the face is not LBM_FACE_MOVING");
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   if (!u) {
-    if (h->p.face_prof[face]) cudaFree((void*)h->p.face_prof[face]);
+    gfree(h, (void*)h->p.face_prof[face]);
     h->p.face_prof[face] = nullptr;
     return LBM_OK;
   }
   const size_t bytes = (size_t)face_cells(h, face) * 3 * sizeof(double);
   double* dst = (double*)h->p.face_prof[face];
   if (!dst) {
-    if (cudaMalloc((void**)&dst, bytes) != cudaSuccess) {
+    if (gmalloc(h, (void**)&dst, bytes, false) != cudaSuccess) {
       cudaGetLastError();
       return fail(LBM_ENOMEM, std::string(who) + ": out of device memory for the face profile");
     }
@@ -964,6 +1013,37 @@ int lbm_set_populations(lbm_handle h, const double* f) {
   h->phase = 0;
   h->stepped = false;
   return check_launch("lbm_set_populations");
+}
+
+int lbm_debug_arm(lbm_handle h, int poison) {
+  if (!h) return fail(LBM_EINVAL, "lbm_debug_arm: NULL handle");
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < h->n_owned; ++k) {
+    char* p = (char*)h->owned[k].p;
+    CUDA_TRY(cudaMemsetAsync(p - kGuard, kGuardByte, kGuard, h->stream));
+    CUDA_TRY(cudaMemsetAsync(p + h->owned[k].bytes, kGuardByte, kGuard, h->stream));
+    // all-ones bytes are a NaN as fp64 and as fp32: whatever is computed from a slot nobody wrote shows up as a
+    // non-finite cell (diagnostics[7]) and in every comparison
+    if (poison && h->owned[k].floating) CUDA_TRY(cudaMemsetAsync(p, 0xFF, h->owned[k].bytes, h->stream));
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (poison) h->stepped = false;
+  return LBM_OK;
+}
+
+int64_t lbm_debug_check(lbm_handle h) {
+  if (!h) return fail(LBM_EINVAL, "lbm_debug_check: NULL handle");
+  if (cudaMemsetAsync(h->guard_bad, 0, sizeof(unsigned long long), h->stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), "lbm_debug_check");
+  for (int k = 0; k < h->n_owned; ++k) {
+    const unsigned char* p = (const unsigned char*)h->owned[k].p;
+    guard_count_kernel<<<8, 256, 0, h->stream>>>(p - kGuard, kGuard, h->guard_bad);
+    guard_count_kernel<<<8, 256, 0, h->stream>>>(p + h->owned[k].bytes, kGuard, h->guard_bad);
+  }
+  unsigned long long bad = 0;
+  cudaError_t e = cudaMemcpyAsync(&bad, h->guard_bad, sizeof(bad), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(e, "lbm_debug_check");
+  return (int64_t)bad;
 }
 
 int64_t lbm_time(lbm_handle h) { return h ? h->time : -1; }

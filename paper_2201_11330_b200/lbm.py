@@ -32,6 +32,7 @@ SYMBOLS = (
     "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
     "lbm_set_face_velocity", "lbm_set_face_velocity_host", "lbm_set_face_density",
     "lbm_create_slab", "lbm_slab_export", "lbm_slab_connect", "lbm_slab_set_sync",
+    "lbm_debug_arm", "lbm_debug_check",
 )
 
 
@@ -126,6 +127,10 @@ def load():
     lib.lbm_slab_connect.argtypes = [vp, C.POINTER(lbm_slab_peer_t), C.POINTER(lbm_slab_peer_t)]
     lib.lbm_slab_set_sync.restype = i32
     lib.lbm_slab_set_sync.argtypes = [vp, i32]
+    lib.lbm_debug_arm.restype = i32
+    lib.lbm_debug_arm.argtypes = [vp, i32]
+    lib.lbm_debug_check.restype = i64
+    lib.lbm_debug_check.argtypes = [vp]
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_last_error.argtypes = []
     _lib = lib
@@ -292,6 +297,17 @@ def lbm_set_block(h, bx, by):
     _check(load().lbm_set_block(h, int(bx), int(by)))
 
 
+def lbm_debug_arm(h, poison=True):
+    _check(load().lbm_debug_arm(h, 1 if poison else 0))
+
+
+def lbm_debug_check(h) -> int:
+    n = int(load().lbm_debug_check(h))
+    if n < 0:
+        raise LBMError(n, lbm_last_error())
+    return n
+
+
 def lbm_set_persistent(h, on):
     _check(load().lbm_set_persistent(h, 1 if on else 0))
 
@@ -360,7 +376,9 @@ class Solver:
         lbm_set_face_density(self.h, rho6)
 
     def init_equilibrium(self, rho=None, u=None):
+        self._before()
         lbm_init_equilibrium(self.h, rho, u)
+        self._after(rho, u)
 
     def init_equilibrium_host(self, rho=None, u=None):
         lbm_init_equilibrium_host(self.h, rho, u)
@@ -368,11 +386,35 @@ class Solver:
     def step(self, n=1):
         lbm_step(self.h, n)
 
+    # The library works on the handle's stream; tensors handed over or returned here belong to torch's current stream.
+    # _before / _after order the two (no-ops when they are the same stream) so that a temporary is not recycled while a
+    # kernel still reads it and a result is not read before it has been written.
+    def _before(self):
+        import torch
+        cur = torch.cuda.current_stream()
+        if self.torch_stream is not None:
+            self.torch_stream.wait_stream(cur)
+        elif cur != torch.cuda.default_stream():
+            cur.synchronize()  # the handle runs on the default stream, torch on another one
+
+    def _after(self, *tensors):
+        import torch
+        cur = torch.cuda.current_stream()
+        if self.torch_stream is not None:
+            cur.wait_stream(self.torch_stream)
+            for t in tensors:
+                if t is not None:
+                    t.record_stream(self.torch_stream)
+        elif cur != torch.cuda.default_stream():
+            torch.cuda.default_stream().synchronize()
+
     def moments(self, fields=True, diagnostics=True):
         import torch
         rho = torch.empty(self.N, dtype=torch.float64, device="cuda") if fields else None
         u = torch.empty(3 * self.N, dtype=torch.float64, device="cuda") if fields else None
+        self._before()
         diag = lbm_moments(self.h, rho, u, diagnostics)
+        self._after(rho, u)
         return rho, (None if u is None else u.view(3, self.N)), diag
 
     def diagnostics(self):
@@ -381,11 +423,16 @@ class Solver:
     def get_populations(self, out=None):
         import torch
         f = torch.empty(self.Q * self.N, dtype=torch.float64, device="cuda") if out is None else out
+        self._before()
         lbm_get_populations(self.h, f)
+        self._after(f)
         return f.view(self.Q, self.N)
 
     def set_populations(self, f):
-        lbm_set_populations(self.h, f.contiguous().view(-1))
+        f = f.contiguous().view(-1)
+        self._before()
+        lbm_set_populations(self.h, f)
+        self._after(f)
 
     @property
     def time(self):
@@ -400,3 +447,9 @@ class Solver:
 
     def set_persistent(self, on):
         lbm_set_persistent(self.h, on)
+
+    def debug_arm(self, poison=True):
+        lbm_debug_arm(self.h, poison)
+
+    def debug_check(self) -> int:
+        return lbm_debug_check(self.h)

@@ -90,6 +90,23 @@ def test_invalid_arguments_fail_before_cuda(lib):
     assert lib.lbm_lattice(5, e, (C.c_double * 1)()) == lbm.LBM_EINVAL
 
 
+def test_size_limits_are_checked_before_cuda(lib):
+    """Cell indices are 32-bit: nx*ny*nz >= 2^31 is refused (LBM_EUNSUPPORTED) before any CUDA call.  In-plane storage
+    offsets are 32-bit too, but a plane with Q*nx*ny >= 2^31 (D2Q9 16384^2) is NOT refused: it is stored as a plain
+    structure of arrays (include/lbm.h LBM_LAYOUT_ROWS; the GPU test test_large_plane_beyond_32bit_row_offsets_equals_its_tile
+    runs it) — without a device the call gets as far as the allocation and fails there."""
+    with pytest.raises(lbm.LBMError) as ei:
+        lbm.lbm_create(2048, 1024, 1024, 19, 0.8)
+    assert ei.value.code == lbm.LBM_EUNSUPPORTED or "2^31" in str(ei.value)
+    import torch
+    if not torch.cuda.is_available():
+        with pytest.raises(lbm.LBMError) as ei:
+            lbm.lbm_create(16384, 16384, 1, 9, 0.8)
+        assert "2^31" not in str(ei.value) and "must be" not in str(ei.value)  # an allocation / CUDA error, not a refusal
+    assert lib.lbm_debug_arm(None, 1) == lbm.LBM_EINVAL
+    assert lib.lbm_debug_check(None) == lbm.LBM_EINVAL
+
+
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):
     monkeypatch.setattr(lbm, "_lib", None)
     monkeypatch.setattr(lbm, "LIB_PATH", str(tmp_path / "nope.so"))

@@ -126,6 +126,7 @@ def test_config3_tgv512_every_cell_full_length_chain(lbm, scheme):
     assert err <= 1e-12, err
     N = n * k
     big = lbm.Solver(N, N, N, 19, w.tau, scheme=sch)
+    big.debug_arm(poison=True)  # NaNs everywhere before the initialisation; guard zones checked after the run
     rho_b = rho_s.view(n, n, n).repeat(k, k, k).reshape(-1)
     u_b = u_s.view(3, n, n, n).repeat(1, k, k, k).reshape(-1)
     big.init_equilibrium(rho_b, u_b)
@@ -133,6 +134,7 @@ def test_config3_tgv512_every_cell_full_length_chain(lbm, scheme):
     big.step(steps)
     d_big = big.diagnostics()
     f_big = big.get_populations()
+    assert big.debug_check() == 0
     big.close()
     same = f_big.view(19, k, n, k, n, k, n) == f_small.view(19, 1, n, 1, n, 1, n)
     assert bool(same.all()), f"{int((~same).sum())} of {same.numel()} populations differ from the 128^3 tile"

@@ -529,6 +529,38 @@ def test_large_box_equals_its_periodic_tile(lbm, scheme):
 
 
 @pytest.mark.parametrize("scheme", ["ab", "aa"])
+def test_large_plane_beyond_32bit_row_offsets_equals_its_tile(lbm, scheme):
+    """D2Q9 16384 x 16384 x 1: Q*nx*ny = 2.4e9 >= 2^31, so the row-interleaved layout's 32-bit in-plane offsets x + y*(Q*nx)
+    would overflow; lbm_create stores such a grid as a plain structure of arrays instead (include/lbm.h LBM_LAYOUT_ROWS).
+    Started from a 2048^2 Taylor-Green field tiled 8 x 8 it must reproduce the small box tile by tile, bit for bit, and
+    leave the guard zones around its buffers intact."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80e9:
+        pytest.skip("needs 80 GB of free device memory")
+    n, k, steps = 2048, 8, 5
+    rho, u = inputs.taylor_green_2d(n, n, 1, 0.03)
+    rho_s, u_s = dev(rho), dev(u.reshape(-1))
+    sch = dict(schemes(lbm))[scheme]
+    s = lbm.Solver(n, n, 1, 9, 0.7, scheme=sch)
+    s.init_equilibrium(rho_s, u_s)
+    s.step(steps)
+    r_small, u_small, d_small = s.moments()
+    r_small, u_small = r_small.clone().view(n, n), u_small.clone().view(3, n, n)
+    s.close()
+    N = n * k
+    big = lbm.Solver(N, N, 1, 9, 0.7, scheme=sch)
+    big.debug_arm(poison=True)
+    big.init_equilibrium(rho_s.view(n, n).repeat(k, k).reshape(-1), u_s.view(3, n, n).repeat(1, k, k).reshape(-1))
+    big.step(steps)
+    r_big, u_big, d_big = big.moments()
+    assert big.debug_check() == 0
+    big.close()
+    assert bool((r_big.view(k, n, k, n) == r_small.view(1, n, 1, n)).all())
+    assert bool((u_big.view(3, k, n, k, n) == u_small.view(3, 1, n, 1, n)).all())
+    assert d_big[7] == 0 and d_big[5] == d_small[5] and d_big[6] == d_small[6]
+
+
+@pytest.mark.parametrize("scheme", ["ab", "aa"])
 def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
     """lbm_step(n) on a small grid runs in ONE cooperative launch of the persistent kernel (all n steps, a grid-wide
     barrier between them); with lbm_set_persistent(0) it is n launches.  Same cell code: identical bits — periodic,

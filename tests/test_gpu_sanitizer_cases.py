@@ -7,8 +7,12 @@ that is run under compute-sanitizer (SURVEY.md section 4 T4, section 5 "race det
     compute-sanitizer --tool synccheck --error-exitcode 1 python -m pytest tests/test_gpu_sanitizer_cases.py -m gpu -q -x
 
 (one tool per GPU-box call; PYTORCH_NO_CUDA_MEMORY_CACHING=1 gives every tensor its own allocation so that memcheck sees
-the bounds of the caller's arrays too).  Results: profiles/sanitizer_r02.md.  Without the sanitizer it is an ordinary
-`-m gpu` parity test file (a few seconds).
+the bounds of the caller's arrays too).  On the pool this was written on compute-sanitizer is closed (profiles/sanitizer_r02.md
+has the answer it gives), so every case here also runs the library's own stand-ins (include/lbm.h "Debug aids"):
+lbm_debug_arm(poison) fills every population / scratch array with NaNs before the initialisation — a value computed from
+a slot nobody wrote fails the comparison with the oracle — and lbm_debug_check verifies the guard zones around every
+device array afterwards (an out-of-bounds store).  Two negative tests prove that both alarms ring.  Without a sanitizer
+it is an ordinary `-m gpu` parity test file (a few seconds).
 
 Covered: stream_collide_ab (periodic / walls / link mask, forcing, fp32 storage, mirror planes), stream_collide_aa_even /
 _odd, stream_collide_ab_persistent, stream_collide_aa_persistent, init_equilibrium (device and host entry points),
@@ -75,6 +79,7 @@ def run_single(lbm, w, scheme, store, persistent, host_entry):
     uf = np.ascontiguousarray(u.reshape(-1))
     s = lbm.Solver.from_workload(w, scheme=scheme, store=store)
     s.set_persistent(persistent)
+    s.debug_arm(poison=True)  # NaNs in every population / scratch array: a slot used before it is written shows up below
     if host_entry:
         s.init_equilibrium_host(torch.from_numpy(rho), torch.from_numpy(uf))
     else:
@@ -95,6 +100,7 @@ def run_single(lbm, w, scheme, store, persistent, host_entry):
     s.step(1)
     f1 = s.get_populations().cpu().numpy()
     torch.cuda.synchronize()
+    assert s.debug_check() == 0, "a kernel stored outside an array (guard zone damaged)"
     s.close()
     return f0, f, r, uu, d, F, f1
 
@@ -161,11 +167,15 @@ def test_slabs_in_one_process(mods, name, nslabs, store):
     Fo = o.boundary_force() if w.has_geometry else None
     o.close()
     g = slabs.SlabGroup(w, nslabs, store=lbm.LBM_STORE_F32 if store == "f32" else lbm.LBM_STORE_F64)
+    for sl in g.slabs:
+        lbm.lbm_debug_arm(sl.h, True)
     g.init_equilibrium()
     g.step(w.steps)
     f = g.get_populations().cpu().numpy()
     d = g.diagnostics()
     F = g.boundary_force() if w.has_geometry else None
+    g.synchronize()
+    assert [lbm.lbm_debug_check(sl.h) for sl in g.slabs] == [0] * nslabs
     g.close()
     if store == "f64":
         assert np.abs(f - ref).max() <= TOL
@@ -174,3 +184,39 @@ def test_slabs_in_one_process(mods, name, nslabs, store):
     else:
         assert (np.abs(f - ref) / np.abs(ref).max(axis=1, keepdims=True)).max() <= 2e-5
     assert d[7] == 0
+
+
+def test_guard_zones_detect_an_out_of_bounds_store(mods):
+    """The alarm rings: one byte written just outside a population buffer (its address comes from the slab descriptor)
+    is counted by lbm_debug_check; nothing is counted before, nothing after re-arming."""
+    lbm, _ = mods
+    runtime = pytest.importorskip("cuda.bindings.runtime")
+    h = lbm.lbm_create_slab(16, 8, 4, 0, 4, 19, 0.8)
+    try:
+        assert lbm.lbm_debug_check(h) == 0
+        d = lbm.lbm_slab_export(h)
+        nbytes = 19 * 16 * 8 * 6 * 8
+        for addr in (int(d.buf[0]) - 1, int(d.buf[1]) + nbytes):  # one byte before buffer 0, one byte after buffer 1
+            (err,) = runtime.cudaMemset(addr, 0, 1)
+            assert int(err) == 0
+        torch.cuda.synchronize()
+        assert lbm.lbm_debug_check(h) == 2
+        lbm.lbm_debug_arm(h, False)
+        assert lbm.lbm_debug_check(h) == 0
+    finally:
+        lbm.lbm_destroy(h)
+
+
+def test_poison_makes_an_uninitialised_read_visible(mods):
+    """The alarm rings: poisoned and NOT initialised, every cell reports non-finite moments; after the initialisation
+    (which must overwrite every slot a step reads) none does, through steps of both schemes."""
+    lbm, _ = mods
+    for scheme in (lbm.LBM_SCHEME_AB, lbm.LBM_SCHEME_AA):
+        s = lbm.Solver(12, 10, 8, 19, 0.8, scheme=scheme, face_kind=[B, B, P, P, B, M], face_u=[[0, 0, 0]] * 5 + [[0.05, 0, 0]])
+        s.debug_arm(poison=True)
+        assert s.diagnostics()[7] == 12 * 10 * 8
+        s.init_equilibrium()
+        s.set_persistent(0)
+        s.step(3)
+        assert s.diagnostics()[7] == 0
+        s.close()
