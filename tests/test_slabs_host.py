@@ -77,7 +77,8 @@ def test_combine_diagnostics():
 def test_descriptor_struct_matches_the_header():
     """lbm_slab_peer_t in the binding has the size and field order of include/lbm.h (plain bytes cross processes)."""
     import ctypes as C
-    assert C.sizeof(lbm.lbm_slab_peer_t) == 2 * 8 + 8 + 8 + 4 + 4 + 8 + 2 * 64 + 64
+    # buf[2], flags, plane_stride | nz_local, device | pid | Q, elem_bytes, layout_soa, reserved | stream | ipc handles
+    assert C.sizeof(lbm.lbm_slab_peer_t) == 2 * 8 + 8 + 8 + 4 + 4 + 8 + 4 * 4 + 8 + 2 * 64 + 64
     d = lbm.lbm_slab_peer_t()
     d.buf[0], d.buf[1], d.flags, d.plane_stride, d.nz_local, d.device, d.pid = 1, 2, 3, 4, 5, 6, 7
     back = lbm.lbm_slab_peer_t.from_buffer_copy(bytes(d))
