@@ -213,6 +213,15 @@ int64_t lbm_debug_check(lbm_handle h);
  * results bit for bit).  on = 0 switches that off (one launch per step, as for every larger grid); default on. */
 int lbm_set_persistent(lbm_handle h, int on);
 
+/* Two time steps per pass through HBM (Eq. 7 applied twice; the same collision, Eq. 6, in between).  For a
+ * whole box (no z-slab) of D3Q19 populations stored as fp64 under LBM_SCHEME_AB — periodic, BOUNCE, MOVING and PRESSURE
+ * faces; no solid mask (lbm_set_geometry) and no SYMMETRY face — lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
+ * runs step t+1 from there, so that every population is read from HBM once and written once per TWO steps.  Same
+ * arithmetic per cell, same results bit for bit as single steps; an odd n ends with one single step.  on = 0 switches
+ * it off (one pass per step, as for every other variant); default on.  Grids small enough for the persistent kernel
+ * (lbm_set_persistent) keep using that one. */
+int lbm_set_two_step(lbm_handle h, int on);
+
 /* Tuning knob for measurements: CUDA block shape (threads along x, along y) of the
  * stream-collide kernel; 0,0 restores the default.  bx*by must be <= 256 and a multiple of 32. */
 int lbm_set_block(lbm_handle h, int bx, int by);

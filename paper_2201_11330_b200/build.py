@@ -20,8 +20,9 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 DEPS = ["lbm_abi.cu", "lbm_inst.cu", "lbm_kernels.cuh", "lbm_launch.cuh", os.path.join(ROOT, "include", "lbm.h")]
 LATTICES = (9, 19, 27)
-PARTS = (0, 1, 2, 3, 4, 5, 6, 7, 8, 9)  # A/B step, AA even, AA odd, export/import/init/geometry, moments/force, A/B slab step,
-                                  # A/B step with SYMMETRY faces, A/B slab step with SYMMETRY faces, persistent A/B kernel, persistent AA kernel
+PARTS = (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10)  # A/B step, AA even, AA odd, export/import/init/geometry, moments/force, A/B slab step,
+                                  # A/B step with SYMMETRY faces, A/B slab step with SYMMETRY faces, persistent A/B kernel, persistent AA kernel,
+                                  # A/B two steps per pass
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

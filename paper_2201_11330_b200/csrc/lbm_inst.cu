@@ -3,12 +3,12 @@
 //   LBM_PART 0 A/B step   1 AA even step   2 AA odd step   3 export/import/init/geometry   4 moments/force
 //            5 A/B step of a z-slab (fused halo push)   6 A/B step with SYMMETRY faces (link mask + mirror links)
 //            7 A/B step of a z-slab with SYMMETRY faces   8 persistent A/B kernel (all steps of a call in one launch)
-//            9 persistent in-place AA kernel
+//            9 persistent in-place AA kernel   10 A/B, two steps per pass (stream_collide_ab2)
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
-#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..9"
+#error "compile with -DLBM_Q=9|19|27 -DLBM_PART=0..10"
 #endif
 
 namespace lbm {
@@ -206,6 +206,65 @@ void launch_step_ab_slab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
     });
   });
 }
+#elif LBM_PART == 10
+template <>
+bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst) {
+  // D3Q19, fp64 storage, all faces periodic, whole box (measured: 512^3 22.5 -> 33.4 GLUPS).  D2Q9 has no z to march
+  // along; D3Q27 needs 81 population planes of shared memory per tile cell and is left to the one-step kernel.
+  if constexpr (Q_ != 19) {
+    return false;
+  } else {
+    constexpr int TX = 32, TY = 8;
+    if (c.bc == BC_GEO || c.f32 || c.p.slab || c.p.nx < TX || c.p.ny < TY || c.p.nz < 4) return false;
+    bool ok = true;
+    dispatch_eq(c, [&](auto eq) {
+      dispatch_force(c, [&](auto force) {
+       dispatch_bc(c, [&](auto bc) {
+        if constexpr (decltype(bc)::value == BC_GEO) {
+          ok = false;
+          return;
+        } else {
+        using T = Ab2Tile<Q_, TX, TY, true, decltype(bc)::value == BC_WALLS>;
+        auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, TX, TY, 1, true, true>;
+        static int resident_on[64] = {0};  // per device: blocks of this instantiation resident at once (0 = not asked yet)
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+          cudaGetLastError();
+          ok = false;
+          return;
+        }
+        if (resident_on[dev] == 0) {
+          int sms = 0, per_sm = 0;
+          if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
+              cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+              cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, T::THREADS, T::SMEM_BYTES) != cudaSuccess || per_sm < 1) {
+            cudaGetLastError();
+            resident_on[dev] = -1;
+          } else {
+            resident_on[dev] = per_sm * sms;
+          }
+        }
+        const int resident = resident_on[dev];
+        if (resident < 0) {
+          ok = false;
+          return;
+        }
+        // z-chunks: enough blocks for ~16 waves (the tail of the last wave stays below a few percent), chunks of at least
+        // 16 planes (every chunk runs stage 1 on two planes more than it stores)
+        const long long tiles = (long long)((c.p.nx + TX - 1) / TX) * ((c.p.ny + TY - 1) / TY);
+        long long chunks = (16LL * resident + tiles - 1) / tiles;
+        if (chunks > c.p.nz / 16) chunks = c.p.nz / 16;
+        if (chunks < 1) chunks = 1;
+        const int zchunk = (int)((c.p.nz + chunks - 1) / chunks);
+        const dim3 grid((c.p.nx + TX - 1) / TX, (c.p.ny + TY - 1) / TY, (c.p.nz + zchunk - 1) / zchunk);
+        kernel<<<grid, T::THREADS, T::SMEM_BYTES, c.stream>>>((const double*)src, (double*)dst, zchunk, c.p);
+        }
+       });
+      });
+    });
+    return ok;
+  }
+}
 #elif LBM_PART == 1
 template <>
 void launch_step_aa_even<Q_>(const Ctx& c, void* buf) {
@@ -218,10 +277,31 @@ void launch_step_aa_even<Q_>(const Ctx& c, void* buf) {
 #elif LBM_PART == 2
 template <>
 void launch_step_aa_odd<Q_>(const Ctx& c, void* buf) {
-  dispatch_step(c, [&](auto eq, auto bc, auto force, auto st) {
-    using ST = decltype(st);
-    stream_collide_aa_odd<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, ST>
-        <<<c.grid, c.block, 0, c.stream>>>((ST*)buf, c.p);
+  if (c.bc != BC_GEO) {
+    // one grid row per block (stream_collide_aa_odd_row): the row bases of all Q slots are block-uniform
+    int bx = 32;
+    while (bx < 256 && bx < c.p.nx) bx *= 2;
+    const dim3 block(bx, 1, 1), grid((c.p.nx + bx - 1) / bx, c.p.ny, c.p.nz);
+    dispatch_eq(c, [&](auto eq) {
+      dispatch_force(c, [&](auto force) {
+        dispatch_storage(c, [&](auto st) {
+          using ST = decltype(st);
+          if (c.bc == BC_WALLS)
+            stream_collide_aa_odd_row<Q_, decltype(eq)::value, BC_WALLS, decltype(force)::value != 0, ST><<<grid, block, 0, c.stream>>>((ST*)buf, c.p);
+          else
+            stream_collide_aa_odd_row<Q_, decltype(eq)::value, BC_PERIODIC, decltype(force)::value != 0, ST><<<grid, block, 0, c.stream>>>((ST*)buf, c.p);
+        });
+      });
+    });
+    return;
+  }
+  dispatch_eq(c, [&](auto eq) {
+    dispatch_force(c, [&](auto force) {
+      dispatch_storage(c, [&](auto st) {
+        using ST = decltype(st);
+        stream_collide_aa_odd<Q_, decltype(eq)::value, BC_GEO, decltype(force)::value != 0, ST><<<c.grid, c.block, 0, c.stream>>>((ST*)buf, c.p);
+      });
+    });
   });
 }
 #elif LBM_PART == 3
@@ -292,7 +372,7 @@ void launch_boundary_force<Q_>(const Ctx& c, int mode, const void* buf, const ui
   });
 }
 #else
-#error "LBM_PART must be 0..9"
+#error "LBM_PART must be 0..10"
 #endif
 
 }  // namespace lbm

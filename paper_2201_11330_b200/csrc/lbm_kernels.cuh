@@ -506,9 +506,12 @@ __device__ __forceinline__ void collide(double (&f)[Q], const Params& p, const C
       if constexpr (FORCE) g -= (k * D::t) * uF3;
       f[a] = fma(om1, f[a], g);
     } else {
+      // omega t_a (base + 4.5 A (e.u)^2) and 3 omega t_a A (e.u) with the factors that depend on the speed class only
+      // (three values of t_a) folded once per cell: 7 instead of 10 fp64 operations per +- pair
       const double eu = edot<Q, a>(ux, uy, uz);
-      double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
-      double d = (3.0 * om * D::t) * (A * eu);
+      const double w = om * D::t;
+      double s = fma(((4.5 * w) * A) * eu, eu, w * base);
+      double d = ((3.0 * w) * A) * eu;
       if constexpr (FORCE) {
         const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
         s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
@@ -613,8 +616,9 @@ __device__ __forceinline__ void collide_shifted(const float (&g)[Q], const Param
         store(IC<a>{}, fma(om1, (double)g[a], gq));
       } else {
         const double eu = edot<Q, a>(ux, uy, uz);
-        double s = (om * D::t) * fma(4.5 * A * eu, eu, base);
-        double d = (3.0 * om * D::t) * (A * eu);
+        const double w = om * D::t;  // per speed class, as in collide
+        double s = fma(((4.5 * w) * A) * eu, eu, w * base);
+        double d = ((3.0 * w) * A) * eu;
         if constexpr (FORCE) {
           const double eF = edot<Q, a>(p.F[0], p.F[1], p.F[2]);
           s = fma(k * D::t, fma(9.0 * eu, eF, -uF3), s);
@@ -914,6 +918,166 @@ __global__ void __launch_bounds__(kF32x2Threads, 5) stream_collide_ab_f32x2(cons
   });
 }
 
+// ---------------------------------------------------------------------------------------
+// Two time steps per pass through HBM (A/B scheme, BC_PERIODIC, fp64).  The one-step kernel above sits at the ceiling of
+// its access pattern (every population read once and written once per step: 0.999 x algorithmic DRAM bytes at 1.05 x the
+// device-copy bandwidth), so more lattice updates per second means fewer bytes per update.  A block owns a TX x TY
+// column of the box and marches along z.  Per plane it runs
+//   stage 1  the ordinary step t -> t+1 (pull from `src`, collide) on the tile EXTENDED by one cell on every side in
+//            x and y, and keeps the result in shared memory instead of storing it;
+//   stage 2  step t+1 -> t+2 on the tile itself, one plane behind, pulling from the three planes of stage-1 results in
+//            shared memory, and stores to `dst`.
+// What stage 2 pulls from plane q-1 are the e_z = +1 populations only, from plane q the e_z = 0 ones and from plane q+1
+// the e_z = -1 ones, so a plane's stage-1 result is kept per class for exactly as long as it is needed: the e_z = -1
+// class for the rest of the iteration that made it, e_z = 0 for one more iteration (2 slots), e_z = +1 for two more
+// (3 slots) — 38 population planes of the extended tile for D3Q19 instead of 3 x 19.  HBM traffic per TWO steps: one read
+// of the extended tile (the rim is shared with the neighbouring blocks through the L2) and one write of the tile,
+// against two reads and two writes; the price is (TX+2)(TY+2)/(TX TY) collisions in stage 1 and two block barriers per plane.
+// Same arithmetic per cell as ab_cell (collide): bit-identical to two launches of stream_collide_ab.
+template <int Q, int EZ>
+__host__ __device__ constexpr int ez_class_size() {
+  int n = 0;
+  for (int a = 0; a < Q; ++a) n += (Lattice<Q>::e[a][2] == EZ);
+  return n;
+}
+template <int Q, int A>
+__host__ __device__ constexpr int ez_class_index() {  // position of direction A among the directions with the same e_z
+  int n = 0;
+  for (int a = 0; a < A; ++a) n += (Lattice<Q>::e[a][2] == Lattice<Q>::e[A][2]);
+  return n;
+}
+
+// ONEBAR: one more slot per class (2 / 3 / 4), so that stage 1 of the next plane never writes a slot stage 2 of this plane
+// still reads and ONE block barrier per plane is enough.  PREFETCH: the stage-1 loads of the next plane are issued
+// before stage 2 of this one, so that their latency is covered by it (19 more registers pairs).
+template <int Q, int TX, int TY, bool ONEBAR, bool WALLS = false>
+struct Ab2Tile {
+  static constexpr int EX = TX + 2, EY = TY + 2, CELLS = EX * EY;  // stage-1 tile
+  static constexpr int THREADS = ((CELLS + 31) / 32) * 32;
+  static constexpr int NM = ez_class_size<Q, -1>(), N0 = ez_class_size<Q, 0>(), NP = ez_class_size<Q, 1>();
+  // Slots per class.  With one barrier per plane (between stage 1 and stage 2) a warp may run stage 1 of iteration k+1
+  // while another still runs stage 2 of iteration k, so slot (k+1) mod S must differ from every slot stage 2(k) reads:
+  // e_z = -1: k, and with walls k-1 (a wall link's own-plane value);  e_z = 0: k-1;  e_z = +1: k-2, with walls k-1.
+  static constexpr int SM_ = ONEBAR ? (WALLS ? 3 : 2) : 1, S0 = ONEBAR ? 3 : 2, SP = ONEBAR ? 4 : 3;
+  // shared memory, in doubles: [SM_][NM][CELLS] | [S0][N0][CELLS] | [SP][NP][CELLS]
+  static constexpr int OFF0 = SM_ * NM * CELLS, OFFP = OFF0 + S0 * N0 * CELLS, DOUBLES = OFFP + SP * NP * CELLS;
+  static constexpr size_t SMEM_BYTES = (size_t)DOUBLES * sizeof(double);
+};
+
+// BC_WALLS (halfway bounce-back, Ladd lid, inlet / outlet through collide's open_link): cells of the extended tile that lie
+// beyond a wall face are no nodes and are skipped; stage 1 pulls with the wall-slot select of the one-step kernel; stage 2
+// takes a wall link from the OWN cell's opposite direction in plane q — the e_z = +1 / 0 / -1 class of the previous
+// iteration (the e_z = -1 class lives one iteration longer for that: three slots instead of two).
+template <int Q, int EQ, int BC, bool FORCE, int TX, int TY, int MINB, bool ONEBAR, bool PREFETCH>
+__global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::THREADS, MINB)
+    stream_collide_ab2(const double* __restrict__ src, double* __restrict__ dst, int zchunk, const __grid_constant__ Params p) {
+  static_assert(BC == BC_PERIODIC || (BC == BC_WALLS && ONEBAR), "no link mask; wall links need the e_z = -1 class of the own plane");
+  using T = Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>;
+  extern __shared__ double sm[];
+  const int t = threadIdx.x;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int zs = blockIdx.z * zchunk, ze = min(zs + zchunk, p.nz);  // stage-2 planes [zs, ze)
+  // stage 1: thread t owns cell (xe, ye) of the extended tile = node (x0-1+xe, y0-1+ye), wrapped periodically
+  bool s1 = t < T::CELLS;
+  const int ye = t / T::EX, xe = t - ye * T::EX;
+  int gx = x0 - 1 + xe, gy = y0 - 1 + ye;
+  if constexpr (BC == BC_WALLS) {  // beyond a wall face: no node (faces of an axis are periodic or walls in pairs)
+    s1 = s1 & !(((gx < 0) | (gx >= p.nx)) & (p.wall[0] != 0)) & !(((gy < 0) | (gy >= p.ny)) & (p.wall[2] != 0));
+  }
+  gx = (gx < 0) ? gx + p.nx : (gx >= p.nx) ? gx - p.nx : gx;
+  gy = (gy < 0) ? gy + p.ny : (gy >= p.ny) ? gy - p.ny : gy;
+  const int ox[3] = {(gx == 0) ? p.nx - 1 : gx - 1, gx, (gx == p.nx - 1) ? 0 : gx + 1};
+  const int oy[3] = {((gy == 0) ? p.ny - 1 : gy - 1) * p.rs, gy * p.rs, ((gy == p.ny - 1) ? 0 : gy + 1) * p.rs};
+  const int c1xy = gx + p.nx * gy;
+  // stage 2: thread t < TX*TY owns node (x0+xi, y0+yi) = cell t2 of the extended tile
+  const int yi = t / TX, xi = t - yi * TX;
+  const bool s2 = (t < TX * TY) & (x0 + xi < p.nx) & (y0 + yi < p.ny);  // (ragged grids: the last tiles hang over the box)
+  const int t2 = (yi + 1) * T::EX + xi + 1;
+  const int o2 = (x0 + xi) + (y0 + yi) * p.rs;
+  const int c2xy = (x0 + xi) + p.nx * (y0 + yi);
+  // plane pz of stage 1 exists unless it lies beyond a z wall (block-uniform)
+  auto plane_exists = [&](int pz) { return BC == BC_PERIODIC || !((pz < 0 || pz >= p.nz) && p.wall[4] != 0); };
+  auto wrap_z = [&](int pz) { return (pz < 0) ? pz + p.nz : (pz >= p.nz) ? pz - p.nz : pz; };
+  auto pull_plane = [&](double (&f)[Q], int pz) {  // the Q populations that stream into the thread's stage-1 cell in plane pz
+    const int z = wrap_z(pz);
+    const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
+    const long long oz[3] = {zm * p.zs, z * p.zs, zp * p.zs};
+    const CellFlags<BC> c(p, gx, gy, z, 0);
+    static_for<0, Q>([&](auto A) {
+      constexpr int a = decltype(A)::value;
+      using D = Dir<Q, a>;
+      const double* q = plane<a>(src, p.ds) + ((ox[1 - D::ex] + oy[1 - D::ey]) + oz[1 - D::ez]);
+      if constexpr (BC == BC_WALLS && D::s > 0) {
+        if (c.template leaves<Q, a, -1>()) q = plane<D::opp>(src, p.ds) + ((ox[1] + oy[1]) + oz[1]);  // a select, not a branch
+      }
+      f[a] = LBM_LD_STREAM(q);
+    });
+  };
+  double fn[PREFETCH ? Q : 1];
+  if constexpr (PREFETCH) {
+    if (s1 && plane_exists(zs - 1)) pull_plane(fn, zs - 1);
+  }
+  for (int k = 0, pz = zs - 1; pz <= ze; ++pz, ++k) {
+    const int km = k % T::SM_, k0 = k % T::S0, kp = k % T::SP;
+    if (s1) {
+      if (plane_exists(pz)) {
+        const int z = wrap_z(pz);
+        double f[Q];
+        if constexpr (PREFETCH) {
+          static_for<0, Q>([&](auto A) { f[decltype(A)::value] = fn[decltype(A)::value]; });
+        } else {
+          pull_plane(f, pz);
+        }
+        const CellFlags<BC> c(p, gx, gy, z, 0);
+        collide<Q, EQ, BC, FORCE>(f, p, c, c1xy + p.nx * p.ny * z, z);
+        static_for<0, Q>([&](auto A) {
+          constexpr int a = decltype(A)::value;
+          constexpr int j = ez_class_index<Q, a>();
+          if constexpr (Dir<Q, a>::ez == -1) sm[(km * T::NM + j) * T::CELLS + t] = f[a];
+          else if constexpr (Dir<Q, a>::ez == 0) sm[T::OFF0 + (k0 * T::N0 + j) * T::CELLS + t] = f[a];
+          else sm[T::OFFP + (kp * T::NP + j) * T::CELLS + t] = f[a];
+        });
+      }
+      if constexpr (PREFETCH) {
+        if (pz < ze && plane_exists(pz + 1)) pull_plane(fn, pz + 1);
+      }
+    }
+    __syncthreads();
+    if (s2 && k >= 2) {
+      // plane q = pz - 1: e_z = -1 populations of plane q+1 (this iteration), e_z = 0 of plane q (previous iteration),
+      // e_z = +1 of plane q-1 (the one before)
+      const int q = pz - 1;
+      const double* sn = sm + (km * T::NM) * T::CELLS + t2;
+      const double* s0 = sm + T::OFF0 + (((k + T::S0 - 1) % T::S0) * T::N0) * T::CELLS + t2;
+      const double* sp = sm + T::OFFP + (((k + T::SP - 2) % T::SP) * T::NP) * T::CELLS + t2;
+      // the own plane's classes, for wall links: e_z = -1 and e_z = +1 of plane q were stored in the previous iteration
+      const double* snq = sm + (((k + T::SM_ - 1) % T::SM_) * T::NM) * T::CELLS + t2;
+      const double* spq = sm + T::OFFP + (((k + T::SP - 1) % T::SP) * T::NP) * T::CELLS + t2;
+      const CellFlags<BC> c(p, x0 + xi, y0 + yi, q, 0);
+      double f[Q];
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        using D = Dir<Q, a>;
+        constexpr int j = ez_class_index<Q, a>();
+        constexpr int d = j * T::CELLS - D::ey * T::EX - D::ex;  // class row + the upstream cell inside the extended tile
+        const double* r = (D::ez == -1) ? sn + d : (D::ez == 0) ? s0 + d : sp + d;
+        if constexpr (BC == BC_WALLS && D::s > 0) {
+          constexpr int jo = ez_class_index<Q, D::opp>() * T::CELLS;  // f_a = f*_abar of the own cell (Eq. 10's rule)
+          if (c.template leaves<Q, a, -1>()) r = (D::ez == -1) ? spq + jo : (D::ez == 0) ? s0 + jo : snq + jo;
+        }
+        f[a] = *r;
+      });
+      collide<Q, EQ, BC, FORCE>(f, p, c, c2xy + p.nx * p.ny * q, q);
+      double* out = dst + (o2 + q * p.zs);
+      static_for<0, Q>([&](auto A) {
+        constexpr int a = decltype(A)::value;
+        LBM_ST_STREAM(plane<a>(out, p.ds), f[a]);
+      });
+    }
+    if constexpr (!ONEBAR) __syncthreads();
+  }
+}
+
 // Small grids (both buffers resident in the L2: 32^3, 64^3, the paper's 512 x 128 channel) are bound by the launch
 // rate of one kernel per step (4-5 us), and CUDA-graph replay is slower still.  This persistent kernel takes all the steps of one lbm_step call in ONE cooperative
 // launch: every thread keeps its cell, the two buffers swap roles each step, a grid-wide barrier separates the steps
@@ -1011,6 +1175,69 @@ __global__ void __launch_bounds__(256, kMinBlocks<Q, FORCE, true>) stream_collid
   const int z = blockIdx.z;
   if (x >= p.nx || y >= p.ny) return;
   aa_odd_cell<Q, EQ, BC, FORCE, ST, false>(buf, p, x, y, z);
+}
+
+// Odd phase, one grid row per block (y = blockIdx.y, z = blockIdx.z; BC_PERIODIC / BC_WALLS).  The odd phase touches Q
+// DIFFERENT slots per cell and touches each of them twice (f_a is read where f*_abar is written: the link x <-> x - e_a
+// traversed both ways); in aa_odd_cell ptxas keeps or rebuilds Q 64-bit addresses across the collision (124-128
+// registers, D3Q27 spills up to 360 B, two blocks per SM).  Here everything but x is block-uniform: the row base of
+// every slot (direction row + y row + z plane, wall rows included for the y / z faces) lives in the uniform datapath, a
+// thread holds x-1, x, x+1 and its two x-face flags, and a slot address is one 64-bit add that is simply repeated
+// for the store.
+template <int Q, bool FORCE>
+constexpr int kAaRowMinBlocks = (Q == 27) ? 2 : (Q == 19) ? (FORCE ? 2 : 3) : (FORCE ? 3 : 4);
+
+template <int Q, int EQ, int BC, bool FORCE, typename ST>
+__global__ void __launch_bounds__(256, kAaRowMinBlocks<Q, FORCE>) stream_collide_aa_odd_row(ST* buf, const __grid_constant__ Params p) {
+  static_assert(BC != BC_GEO, "the link-mask kernels keep aa_odd_cell");
+  typedef unsigned long long addr_t;
+  constexpr long long E = sizeof(ST);
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y, z = blockIdx.z;
+  if (x >= p.nx) return;
+  const int ym = (y == 0) ? p.ny - 1 : y - 1, yp = (y == p.ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
+  // block-uniform byte offsets of the three y rows and the three z planes; per thread: the byte address of x-1, x, x+1
+  // in row 0 of plane 0 of direction 0
+  long long oy[3] = {E * ym * p.rs, E * y * p.rs, E * yp * p.rs};
+  long long oz[3] = {E * zm * p.zs, E * z * p.zs, E * zp * p.zs};
+  const long long dsb = E * p.ds;
+  const addr_t b0 = (addr_t)__cvta_generic_to_global(buf);
+  addr_t X[3] = {b0 + E * ((x == 0) ? p.nx - 1 : x - 1), b0 + E * x, b0 + E * ((x == p.nx - 1) ? 0 : x + 1)};
+  const int cell = x + p.nx * (y + p.ny * z);
+  const CellFlags<BC> c(p, x, y, z, cell);
+  // slot(a): where f_a(x) is read and f*_abar(x) is written — slot (x - e_a, abar), or (x, a) at a wall link
+  auto slot = [&](auto A) -> addr_t {
+    constexpr int a = decltype(A)::value;
+    using D = Dir<Q, a>;
+    const long long row = D::opp * dsb + oy[1 - D::ey] + oz[1 - D::ez];  // block-uniform
+    addr_t q = X[1 - D::ex] + (addr_t)row;
+    if constexpr (BC == BC_WALLS && D::s > 0) {
+      bool w = false;
+      if constexpr (D::ey == 1) w = w | c.lo[1];
+      if constexpr (D::ey == -1) w = w | c.hi[1];
+      if constexpr (D::ez == 1) w = w | c.lo[2];
+      if constexpr (D::ez == -1) w = w | c.hi[2];
+      if constexpr (D::ex == 1) w = w | c.lo[0];
+      if constexpr (D::ex == -1) w = w | c.hi[0];
+      if (w) q = X[1] + (addr_t)(a * dsb + oy[1] + oz[1]);
+    }
+    return q;
+  };
+  double f[Q];
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    f[a] = ld_pop_rw<ST, Q, a>((const ST*)slot(A), 0);
+  });
+  // the store addresses are rebuilt after the collision (two adds each) instead of Q of them staying live across it
+  asm volatile("" : "+l"(X[0]), "+l"(X[1]), "+l"(X[2]));
+  asm volatile("" : "+l"(oy[0]), "+l"(oy[1]), "+l"(oy[2]), "+l"(oz[0]), "+l"(oz[1]), "+l"(oz[2]));
+  collide<Q, EQ, BC, FORCE>(f, p, c, cell, z);
+  static_for<0, Q>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    constexpr int o = Dir<Q, a>::opp;
+    st_pop<ST, Q, o>((ST*)slot(A), 0, f[o]);
+  });
 }
 
 // The in-place scheme in one cooperative launch per lbm_step call, for grids whose ONE buffer fits the L2 (where

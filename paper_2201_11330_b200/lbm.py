@@ -28,7 +28,7 @@ LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200
 SYMBOLS = (
     "lbm_create", "lbm_destroy", "lbm_init_equilibrium", "lbm_init_equilibrium_host", "lbm_step",
     "lbm_moments", "lbm_moments_host", "lbm_get_populations", "lbm_set_populations", "lbm_lattice",
-    "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_set_persistent", "lbm_last_error",
+    "lbm_time", "lbm_launch_count", "lbm_set_block", "lbm_set_persistent", "lbm_set_two_step", "lbm_last_error",
     "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
     "lbm_set_face_velocity", "lbm_set_face_velocity_host", "lbm_set_face_density",
     "lbm_create_slab", "lbm_slab_export", "lbm_slab_connect", "lbm_slab_set_sync",
@@ -109,6 +109,8 @@ def load():
     lib.lbm_set_block.argtypes = [vp, i32, i32]
     lib.lbm_set_persistent.restype = i32
     lib.lbm_set_persistent.argtypes = [vp, i32]
+    lib.lbm_set_two_step.restype = i32
+    lib.lbm_set_two_step.argtypes = [vp, i32]
     for name in ("lbm_set_geometry", "lbm_set_geometry_host"):
         getattr(lib, name).restype = i32
         getattr(lib, name).argtypes = [vp, C.c_void_p, i32]
@@ -312,6 +314,10 @@ def lbm_set_persistent(h, on):
     _check(load().lbm_set_persistent(h, 1 if on else 0))
 
 
+def lbm_set_two_step(h, on):
+    _check(load().lbm_set_two_step(h, 1 if on else 0))
+
+
 # ---- convenience wrapper ----------------------------------------------------------------
 class Solver:
     """Owns one handle.  All tensors are torch float64, on the solver's CUDA device unless the
@@ -447,6 +453,9 @@ class Solver:
 
     def set_persistent(self, on):
         lbm_set_persistent(self.h, on)
+
+    def set_two_step(self, on):
+        lbm_set_two_step(self.h, on)
 
     def debug_arm(self, poison=True):
         lbm_debug_arm(self.h, poison)

@@ -31,7 +31,10 @@ def test_bench_line_has_the_contract_keys():
     assert d["unit"] == "MLUPS" and d["dtype"] == "f64" and d["data"] == "synthetic" and d["vs_baseline"] is None
     assert d["n_gpus"] == 1 and d["steps"] == 50 and d["warmup"] >= 3 and d["higher_is_better"] is True
     assert d["config"]["workload"] == "cfg1_q19_tgv128" and "model" not in d["config"]
-    assert d["gpu_launches"] == 50                                  # one fused kernel per time step, nothing else timed
+    # nothing but the fused kernel is timed: periodic D3Q19 fp64 takes two time steps per launch (stream_collide_ab2)
+    assert d["gpu_launches"] == 25 and d["roofline"]["steps_per_launch"] == 2
+    one = _run("--config", "1", "--steps", "50", "--warmup", "3", "--two-step", "0", "--no-cpu-baseline")
+    assert one["gpu_launches"] == 50 and one["roofline"]["steps_per_launch"] == 1  # one launch per time step
     assert abs(d["value"] - 128**3 * 50 / (d["ms_per_step"] * 50 * 1e-3) / 1e6) <= 1e-6 * d["value"]
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["bytes_per_cell_update"] == 304

@@ -578,6 +578,7 @@ def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
         for on in (1, 0):
             s = lbm.Solver(*dims, 19, 0.7, scheme=sch, **case)
             s.set_persistent(on)
+            s.set_two_step(0)  # (without the persistent kernel: one launch per step, not stream_collide_ab2's one per two)
             if use_geo:
                 s.set_geometry(geo, lbm.LBM_WALL_NODAL)
             s.set_populations(f0)
@@ -588,3 +589,70 @@ def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
             s.close()
         assert torch.equal(out[0][0], out[1][0])
         assert out[1][1] - out[0][1] == 15, out  # 17 step launches became 2
+
+
+@pytest.mark.parametrize("dims", [(32, 8, 4), (64, 16, 21), (40, 27, 19), (33, 9, 35), (96, 40, 50)])
+@pytest.mark.parametrize("faces", list(FACE_CASES))
+@pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
+def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq, forced):
+    """stream_collide_ab2 (two time steps per pass through HBM: stage 1 on a tile extended by one cell into shared memory,
+    stage 2 from there; lbm_set_two_step, default on for D3Q19 fp64 A/B without a solid mask) against the one-step kernel
+    — same arithmetic per cell: identical bits — and against the oracle, from random non-equilibrium populations: periodic
+    boxes, walls, the lid, moving walls on every face; grids of one tile, of ragged tiles in x and y, more z-chunks than
+    one, odd and even step counts."""
+    nx, ny, nz = dims
+    N = nx * ny * nz
+    kinds, uspec = FACE_CASES[faces]
+    fu = face_u_of(uspec)
+    force = (1e-5, -2e-6, 3e-6) if forced else None
+    f0 = random_f(19, N, seed=nx + ny + nz)
+    o, _s = make_pair(lbm, dims, 19, 0.57, eq=eq, face_kind=kinds, face_u=fu, force=force)
+    _s.close()
+    o.set_f(f0)
+    o.step(7)
+    ref = o.get_f()
+    o.close()
+    out = []
+    for on in (1, 0):
+        s = lbm.Solver(nx, ny, nz, 19, 0.57, eq=eq_flag(lbm, eq), scheme=lbm.LBM_SCHEME_AB, face_kind=kinds, face_u=fu, force=force)
+        s.set_persistent(0)  # (these grids would otherwise run in the persistent kernel)
+        s.set_two_step(on)
+        s.debug_arm(poison=True)
+        s.set_populations(dev(f0).reshape(-1))
+        l0 = s.launches
+        s.step(4)  # two passes
+        s.step(3)  # one pass + one single step
+        launches = s.launches - l0
+        out.append((s.get_populations().clone(), launches))
+        assert s.debug_check() == 0
+        s.close()
+    assert out[0][1] == 4 and out[1][1] == 7, (out[0][1], out[1][1])
+    assert torch.equal(out[0][0], out[1][0])
+    assert float(np.abs(out[0][0].cpu().numpy().reshape(19, N) - ref).max()) <= TOL
+
+
+@pytest.mark.parametrize("faces", ["periodic", "cavity", "mixed"])
+def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces):
+    """The same bit-for-bit comparison where every SM runs blocks of stream_collide_ab2 at once and warps of a block drift
+    apart between its barriers (320 x 192 x 96 = 5.9 M cells, 1440 blocks in 6 z-chunks, 40 steps): a hazard between
+    stage 1 of one plane and stage 2 of the previous one on a shared-memory slot shows up here, not on 10^4 cells."""
+    nx, ny, nz = 320, 192, 96
+    kinds, uspec = FACE_CASES[faces]
+    fu = face_u_of(uspec)
+    w = inputs.Workload("fill", nx, ny, nz, 19, 0.55, 40, face_kind=tuple(kinds), face_u=tuple(map(tuple, fu)), u0=0.04, noise=1e-3,
+                        seed=inputs.SEED_BASE + 77, kind="tgv" if faces == "periodic" else "rest")
+    rho, u = w.fields()
+    rho_d, u_d = dev(rho), dev(u.reshape(-1))
+    out = []
+    for on in (1, 0):
+        s = lbm.Solver.from_workload(w, scheme=lbm.LBM_SCHEME_AB)
+        s.set_two_step(on)
+        s.init_equilibrium(rho_d, u_d)
+        d0 = s.diagnostics()
+        s.step(w.steps)
+        out.append((s.get_populations().clone(), s.diagnostics()))
+        s.close()
+    assert torch.equal(out[0][0], out[1][0])
+    assert out[0][1][7] == 0
+    if faces != "mixed":
+        assert abs(out[0][1][0] - d0[0]) <= 1e-12 * d0[0]  # mass: the lid's +- links cancel (R6)
