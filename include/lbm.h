@@ -51,7 +51,11 @@ enum {
   LBM_EQ_INCOMP = 1 << 8,   /* Eq. 5, incompressible model with rho0 = 1               */
   LBM_SCHEME_AUTO = 0,      /* LBM_SCHEME_AB, except LBM_SCHEME_AA where one buffer fits the L2 and two do not */
   LBM_SCHEME_AB = 1 << 12,  /* two buffers, pull ("stream on read")                            */
-  LBM_SCHEME_AA = 2 << 12,  /* one buffer, in-place AA pattern                                 */
+  LBM_SCHEME_AA = 2 << 12,  /* one buffer, in-place AA pattern.  Measured cost against LBM_SCHEME_AB on one B200 (one step
+                               per pass, MLUPS, AA / AB): 512^3 D3Q19 periodic 22 470 / 22 520; 256^3 D3Q19 cavity
+                               22 420 / 22 560; 512^3 D3Q27 channel with forcing 14 760 / 15 900; with a solid mask the
+                               odd phase keeps Q addresses live (124-128 registers) and runs at 0.75-0.9 of AB.  AB also
+                               takes two steps per pass for D3Q19 fp64 (lbm_set_two_step: 31 400), AA does not.         */
   LBM_STORE_F64 = 0,        /* populations stored as fp64 (default)                            */
   LBM_STORE_F32 = 1 << 16,  /* populations stored as fp32 (f - t_a), arithmetic in fp64        */
   LBM_LAYOUT_ROWS = 0,      /* internal buffers f[z][y][a][x]: the Q rows of a grid row adjacent (default, faster);
@@ -214,8 +218,9 @@ int64_t lbm_debug_check(lbm_handle h);
 int lbm_set_persistent(lbm_handle h, int on);
 
 /* Two time steps per pass through HBM (Eq. 7 applied twice; the same collision, Eq. 6, in between).  For a
- * whole box (no z-slab) of D3Q19 populations stored as fp64 under LBM_SCHEME_AB — periodic, BOUNCE, MOVING and PRESSURE
- * faces; no solid mask (lbm_set_geometry) and no SYMMETRY face — lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
+ * whole box (no z-slab) of populations stored as fp64 under LBM_SCHEME_AB, without a solid mask (lbm_set_geometry) and
+ * without SYMMETRY faces — D3Q19 with periodic, BOUNCE, MOVING and PRESSURE faces; D3Q27 with all faces periodic —
+ * lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
  * runs step t+1 from there, so that every population is read from HBM once and written once per TWO steps.  Same
  * arithmetic per cell, same results bit for bit as single steps; an odd n ends with one single step.  on = 0 switches
  * it off (one pass per step, as for every other variant); default on.  Grids small enough for the persistent kernel

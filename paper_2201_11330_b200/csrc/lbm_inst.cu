@@ -209,57 +209,61 @@ void launch_step_ab_slab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
 #elif LBM_PART == 10
 template <>
 bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst) {
-  // D3Q19, fp64 storage, all faces periodic, whole box (measured: 512^3 22.5 -> 33.4 GLUPS).  D2Q9 has no z to march
-  // along; D3Q27 needs 81 population planes of shared memory per tile cell and is left to the one-step kernel.
-  if constexpr (Q_ != 19) {
+  // fp64 storage, no link mask, whole box.  D3Q19: 32 x 8 tiles, one block of 352 threads per SM, one barrier per plane,
+  // register prefetch of the next plane (512^3 periodic: 22.5 -> 33.6 GLUPS in one launch; z walls + forcing 22.5 -> 26.7).
+  // D3Q27 keeps 27 populations of three planes: 16 x 8 tiles, two blocks of 192 threads per SM, two barriers per plane
+  // (fewer shared-memory slots), no prefetch — periodic boxes only (400^3: 15.8 -> 21.0 GLUPS, with forcing 18.7; with
+  // walls the wall-link selects and the extra slots eat the gain: 15.2-16.3 against 15.5, measured for six tile shapes).
+  // D2Q9 has no z to march along.
+  if constexpr (Q_ == 9) {
     return false;
   } else {
-    constexpr int TX = 32, TY = 8;
-    if (c.bc == BC_GEO || c.f32 || c.p.slab || c.p.nx < TX || c.p.ny < TY || c.p.nz < 4) return false;
+    constexpr int TX = (Q_ == 19) ? 32 : 16, TY = 8, MINB = (Q_ == 19) ? 1 : 2;
+    constexpr bool ONEBAR = (Q_ == 19), PREFETCH = (Q_ == 19);
+    if (c.bc == BC_GEO || (Q_ == 27 && c.bc != BC_PERIODIC) || c.f32 || c.p.slab || c.p.nx < TX || c.p.ny < TY || c.p.nz < 4) return false;
     bool ok = true;
     dispatch_eq(c, [&](auto eq) {
       dispatch_force(c, [&](auto force) {
-       dispatch_bc(c, [&](auto bc) {
-        if constexpr (decltype(bc)::value == BC_GEO) {
-          ok = false;
-          return;
-        } else {
-        using T = Ab2Tile<Q_, TX, TY, true, decltype(bc)::value == BC_WALLS>;
-        auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, TX, TY, 1, true, true>;
-        static int resident_on[64] = {0};  // per device: blocks of this instantiation resident at once (0 = not asked yet)
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
-          cudaGetLastError();
-          ok = false;
-          return;
-        }
-        if (resident_on[dev] == 0) {
-          int sms = 0, per_sm = 0;
-          if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
-              cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-              cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, T::THREADS, T::SMEM_BYTES) != cudaSuccess || per_sm < 1) {
-            cudaGetLastError();
-            resident_on[dev] = -1;
+        dispatch_bc(c, [&](auto bc) {
+          if constexpr (decltype(bc)::value == BC_GEO || (Q_ == 27 && decltype(bc)::value != BC_PERIODIC)) {
+            ok = false;
           } else {
-            resident_on[dev] = per_sm * sms;
+            using T = Ab2Tile<Q_, TX, TY, ONEBAR, decltype(bc)::value == BC_WALLS>;
+            auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, TX, TY, MINB, ONEBAR, PREFETCH>;
+            static int resident_on[64] = {0};  // per device: blocks of this instantiation resident at once (0 = not asked yet)
+            int dev = 0;
+            if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+              cudaGetLastError();
+              ok = false;
+              return;
+            }
+            if (resident_on[dev] == 0) {
+              int sms = 0, per_sm = 0;
+              if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
+                  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+                  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, T::THREADS, T::SMEM_BYTES) != cudaSuccess || per_sm < 1) {
+                cudaGetLastError();
+                resident_on[dev] = -1;
+              } else {
+                resident_on[dev] = per_sm * sms;
+              }
+            }
+            const int resident = resident_on[dev];
+            if (resident < 0) {
+              ok = false;
+              return;
+            }
+            // z-chunks: enough blocks for ~16 waves (the tail of the last wave stays below a few percent), chunks of at
+            // least 16 planes (every chunk runs stage 1 on two planes more than it stores)
+            const long long tiles = (long long)((c.p.nx + TX - 1) / TX) * ((c.p.ny + TY - 1) / TY);
+            long long chunks = (16LL * resident + tiles - 1) / tiles;
+            if (chunks > c.p.nz / 16) chunks = c.p.nz / 16;
+            if (chunks < 1) chunks = 1;
+            const int zchunk = (int)((c.p.nz + chunks - 1) / chunks);
+            const dim3 grid((c.p.nx + TX - 1) / TX, (c.p.ny + TY - 1) / TY, (c.p.nz + zchunk - 1) / zchunk);
+            kernel<<<grid, T::THREADS, T::SMEM_BYTES, c.stream>>>((const double*)src, (double*)dst, zchunk, c.p);
           }
-        }
-        const int resident = resident_on[dev];
-        if (resident < 0) {
-          ok = false;
-          return;
-        }
-        // z-chunks: enough blocks for ~16 waves (the tail of the last wave stays below a few percent), chunks of at least
-        // 16 planes (every chunk runs stage 1 on two planes more than it stores)
-        const long long tiles = (long long)((c.p.nx + TX - 1) / TX) * ((c.p.ny + TY - 1) / TY);
-        long long chunks = (16LL * resident + tiles - 1) / tiles;
-        if (chunks > c.p.nz / 16) chunks = c.p.nz / 16;
-        if (chunks < 1) chunks = 1;
-        const int zchunk = (int)((c.p.nz + chunks - 1) / chunks);
-        const dim3 grid((c.p.nx + TX - 1) / TX, (c.p.ny + TY - 1) / TY, (c.p.nz + zchunk - 1) / zchunk);
-        kernel<<<grid, T::THREADS, T::SMEM_BYTES, c.stream>>>((const double*)src, (double*)dst, zchunk, c.p);
-        }
-       });
+        });
       });
     });
     return ok;

@@ -292,20 +292,43 @@ __device__ __forceinline__ void st_pop(ST* __restrict__ p, long long i, double v
 
 // ---------------------------------------------------------------------------------------
 // Moments (Eq. 8-9; D:R5, D:R7): rho = sum f; u = (sum e f + F/2)/rho  [Eq. 5: /rho0 = 1]
+// Sums over +- pairs first (s_a = f_a + f_abar feeds rho, d_a = f_a - f_abar feeds the momentum): 39 instead of 49 additions
+// for D3Q19 and dependency chains of depth 5 instead of 19 — the kernels that keep few warps per SM (stream_collide_ab2)
+// are bound by exactly that latency.
 template <int Q, int EQ, bool FORCE>
 __device__ __forceinline__ void moments(const double (&f)[Q], const Params& p, double& rho, double& ux, double& uy, double& uz) {
-  double r = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
-  static_for<0, Q>([&](auto A) {
+  constexpr int H = (Q - 1) / 2;  // pairs (a, Q-1-a), a < H; the rest direction is H
+  double sp[H], dp[H];
+  static_for<0, H>([&](auto A) {
+    constexpr int a = decltype(A)::value;
+    sp[a] = f[a] + f[Q - 1 - a];
+    dp[a] = f[a] - f[Q - 1 - a];
+  });
+  // balanced sums over compile-time index lists
+  double r = f[H], mx = 0.0, my = 0.0, mz = 0.0;
+  double r2 = 0.0, mx2 = 0.0, my2 = 0.0, mz2 = 0.0;  // two accumulators per sum halve the chains once more
+  static_for<0, H>([&](auto A) {
     constexpr int a = decltype(A)::value;
     using D = Dir<Q, a>;
-    r += f[a];
-    if constexpr (D::ex == 1) mx += f[a];
-    if constexpr (D::ex == -1) mx -= f[a];
-    if constexpr (D::ey == 1) my += f[a];
-    if constexpr (D::ey == -1) my -= f[a];
-    if constexpr (D::ez == 1) mz += f[a];
-    if constexpr (D::ez == -1) mz -= f[a];
+    if constexpr (a % 2 == 0) {
+      r += sp[a];
+      if constexpr (D::ex == 1) mx += dp[a];
+      if constexpr (D::ex == -1) mx -= dp[a];
+      if constexpr (D::ey == 1) my += dp[a];
+      if constexpr (D::ey == -1) my -= dp[a];
+      if constexpr (D::ez == 1) mz += dp[a];
+      if constexpr (D::ez == -1) mz -= dp[a];
+    } else {
+      r2 += sp[a];
+      if constexpr (D::ex == 1) mx2 += dp[a];
+      if constexpr (D::ex == -1) mx2 -= dp[a];
+      if constexpr (D::ey == 1) my2 += dp[a];
+      if constexpr (D::ey == -1) my2 -= dp[a];
+      if constexpr (D::ez == 1) mz2 += dp[a];
+      if constexpr (D::ez == -1) mz2 -= dp[a];
+    }
   });
+  r += r2; mx += mx2; my += my2; mz += mz2;
   if constexpr (FORCE) {
     mx += 0.5 * p.F[0];
     my += 0.5 * p.F[1];
@@ -958,7 +981,9 @@ struct Ab2Tile {
   // Slots per class.  With one barrier per plane (between stage 1 and stage 2) a warp may run stage 1 of iteration k+1
   // while another still runs stage 2 of iteration k, so slot (k+1) mod S must differ from every slot stage 2(k) reads:
   // e_z = -1: k, and with walls k-1 (a wall link's own-plane value);  e_z = 0: k-1;  e_z = +1: k-2, with walls k-1.
-  static constexpr int SM_ = ONEBAR ? (WALLS ? 3 : 2) : 1, S0 = ONEBAR ? 3 : 2, SP = ONEBAR ? 4 : 3;
+  // With two barriers per plane (the second after stage 2) stage 1 of iteration k only has to spare what stage 2 of the
+  // SAME iteration reads: 1 / 2 / 3 slots, with walls 2 / 2 / 3.
+  static constexpr int SM_ = ONEBAR ? (WALLS ? 3 : 2) : (WALLS ? 2 : 1), S0 = ONEBAR ? 3 : 2, SP = ONEBAR ? 4 : 3;
   // shared memory, in doubles: [SM_][NM][CELLS] | [S0][N0][CELLS] | [SP][NP][CELLS]
   static constexpr int OFF0 = SM_ * NM * CELLS, OFFP = OFF0 + S0 * N0 * CELLS, DOUBLES = OFFP + SP * NP * CELLS;
   static constexpr size_t SMEM_BYTES = (size_t)DOUBLES * sizeof(double);
@@ -971,7 +996,7 @@ struct Ab2Tile {
 template <int Q, int EQ, int BC, bool FORCE, int TX, int TY, int MINB, bool ONEBAR, bool PREFETCH>
 __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::THREADS, MINB)
     stream_collide_ab2(const double* __restrict__ src, double* __restrict__ dst, int zchunk, const __grid_constant__ Params p) {
-  static_assert(BC == BC_PERIODIC || (BC == BC_WALLS && ONEBAR), "no link mask; wall links need the e_z = -1 class of the own plane");
+  static_assert(BC == BC_PERIODIC || BC == BC_WALLS, "no link mask");
   using T = Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>;
   extern __shared__ double sm[];
   const int t = threadIdx.x;
@@ -998,20 +1023,30 @@ __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::TH
   // plane pz of stage 1 exists unless it lies beyond a z wall (block-uniform)
   auto plane_exists = [&](int pz) { return BC == BC_PERIODIC || !((pz < 0 || pz >= p.nz) && p.wall[4] != 0); };
   auto wrap_z = [&](int pz) { return (pz < 0) ? pz + p.nz : (pz >= p.nz) ? pz - p.nz : pz; };
-  auto pull_plane = [&](double (&f)[Q], int pz) {  // the Q populations that stream into the thread's stage-1 cell in plane pz
-    const int z = wrap_z(pz);
+  // BC_WALLS: only the tiles on an x / y wall and the planes on a z wall hold wall links; everything else takes the
+  // periodic code (no flag tests, no second address, no select: block-uniform branches), which is what the step costs
+  // in this latency-bound kernel (512^3, z walls: 28.7 against 31.2 GLUPS periodic when every cell ran the selects).
+  // (the extended tile reaches one cell beyond the tile: it must not contain the last node either)
+  const bool tile_walls = (BC == BC_WALLS) && ((((x0 == 0) | (x0 + TX >= p.nx - 1)) & (p.wall[0] != 0)) | (((y0 == 0) | (y0 + TY >= p.ny - 1)) & (p.wall[2] != 0)));
+  auto plane_walls = [&](int z) { return (BC == BC_WALLS) && (tile_walls | (((z == 0) | (z == p.nz - 1)) & (p.wall[4] != 0))); };
+  auto pull_plane_as = [&](auto W, double (&f)[Q], int z) {
     const int zm = (z == 0) ? p.nz - 1 : z - 1, zp = (z == p.nz - 1) ? 0 : z + 1;
     const long long oz[3] = {zm * p.zs, z * p.zs, zp * p.zs};
-    const CellFlags<BC> c(p, gx, gy, z, 0);
+    const CellFlags<decltype(W)::value ? BC_WALLS : BC_PERIODIC> c(p, gx, gy, z, 0);
     static_for<0, Q>([&](auto A) {
       constexpr int a = decltype(A)::value;
       using D = Dir<Q, a>;
       const double* q = plane<a>(src, p.ds) + ((ox[1 - D::ex] + oy[1 - D::ey]) + oz[1 - D::ez]);
-      if constexpr (BC == BC_WALLS && D::s > 0) {
+      if constexpr (decltype(W)::value != 0 && D::s > 0) {
         if (c.template leaves<Q, a, -1>()) q = plane<D::opp>(src, p.ds) + ((ox[1] + oy[1]) + oz[1]);  // a select, not a branch
       }
       f[a] = LBM_LD_STREAM(q);
     });
+  };
+  auto pull_plane = [&](double (&f)[Q], int pz) {  // the Q populations that stream into the thread's stage-1 cell in plane pz
+    const int z = wrap_z(pz);
+    if (plane_walls(z)) pull_plane_as(IC<1>{}, f, z);
+    else pull_plane_as(IC<0>{}, f, z);
   };
   double fn[PREFETCH ? Q : 1];
   if constexpr (PREFETCH) {
@@ -1038,6 +1073,8 @@ __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::TH
           else sm[T::OFFP + (kp * T::NP + j) * T::CELLS + t] = f[a];
         });
       }
+      // the next plane's loads go out AFTER this plane's collision and shared-memory stores (measured: issued before
+      // the collision, 512^3 falls from 33.6 to 24.4 GLUPS) and have the barrier and stage 2 to arrive
       if constexpr (PREFETCH) {
         if (pz < ze && plane_exists(pz + 1)) pull_plane(fn, pz + 1);
       }
@@ -1055,18 +1092,22 @@ __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::TH
       const double* spq = sm + T::OFFP + (((k + T::SP - 1) % T::SP) * T::NP) * T::CELLS + t2;
       const CellFlags<BC> c(p, x0 + xi, y0 + yi, q, 0);
       double f[Q];
-      static_for<0, Q>([&](auto A) {
-        constexpr int a = decltype(A)::value;
-        using D = Dir<Q, a>;
-        constexpr int j = ez_class_index<Q, a>();
-        constexpr int d = j * T::CELLS - D::ey * T::EX - D::ex;  // class row + the upstream cell inside the extended tile
-        const double* r = (D::ez == -1) ? sn + d : (D::ez == 0) ? s0 + d : sp + d;
-        if constexpr (BC == BC_WALLS && D::s > 0) {
-          constexpr int jo = ez_class_index<Q, D::opp>() * T::CELLS;  // f_a = f*_abar of the own cell (Eq. 10's rule)
-          if (c.template leaves<Q, a, -1>()) r = (D::ez == -1) ? spq + jo : (D::ez == 0) ? s0 + jo : snq + jo;
-        }
-        f[a] = *r;
-      });
+      auto gather2 = [&](auto W) {
+        static_for<0, Q>([&](auto A) {
+          constexpr int a = decltype(A)::value;
+          using D = Dir<Q, a>;
+          constexpr int j = ez_class_index<Q, a>();
+          constexpr int d = j * T::CELLS - D::ey * T::EX - D::ex;  // class row + the upstream cell inside the extended tile
+          const double* r = (D::ez == -1) ? sn + d : (D::ez == 0) ? s0 + d : sp + d;
+          if constexpr (decltype(W)::value != 0 && D::s > 0) {
+            constexpr int jo = ez_class_index<Q, D::opp>() * T::CELLS;  // f_a = f*_abar of the own cell (Eq. 10's rule)
+            if (c.template leaves<Q, a, -1>()) r = (D::ez == -1) ? spq + jo : (D::ez == 0) ? s0 + jo : snq + jo;
+          }
+          f[a] = *r;
+        });
+      };
+      if (plane_walls(q)) gather2(IC<1>{});
+      else gather2(IC<0>{});
       collide<Q, EQ, BC, FORCE>(f, p, c, c2xy + p.nx * p.ny * q, q);
       double* out = dst + (o2 + q * p.zs);
       static_for<0, Q>([&](auto A) {

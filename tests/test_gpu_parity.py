@@ -234,7 +234,9 @@ def test_config0_tgv32_full_length(lbm, scheme):
         s.step(1)
         E.append(s.diagnostics()[4])
     o.step(w.steps)
-    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    err = float(np.abs(s.get_populations().cpu().numpy() - o.get_f()).max())
+    print(f"\ntest_config0_tgv32_full_length: max|df| vs oracle = {err:.2e}")
+    assert err <= TOL
     d1 = s.diagnostics()
     do = o.moments(False)[2]
     np.testing.assert_allclose(d1[:5], do[:5], rtol=1e-12, atol=1e-12)
@@ -256,7 +258,9 @@ def test_config1_tgv128_full_length(lbm):
     s.init_equilibrium(dev(rho), dev(u.reshape(-1)))
     o.step(w.steps)
     s.step(w.steps)
-    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    err = float(np.abs(s.get_populations().cpu().numpy() - o.get_f()).max())
+    print(f"\ntest_config1_tgv128_full_length: max|df| vs oracle = {err:.2e}")
+    assert err <= TOL
     s.close()
 
 
@@ -270,7 +274,9 @@ def test_config2_cavity_analogue_full_length(lbm, scheme):
     s.init_equilibrium(None, None)
     o.step(w.steps)
     s.step(w.steps)
-    assert np.abs(s.get_populations().cpu().numpy() - o.get_f()).max() <= TOL
+    err = float(np.abs(s.get_populations().cpu().numpy() - o.get_f()).max())
+    print(f"\ntest_config2_cavity_analogue_full_length: max|df| vs oracle = {err:.2e}")
+    assert err <= TOL
     rho, u, d = s.moments()
     assert abs(d[0] - w.N) / w.N < 1e-12  # mass
     uy = u[1].cpu().numpy().reshape(32, 32, 32)
@@ -288,7 +294,9 @@ def test_config2_cavity256_first_steps(lbm):
     o.step(10)
     s.step(10)
     got = s.get_populations().cpu().numpy()
-    assert np.abs(got - o.get_f()).max() <= TOL
+    err = float(np.abs(got - o.get_f()).max())
+    print(f"\ntest_config2_cavity256_first_steps: max|df| vs oracle = {err:.2e}")
+    assert err <= TOL
     s.close()
 
 
@@ -346,7 +354,9 @@ def test_config3_tgv512_sampled(lbm, scheme):
     k = 3
     s.step(k)
     centers = [(0, 0, 0), (511, 511, 511), (0, 255, 511), (256, 0, 17), (100, 200, 300), (255, 256, 511), (31, 32, 33)]
-    assert _subbox_check(lbm, w, s, k, centers) <= TOL
+    err = _subbox_check(lbm, w, s, k, centers)
+    print(f"\ntest_config3_tgv512_sampled: max|df| vs oracle on the sampled sub-boxes = {err:.2e}")
+    assert err <= TOL
     s.step(20 - k)
     d1 = s.diagnostics()
     assert abs(d1[0] - d0[0]) / d0[0] < 1e-13
@@ -365,7 +375,9 @@ def test_config4_channel512_sampled(lbm):
     k = 3
     s.step(k)
     centers = [(0, 0, 0), (511, 511, 511), (17, 300, 1), (200, 5, 510), (256, 256, 256), (511, 0, 2)]
-    assert _subbox_check(lbm, w, s, k, centers) <= TOL
+    err = _subbox_check(lbm, w, s, k, centers)
+    print(f"\ntest_config4_channel512_sampled: max|df| vs oracle on the sampled sub-boxes = {err:.2e}")
+    assert err <= TOL
     steps = 200
     s.step(steps - k)
     _, uf, d = s.moments()
@@ -591,22 +603,14 @@ def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
         assert out[1][1] - out[0][1] == 15, out  # 17 step launches became 2
 
 
-@pytest.mark.parametrize("dims", [(32, 8, 4), (64, 16, 21), (40, 27, 19), (33, 9, 35), (96, 40, 50)])
-@pytest.mark.parametrize("faces", list(FACE_CASES))
-@pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
-def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq, forced):
-    """stream_collide_ab2 (two time steps per pass through HBM: stage 1 on a tile extended by one cell into shared memory,
-    stage 2 from there; lbm_set_two_step, default on for D3Q19 fp64 A/B without a solid mask) against the one-step kernel
-    — same arithmetic per cell: identical bits — and against the oracle, from random non-equilibrium populations: periodic
-    boxes, walls, the lid, moving walls on every face; grids of one tile, of ragged tiles in x and y, more z-chunks than
-    one, odd and even step counts."""
+def _two_step_case(lbm, Q, dims, faces, eq, forced, pairs=True):
     nx, ny, nz = dims
     N = nx * ny * nz
     kinds, uspec = FACE_CASES[faces]
     fu = face_u_of(uspec)
     force = (1e-5, -2e-6, 3e-6) if forced else None
-    f0 = random_f(19, N, seed=nx + ny + nz)
-    o, _s = make_pair(lbm, dims, 19, 0.57, eq=eq, face_kind=kinds, face_u=fu, force=force)
+    f0 = random_f(Q, N, seed=nx + ny + nz + Q)
+    o, _s = make_pair(lbm, dims, Q, 0.57, eq=eq, face_kind=kinds, face_u=fu, force=force)
     _s.close()
     o.set_f(f0)
     o.step(7)
@@ -614,7 +618,7 @@ def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq
     o.close()
     out = []
     for on in (1, 0):
-        s = lbm.Solver(nx, ny, nz, 19, 0.57, eq=eq_flag(lbm, eq), scheme=lbm.LBM_SCHEME_AB, face_kind=kinds, face_u=fu, force=force)
+        s = lbm.Solver(nx, ny, nz, Q, 0.57, eq=eq_flag(lbm, eq), scheme=lbm.LBM_SCHEME_AB, face_kind=kinds, face_u=fu, force=force)
         s.set_persistent(0)  # (these grids would otherwise run in the persistent kernel)
         s.set_two_step(on)
         s.debug_arm(poison=True)
@@ -626,20 +630,48 @@ def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq
         out.append((s.get_populations().clone(), launches))
         assert s.debug_check() == 0
         s.close()
-    assert out[0][1] == 4 and out[1][1] == 7, (out[0][1], out[1][1])
+    assert out[0][1] == (4 if pairs else 7) and out[1][1] == 7, (out[0][1], out[1][1])
     assert torch.equal(out[0][0], out[1][0])
-    assert float(np.abs(out[0][0].cpu().numpy().reshape(19, N) - ref).max()) <= TOL
+    assert float(np.abs(out[0][0].cpu().numpy().reshape(Q, N) - ref).max()) <= TOL
 
 
+@pytest.mark.parametrize("dims", [(32, 8, 4), (64, 16, 21), (40, 27, 19), (33, 9, 35), (96, 40, 50), (65, 17, 9), (128, 25, 12)])
+@pytest.mark.parametrize("faces", list(FACE_CASES))
+@pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
+def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq, forced):
+    """stream_collide_ab2 (two time steps per pass through HBM: stage 1 on a tile extended by one cell into shared memory,
+    stage 2 from there; lbm_set_two_step, default on for fp64 A/B without a solid mask) against the one-step kernel
+    — same arithmetic per cell: identical bits — and against the oracle, from random non-equilibrium populations: periodic
+    boxes, walls, the lid, moving walls on every face; grids of one tile, of ragged tiles in x and y, more z-chunks than
+    one, odd and even step counts.  D3Q19: 32 x 8 tiles, one barrier per plane, register prefetch."""
+    _two_step_case(lbm, 19, dims, faces, eq, forced)
+
+
+@pytest.mark.parametrize("dims", [(16, 8, 4), (48, 16, 21), (40, 27, 19), (17, 9, 35), (96, 40, 50)])
+@pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
+def test_two_step_kernel_d3q27(lbm, dims, eq, forced):
+    """The same for D3Q27, periodic boxes: 16 x 8 tiles, two barriers per plane (1 / 2 / 3 slots per e_z class), no
+    prefetch, two blocks per SM."""
+    _two_step_case(lbm, 27, dims, "periodic", eq, forced)
+
+
+@pytest.mark.parametrize("faces", ["channel_z", "cavity"])
+def test_two_step_mode_leaves_d3q27_with_walls_to_the_one_step_kernel(lbm, faces):
+    """D3Q27 with wall faces has no two-step kernel (measured: no gain): lbm_step falls back to one launch per step."""
+    _two_step_case(lbm, 27, (48, 16, 21), faces, EQ_STANDARD, True, pairs=False)
+
+
+@pytest.mark.parametrize("Q", [19, 27])
 @pytest.mark.parametrize("faces", ["periodic", "cavity", "mixed"])
-def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces):
+def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces, Q):
     """The same bit-for-bit comparison where every SM runs blocks of stream_collide_ab2 at once and warps of a block drift
     apart between its barriers (320 x 192 x 96 = 5.9 M cells, 1440 blocks in 6 z-chunks, 40 steps): a hazard between
     stage 1 of one plane and stage 2 of the previous one on a shared-memory slot shows up here, not on 10^4 cells."""
     nx, ny, nz = 320, 192, 96
     kinds, uspec = FACE_CASES[faces]
     fu = face_u_of(uspec)
-    w = inputs.Workload("fill", nx, ny, nz, 19, 0.55, 40, face_kind=tuple(kinds), face_u=tuple(map(tuple, fu)), u0=0.04, noise=1e-3,
+    w = inputs.Workload("fill", nx, ny, nz, Q, 0.55, 40, face_kind=tuple(kinds), face_u=tuple(map(tuple, fu)), u0=0.04, noise=1e-3,
+                        force=(1e-6, 0.0, 0.0) if Q == 27 else (0.0, 0.0, 0.0),
                         seed=inputs.SEED_BASE + 77, kind="tgv" if faces == "periodic" else "rest")
     rho, u = w.fields()
     rho_d, u_d = dev(rho), dev(u.reshape(-1))

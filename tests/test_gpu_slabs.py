@@ -268,6 +268,58 @@ def test_two_processes_connected_through_cuda_ipc(mods, tmp_path):
     assert out["mass_rel"] <= 1e-13 and out["umax_equal"]
 
 
+IPC_WORKER_DEVICE_SYNC = IPC_WORKER.replace(
+    "g = slabs.SlabSolver(w, rank, world, device_sync=False)", "g = slabs.SlabSolver(w, rank, world, device_sync=True)").replace(
+    """for _ in range(w.steps):
+    g.step(1)
+    torch.cuda.synchronize(); replicas.barrier()
+""", """g.step(w.steps)   # all steps in one call, no host synchronisation between them: the two processes are ordered by
+# lbm_moments_host between unsynchronised step calls (the neighbour may already be a step ahead and push into the idle
+# buffer's halo planes: the host entry points of a slab stage in a scratch allocation, not in that buffer)
+r_h = torch.empty(g.N, dtype=torch.float64).pin_memory(); u_h = torch.empty(3 * g.N, dtype=torch.float64).pin_memory()
+d_mid = lbm.lbm_moments_host(g.h, r_h, u_h, True)
+assert d_mid[7] == 0 and abs(float(r_h.view(g.nz_local + 2, -1)[1:-1].sum()) - d_mid[0]) <= 1e-9 * d_mid[0]
+g.step(w.steps)   # the device-side step counters alone (cuStreamWaitValue32 on the neighbour's counter)
+torch.cuda.synchronize(); replicas.barrier()
+""").replace("s.step(w.steps)\n    one =", "s.step(2 * w.steps)\n    one =")
+
+
+def test_two_processes_with_device_side_ordering(mods, tmp_path):
+    """The same two processes with lbm_slab_set_sync left ON: each rank enqueues all its steps at once, and a step starts
+    when the stream's cuStreamWaitValue32 sees the neighbour's counter (written by the OTHER process's slab_signal_kernel
+    through CUDA IPC memory).  Two contexts time-share this one GPU; a wait-value is a front-end wait, not a spinning
+    kernel, so the waiting context yields and the pair makes progress (measured: 2 x 200 steps in 34 ms).  The worker
+    runs under its own process group with a 150 s limit, so a deadlock would fail the test instead of hanging the box."""
+    import json
+    import os
+    import signal
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    assert "device_sync=True" in IPC_WORKER_DEVICE_SYNC and "g.step(w.steps)   # all steps" in IPC_WORKER_DEVICE_SYNC
+    assert "s.step(2 * w.steps)" in IPC_WORKER_DEVICE_SYNC
+    script = tmp_path / "ipc_worker_device_sync.py"
+    script.write_text(IPC_WORKER_DEVICE_SYNC)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, LBM_ROOT=root, MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
+    p = subprocess.Popen(cmd, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, start_new_session=True)
+    try:
+        out, err = p.communicate(timeout=150)
+    except subprocess.TimeoutExpired:
+        os.killpg(p.pid, signal.SIGKILL)
+        p.communicate()
+        pytest.fail("two processes ordered by device-side counters made no progress on one GPU within 150 s")
+    assert p.returncode == 0, err[-8000:]
+    res = [json.loads(ln[3:]) for ln in out.splitlines() if ln.startswith("OUT")][-1]
+    assert res["equal"], res
+    assert res["mass_rel"] <= 1e-13 and res["umax_equal"]
+
+
 # --------------------------------------------------------------------------- solid masks, nodal walls, mirror planes on slabs
 def _oracle_geo_run(w, steps):
     rho, u = w.fields()
