@@ -219,8 +219,8 @@ int lbm_set_persistent(lbm_handle h, int on);
 
 /* Two time steps per pass through HBM (Eq. 7 applied twice; the same collision, Eq. 6, in between).  For a
  * whole box (no z-slab) of populations stored as fp64 under LBM_SCHEME_AB, without a solid mask (lbm_set_geometry) and
- * without SYMMETRY faces — D3Q19 with periodic, BOUNCE, MOVING and PRESSURE faces; D3Q27 with all faces periodic —
- * lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
+ * without SYMMETRY faces — D3Q19 with periodic, BOUNCE, MOVING and PRESSURE faces; D3Q27 with periodic x and y faces
+ * (any z faces of those kinds) — lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
  * runs step t+1 from there, so that every population is read from HBM once and written once per TWO steps.  Same
  * arithmetic per cell, same results bit for bit as single steps; an odd n ends with one single step.  on = 0 switches
  * it off (one pass per step, as for every other variant); default on.  Grids small enough for the persistent kernel

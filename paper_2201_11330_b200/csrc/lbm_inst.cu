@@ -207,29 +207,41 @@ void launch_step_ab_slab_sym<Q_>(const Ctx& c, const void* src, void* dst) {
   });
 }
 #elif LBM_PART == 10
+namespace {
+// tile, blocks per SM, barrier scheme and prefetch of stream_collide_ab2 per lattice (measured; comment in launch_step_ab2)
+template <int Q, int BCV>
+struct Ab2Pick {
+  static constexpr int TX = (Q == 19) ? 32 : 16, TY = 8, MINB = (Q == 19) ? 1 : 2;
+  static constexpr bool ONEBAR = (Q == 19), PREFETCH = (Q == 19);
+  using T = Ab2Tile<Q, TX, TY, ONEBAR, (BCV == BC_WALLS) && ONEBAR>;
+};
+}  // namespace
+
 template <>
 bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst) {
   // fp64 storage, no link mask, whole box.  D3Q19: 32 x 8 tiles, one block of 352 threads per SM, one barrier per plane,
   // register prefetch of the next plane (512^3 periodic: 22.5 -> 33.6 GLUPS in one launch; z walls + forcing 22.5 -> 26.7).
   // D3Q27 keeps 27 populations of three planes: 16 x 8 tiles, two blocks of 192 threads per SM, two barriers per plane
-  // (fewer shared-memory slots), no prefetch — periodic boxes only (400^3: 15.8 -> 21.0 GLUPS, with forcing 18.7; with
-  // walls the wall-link selects and the extra slots eat the gain: 15.2-16.3 against 15.5, measured for six tile shapes).
-  // D2Q9 has no z to march along.
+  // (fewer shared-memory slots), no prefetch (400^3 periodic: 15.8 -> 21.0 GLUPS, with forcing 18.7).  Walls through the
+  // stage-2 select and the extra slots ate that gain (15.2-16.3 against 15.5, six tile shapes), so D3Q27 takes walls
+  // only as ghost planes in z (x, y periodic: 512^3 channel with forcing 15.7 -> 17.1 GLUPS).  D2Q9 has no z to march along.
   if constexpr (Q_ == 9) {
     return false;
   } else {
-    constexpr int TX = (Q_ == 19) ? 32 : 16, TY = 8, MINB = (Q_ == 19) ? 1 : 2;
-    constexpr bool ONEBAR = (Q_ == 19), PREFETCH = (Q_ == 19);
-    if (c.bc == BC_GEO || (Q_ == 27 && c.bc != BC_PERIODIC) || c.f32 || c.p.slab || c.p.nx < TX || c.p.ny < TY || c.p.nz < 4) return false;
+    constexpr int TX = Ab2Pick<Q_, 0>::TX, TY = Ab2Pick<Q_, 0>::TY;
+    // D3Q27 with walls: z walls only (x and y periodic), which the two-barrier kernel resolves through ghost planes
+    const bool q27_ok = c.bc == BC_PERIODIC || (c.bc == BC_WALLS && !c.p.wall[0] && !c.p.wall[1] && !c.p.wall[2] && !c.p.wall[3]);
+    if (c.bc == BC_GEO || (Q_ == 27 && !q27_ok) || c.f32 || c.p.slab || c.p.nx < TX || c.p.ny < TY || c.p.nz < 4) return false;
     bool ok = true;
     dispatch_eq(c, [&](auto eq) {
       dispatch_force(c, [&](auto force) {
         dispatch_bc(c, [&](auto bc) {
-          if constexpr (decltype(bc)::value == BC_GEO || (Q_ == 27 && decltype(bc)::value != BC_PERIODIC)) {
+          if constexpr (decltype(bc)::value == BC_GEO) {
             ok = false;
           } else {
-            using T = Ab2Tile<Q_, TX, TY, ONEBAR, decltype(bc)::value == BC_WALLS>;
-            auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, TX, TY, MINB, ONEBAR, PREFETCH>;
+            using P = Ab2Pick<Q_, decltype(bc)::value>;
+            using T = typename P::T;
+            auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, P::TX, P::TY, P::MINB, P::ONEBAR, P::PREFETCH>;
             static int resident_on[64] = {0};  // per device: blocks of this instantiation resident at once (0 = not asked yet)
             int dev = 0;
             if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {

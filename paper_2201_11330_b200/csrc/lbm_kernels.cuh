@@ -994,10 +994,16 @@ struct Ab2Tile {
 // takes a wall link from the OWN cell's opposite direction in plane q — the e_z = +1 / 0 / -1 class of the previous
 // iteration (the e_z = -1 class lives one iteration longer for that: three slots instead of two).
 template <int Q, int EQ, int BC, bool FORCE, int TX, int TY, int MINB, bool ONEBAR, bool PREFETCH>
-__global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::THREADS, MINB)
+__global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS && ONEBAR>::THREADS, MINB)
     stream_collide_ab2(const double* __restrict__ src, double* __restrict__ dst, int zchunk, const __grid_constant__ Params p) {
   static_assert(BC == BC_PERIODIC || BC == BC_WALLS, "no link mask");
-  using T = Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>;
+  // ZGHOST (BC_WALLS with two barriers per plane; the launcher admits it for boxes whose x and y faces are periodic): the
+  // z walls act through GHOST planes.  When stage 1 has plane 0, every cell also puts its outgoing e_z = -1 values where
+  // stage 2 of plane 0 will look for the e_z = +1 populations of plane -1 (f_a(x) = f*_abar(x): Eq. 10's rule), and
+  // in the iteration of the missing plane nz the e_z = +1 values of plane nz-1 go where its e_z = -1 populations are
+  // expected; stage 2 then runs the periodic code on the periodic slot set, with no select and no extra slot.
+  constexpr bool ZGHOST = (BC == BC_WALLS) && !ONEBAR;
+  using T = Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS && ONEBAR>;
   extern __shared__ double sm[];
   const int t = threadIdx.x;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
@@ -1072,6 +1078,31 @@ __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::TH
           else if constexpr (Dir<Q, a>::ez == 0) sm[T::OFF0 + (k0 * T::N0 + j) * T::CELLS + t] = f[a];
           else sm[T::OFFP + (kp * T::NP + j) * T::CELLS + t] = f[a];
         });
+        if constexpr (ZGHOST) {
+          if (z == 0 && p.wall[4] != 0) {  // ghost plane -1: its e_z = +1 class lives in the slot of the previous iteration
+            static_for<0, Q>([&](auto A) {
+              constexpr int a = decltype(A)::value;
+              using D = Dir<Q, a>;
+              if constexpr (D::ez == 1) {
+                // the reader is the cell itself, one plane up the link: it pulls direction a from the cell at -e_a (x, y)
+                const bool in = (xe - D::ex >= 0) & (xe - D::ex < T::EX) & (ye - D::ey >= 0) & (ye - D::ey < T::EY);
+                if (in) sm[T::OFFP + (((k + T::SP - 1) % T::SP) * T::NP + ez_class_index<Q, a>()) * T::CELLS + t - D::ey * T::EX - D::ex] = f[D::opp];
+              }
+            });
+          }
+        }
+      } else if constexpr (ZGHOST) {
+        if (pz == p.nz) {  // ghost plane nz: its e_z = -1 class, from the e_z = +1 values this thread stored for plane nz-1
+          static_for<0, Q>([&](auto A) {
+            constexpr int a = decltype(A)::value;
+            using D = Dir<Q, a>;
+            if constexpr (D::ez == -1) {
+              const bool in = (xe - D::ex >= 0) & (xe - D::ex < T::EX) & (ye - D::ey >= 0) & (ye - D::ey < T::EY);
+              const double v = sm[T::OFFP + (((k + T::SP - 1) % T::SP) * T::NP + ez_class_index<Q, D::opp>()) * T::CELLS + t];
+              if (in) sm[(km * T::NM + ez_class_index<Q, a>()) * T::CELLS + t - D::ey * T::EX - D::ex] = v;
+            }
+          });
+        }
       }
       // the next plane's loads go out AFTER this plane's collision and shared-memory stores (measured: issued before
       // the collision, 512^3 falls from 33.6 to 24.4 GLUPS) and have the barrier and stage 2 to arrive
@@ -1106,7 +1137,7 @@ __global__ void __launch_bounds__(Ab2Tile<Q, TX, TY, ONEBAR, BC == BC_WALLS>::TH
           f[a] = *r;
         });
       };
-      if (plane_walls(q)) gather2(IC<1>{});
+      if (!ZGHOST && plane_walls(q)) gather2(IC<1>{});
       else gather2(IC<0>{});
       collide<Q, EQ, BC, FORCE>(f, p, c, c2xy + p.nx * p.ny * q, q);
       double* out = dst + (o2 + q * p.zs);

@@ -57,6 +57,7 @@ def schemes(lbm):
 FACE_CASES = {
     "periodic": ([P] * 6, None),
     "channel_z": ([P, P, P, P, B, B], None),
+    "couette_z": ([P, P, P, P, B, M], {5: (0.05, 0.02, 0.0)}),
     "cavity": ([B, B, B, B, B, M], {5: (0.1, 0.0, 0.0)}),
     "mixed": ([B, M, P, P, M, B], {1: (0.0, 0.03, -0.02), 4: (0.05, 0.01, 0.0)}),
     "all_moving": ([M] * 6, {k: (0.01 * (k + 1), -0.02, 0.005 * k) for k in range(6)}),
@@ -648,21 +649,23 @@ def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq
 
 
 @pytest.mark.parametrize("dims", [(16, 8, 4), (48, 16, 21), (40, 27, 19), (17, 9, 35), (96, 40, 50)])
+@pytest.mark.parametrize("faces", ["periodic", "channel_z", "couette_z"])
 @pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
-def test_two_step_kernel_d3q27(lbm, dims, eq, forced):
-    """The same for D3Q27, periodic boxes: 16 x 8 tiles, two barriers per plane (1 / 2 / 3 slots per e_z class), no
-    prefetch, two blocks per SM."""
-    _two_step_case(lbm, 27, dims, "periodic", eq, forced)
+def test_two_step_kernel_d3q27(lbm, dims, faces, eq, forced):
+    """The same for D3Q27: 16 x 8 tiles, two barriers per plane (1 / 2 / 3 slots per e_z class), no prefetch, two blocks
+    per SM — periodic boxes, and boxes with z walls (bounce-back, moving) whose x and y faces are periodic: there the
+    walls act through ghost planes that stage 1 fills (BJ config 5's boundary set)."""
+    _two_step_case(lbm, 27, dims, faces, eq, forced)
 
 
-@pytest.mark.parametrize("faces", ["channel_z", "cavity"])
-def test_two_step_mode_leaves_d3q27_with_walls_to_the_one_step_kernel(lbm, faces):
-    """D3Q27 with wall faces has no two-step kernel (measured: no gain): lbm_step falls back to one launch per step."""
+@pytest.mark.parametrize("faces", ["cavity", "mixed"])
+def test_two_step_mode_leaves_d3q27_with_xy_walls_to_the_one_step_kernel(lbm, faces):
+    """D3Q27 with walls in x or y has no two-step kernel (measured: no gain): lbm_step falls back to one launch per step."""
     _two_step_case(lbm, 27, (48, 16, 21), faces, EQ_STANDARD, True, pairs=False)
 
 
 @pytest.mark.parametrize("Q", [19, 27])
-@pytest.mark.parametrize("faces", ["periodic", "cavity", "mixed"])
+@pytest.mark.parametrize("faces", ["periodic", "cavity", "mixed", "couette_z"])
 def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces, Q):
     """The same bit-for-bit comparison where every SM runs blocks of stream_collide_ab2 at once and warps of a block drift
     apart between its barriers (320 x 192 x 96 = 5.9 M cells, 1440 blocks in 6 z-chunks, 40 steps): a hazard between
