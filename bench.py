@@ -496,7 +496,7 @@ def main():
     ap.add_argument("--layout", default="rows", choices=["rows", "soa"],
                     help="internal population layout: f[z][y][a][x] (default) or plain structure of arrays f[a][z][y][x]")
     ap.add_argument("--two-step", type=int, default=1, choices=[0, 1],
-                    help="0: one pass through HBM per step everywhere (lbm_set_two_step(h, 0)); default 1: periodic D3Q19 fp64 A/B takes two steps per pass")
+                    help="lbm_set_two_step: 0 one pass through HBM per step everywhere; 1 (default) fp64 A/B without a mask takes two steps per pass where the grid is large enough")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--repeats", type=int, default=0,
                     help="timed segments of --steps steps each, the median is reported (default: 5, fewer if 5 would exceed a minute)")

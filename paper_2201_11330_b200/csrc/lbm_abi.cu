@@ -87,7 +87,7 @@ struct lbm_handle_s {
   int n_ipc_opened;
   int l2_bytes;       // L2 cache size of the device (0 = unknown)
   int persistent;     // lbm_step may take all steps of a call in one cooperative launch (small grids; lbm_set_persistent)
-  int two_step;       // lbm_step takes steps in pairs through stream_collide_ab2 where that kernel exists (lbm_set_two_step)
+  int two_step;       // lbm_step takes steps in pairs through stream_collide_ab2: 0 never, 1 where it pays (default), 2 wherever it exists
   int bx, by;         // block shape of the fused kernel (lbm_set_block), 0,0 = default_block()
   int fbx;            // row width (power of two <= 256) of the row-wise sweeps off the per-step path
   size_t elem() const { return f32 ? 4 : 8; }
@@ -947,7 +947,7 @@ int lbm_step(lbm_handle h, int nsteps) {
   for (int s = 0; s < nsteps;) {
     if (pairs && s + 2 <= nsteps) {
       bool ok = false;
-      LBM_Q_CALL_RET(h, ok, launch_step_ab2, c, h->buf[h->cur], h->buf[h->cur ^ 1]);
+      LBM_Q_CALL_RET(h, ok, launch_step_ab2, c, h->buf[h->cur], h->buf[h->cur ^ 1], h->two_step == 2);
       if (ok) {
         h->cur ^= 1;
         ++h->launches;
@@ -1075,7 +1075,8 @@ int lbm_set_persistent(lbm_handle h, int on) {
 
 int lbm_set_two_step(lbm_handle h, int on) {
   if (!h) return fail(LBM_EINVAL, "lbm_set_two_step: NULL handle");
-  h->two_step = on ? 1 : 0;
+  if (on < 0 || on > 2) return fail(LBM_EINVAL, "lbm_set_two_step: on must be 0, 1 or 2");
+  h->two_step = on;
   return LBM_OK;
 }
 

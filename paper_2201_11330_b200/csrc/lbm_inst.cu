@@ -218,7 +218,7 @@ struct Ab2Pick {
 }  // namespace
 
 template <>
-bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst) {
+bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst, bool always) {
   // fp64 storage, no link mask, whole box.  D3Q19: 32 x 8 tiles, one block of 352 threads per SM, one barrier per plane,
   // register prefetch of the next plane (512^3 periodic: 22.5 -> 33.6 GLUPS in one launch; z walls + forcing 22.5 -> 26.7).
   // D3Q27 keeps 27 populations of three planes: 16 x 8 tiles, two blocks of 192 threads per SM, two barriers per plane
@@ -273,6 +273,13 @@ bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst) {
             if (chunks < 1) chunks = 1;
             const int zchunk = (int)((c.p.nz + chunks - 1) / chunks);
             const dim3 grid((c.p.nx + TX - 1) / TX, (c.p.ny + TY - 1) / TY, (c.p.nz + zchunk - 1) / zchunk);
+            // Too few blocks: the last (or only) wave leaves SMs idle and ragged tiles waste lanes — measured with the
+            // one-step kernel at 18.8 / 19.6 / 20.5 GLUPS: 80^3 (150 blocks) 15.3, 88^3 (165) 18.9, 96^3 (216) 24.3, 128^3
+            // (512) 28.6.  Below 1.4 waves the one-step kernel takes the steps.
+            if (!always && 10LL * grid.x * grid.y * grid.z < 14LL * resident) {
+              ok = false;
+              return;
+            }
             kernel<<<grid, T::THREADS, T::SMEM_BYTES, c.stream>>>((const double*)src, (double*)dst, zchunk, c.p);
           }
         });

@@ -28,8 +28,9 @@ template <int Q> void launch_step_ab_slab_sym(const Ctx& c, const void* src, voi
 // all nsteps in one cooperative launch (b0 = current buffer); false = the grid does not fit the device at once
 template <int Q> bool launch_step_ab_persistent(const Ctx& c, void* b0, void* b1, int nsteps);
 template <int Q> bool launch_step_aa_persistent(const Ctx& c, void* buf, int nsteps, int phase);
-// TWO steps in one pass through HBM (stream_collide_ab2); false = this handle has no such kernel (use two single steps)
-template <int Q> bool launch_step_ab2(const Ctx& c, const void* src, void* dst);
+// TWO steps in one pass through HBM (stream_collide_ab2); false = this handle has no such kernel, or — unless `always` —
+// the grid gives it too few blocks to pay (use two single steps)
+template <int Q> bool launch_step_ab2(const Ctx& c, const void* src, void* dst, bool always);
 template <int Q> void launch_step_aa_even(const Ctx& c, void* buf);
 template <int Q> void launch_step_aa_odd(const Ctx& c, void* buf);
 template <int Q> void launch_export(const Ctx& c, int mode, const void* buf, double* out);

@@ -315,7 +315,8 @@ def lbm_set_persistent(h, on):
 
 
 def lbm_set_two_step(h, on):
-    _check(load().lbm_set_two_step(h, 1 if on else 0))
+    """0: never; 1 (default): where it pays; 2: wherever stream_collide_ab2 exists."""
+    _check(load().lbm_set_two_step(h, int(on)))
 
 
 # ---- convenience wrapper ----------------------------------------------------------------

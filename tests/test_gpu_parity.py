@@ -618,7 +618,7 @@ def _two_step_case(lbm, Q, dims, faces, eq, forced, pairs=True):
     ref = o.get_f()
     o.close()
     out = []
-    for on in (1, 0):
+    for on in (2, 0):  # 2: the two-step kernel on any grid it exists for (the default, 1, leaves small grids to the one-step kernel)
         s = lbm.Solver(nx, ny, nz, Q, 0.57, eq=eq_flag(lbm, eq), scheme=lbm.LBM_SCHEME_AB, face_kind=kinds, face_u=fu, force=force)
         s.set_persistent(0)  # (these grids would otherwise run in the persistent kernel)
         s.set_two_step(on)
@@ -691,3 +691,24 @@ def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces, Q):
     assert out[0][1][7] == 0
     if faces != "mixed":
         assert abs(out[0][1][0] - d0[0]) <= 1e-12 * d0[0]  # mass: the lid's +- links cancel (R6)
+
+
+def test_two_step_default_leaves_small_grids_to_the_one_step_kernel(lbm):
+    """lbm_set_two_step's default (1) takes steps in pairs only where the grid gives stream_collide_ab2 at least 1.4 waves of
+    blocks (measured: 80^3 = 150 blocks is slower in pairs, 96^3 = 216 faster); 2 forces it, 0 switches it off."""
+    for n, paired in ((80, False), (128, True)):
+        s = lbm.Solver(n, n, n, 19, 0.6, scheme=lbm.LBM_SCHEME_AB)
+        s.set_persistent(0)
+        s.init_equilibrium()
+        for mode, expect in ((1, 5 if paired else 10), (2, 5), (0, 10)):
+            s.set_two_step(mode)
+            l0 = s.launches
+            s.step(10)
+            assert s.launches - l0 == expect, (n, mode, s.launches - l0)
+        s.close()
+    with pytest.raises(lbm.LBMError):
+        s = lbm.Solver(16, 16, 16, 19, 0.6)
+        try:
+            s.set_two_step(3)
+        finally:
+            s.close()
