@@ -942,7 +942,7 @@ __global__ void __launch_bounds__(kF32x2Threads, 5) stream_collide_ab_f32x2(cons
 }
 
 // ---------------------------------------------------------------------------------------
-// Two time steps per pass through HBM (A/B scheme, BC_PERIODIC, fp64).  The one-step kernel above sits at the ceiling of
+// Two time steps per pass through HBM (A/B scheme, fp64, BC_PERIODIC / BC_WALLS).  The one-step kernel above sits at the ceiling of
 // its access pattern (every population read once and written once per step: 0.999 x algorithmic DRAM bytes at 1.05 x the
 // device-copy bandwidth), so more lattice updates per second means fewer bytes per update.  A block owns a TX x TY
 // column of the box and marches along z.  Per plane it runs
@@ -953,10 +953,13 @@ __global__ void __launch_bounds__(kF32x2Threads, 5) stream_collide_ab_f32x2(cons
 // What stage 2 pulls from plane q-1 are the e_z = +1 populations only, from plane q the e_z = 0 ones and from plane q+1
 // the e_z = -1 ones, so a plane's stage-1 result is kept per class for exactly as long as it is needed: the e_z = -1
 // class for the rest of the iteration that made it, e_z = 0 for one more iteration (2 slots), e_z = +1 for two more
-// (3 slots) — 38 population planes of the extended tile for D3Q19 instead of 3 x 19.  HBM traffic per TWO steps: one read
+// (3 slots) — 38 population planes of the extended tile for D3Q19 instead of 3 x 19 — when a second barrier follows
+// stage 2; one slot more per class (57 planes) lets ONE barrier per plane do (Ab2Tile).  HBM traffic per TWO steps: one read
 // of the extended tile (the rim is shared with the neighbouring blocks through the L2) and one write of the tile,
-// against two reads and two writes; the price is (TX+2)(TY+2)/(TX TY) collisions in stage 1 and two block barriers per plane.
+// against two reads and two writes; the price is (TX+2)(TY+2)/(TX TY) collisions in stage 1 and the block barriers.
 // Same arithmetic per cell as ab_cell (collide): bit-identical to two launches of stream_collide_ab.
+// Measured (lbm_inst.cu picks the variant): D3Q19 32 x 8 tiles, one barrier, register prefetch, one block per SM:
+// 512^3 22.5 -> 33.6 GLUPS in one launch, 31.4 sustained; D3Q27 16 x 8, two barriers, two blocks: 400^3 15.8 -> 21.0.
 template <int Q, int EZ>
 __host__ __device__ constexpr int ez_class_size() {
   int n = 0;
@@ -972,7 +975,7 @@ __host__ __device__ constexpr int ez_class_index() {  // position of direction A
 
 // ONEBAR: one more slot per class (2 / 3 / 4), so that stage 1 of the next plane never writes a slot stage 2 of this plane
 // still reads and ONE block barrier per plane is enough.  PREFETCH: the stage-1 loads of the next plane are issued
-// before stage 2 of this one, so that their latency is covered by it (19 more registers pairs).
+// before stage 2 of this one, so that their latency is covered by it (Q more register pairs).
 template <int Q, int TX, int TY, bool ONEBAR, bool WALLS = false>
 struct Ab2Tile {
   static constexpr int EX = TX + 2, EY = TY + 2, CELLS = EX * EY;  // stage-1 tile
