@@ -229,7 +229,9 @@ int lbm_set_persistent(lbm_handle h, int on);
 int lbm_set_two_step(lbm_handle h, int on);
 
 /* Tuning knob for measurements: CUDA block shape (threads along x, along y) of the
- * stream-collide kernel; 0,0 restores the default.  bx*by must be <= 256 and a multiple of 32. */
+ * stream-collide kernel; 0,0 restores the default.  bx*by must be <= 256 and a multiple of 32.
+ * The kernels with a fixed thread-to-cell mapping keep their own shape: two steps per pass (lbm_set_two_step), the
+ * in-place odd phase without a mask (one grid row per block), fp32 storage with two cells per thread. */
 int lbm_set_block(lbm_handle h, int bx, int by);
 
 /* ---------------------------------------------------------------------------------------------
