@@ -161,3 +161,36 @@ def test_config1_tgv128_fp32_storage_full_length(lbm):
         rel = float((np.abs(got - ref) / np.abs(ref)).max())
         print(f"\ncfg1 fp32 storage, scheme {sch >> 12}: max relative |df| = {rel:.2e}")
         assert rel <= 2e-5
+
+
+@pytest.mark.parametrize("name", ["periodic_q19", "cavity_q19", "channel_q27"])
+def test_two_steps_per_pass_equal_single_steps_over_a_long_run(lbm, name):
+    """Soak test of stream_collide_ab2's shared-memory hand-over (stage 1 of plane k+1 may overlap stage 2 of plane k; the
+    ghost planes of the D3Q27 channel): 400 steps on 256 x 256 x 128 cells — every SM busy, thousands of barrier
+    crossings per block — must give the same bits as 400 launches of the one-step kernel, and conserve mass."""
+    B, M, P = inputs.FACE_BOUNCE, inputs.FACE_MOVING, inputs.FACE_PERIODIC
+    lid = tuple((0.0, 0.0, 0.0) for _ in range(5)) + ((0.1, 0.0, 0.0),)
+    w = {
+        "periodic_q19": inputs.Workload("soak_p", 256, 256, 128, 19, 0.52, 400, u0=0.04, noise=1e-4, seed=inputs.SEED_BASE + 41),
+        "cavity_q19": inputs.Workload("soak_c", 256, 256, 128, 19, 0.55, 400, face_kind=(B, B, B, B, B, M), face_u=lid, noise=1e-4,
+                                      seed=inputs.SEED_BASE + 42, kind="rest"),
+        "channel_q27": inputs.Workload("soak_q27", 256, 256, 128, 27, 0.9, 400, face_kind=(P, P, P, P, B, B), force=(1e-6, 0.0, 0.0),
+                                       noise=1e-4, seed=inputs.SEED_BASE + 43, kind="rest"),
+    }[name]
+    rho, u = w.fields()
+    rho_d = torch.from_numpy(rho).cuda()
+    u_d = torch.from_numpy(np.ascontiguousarray(u.reshape(-1))).cuda()
+    out = []
+    for mode in (1, 0):
+        s = lbm.Solver.from_workload(w, scheme=lbm.LBM_SCHEME_AB)
+        s.set_two_step(mode)
+        s.init_equilibrium(rho_d, u_d)
+        d0 = s.diagnostics()
+        l0 = s.launches
+        s.step(w.steps)
+        launches = s.launches - l0
+        out.append((s.get_populations().clone(), s.diagnostics(), launches))
+        s.close()
+    assert out[0][2] == w.steps // 2 and out[1][2] == w.steps
+    assert torch.equal(out[0][0], out[1][0])
+    assert abs(out[0][1][0] - d0[0]) <= 1e-11 * d0[0] and out[0][1][7] == 0
