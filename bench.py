@@ -336,7 +336,9 @@ def run_gpu(args, w):
     # grids, all K for the small ones that run in the persistent kernel)
     achieved = bytes_per_cell * w.N * K / secs / 1e9
     peak, peak_src = measured_peak()
-    traffic, traffic_src = ncu_traffic(w.name, args.scheme + ("2" if 2 * launches == K else "") + ("" if args.store == "f64" else "_f32"))
+    # steps in pairs (stream_collide_ab2; an odd K ends with one single step) vs all K in one launch of the persistent kernel
+    paired = K > 2 and 2 * launches in (K, K + 1)
+    traffic, traffic_src = ncu_traffic(w.name, args.scheme + ("2" if paired else "") + ("" if args.store == "f64" else "_f32"))
     out = {
         "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -357,10 +359,10 @@ def run_gpu(args, w):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                      "traffic_source": traffic_src,
                      "frac_note": (("above 1: `achieved` counts the ALGORITHMIC bytes of one-step-per-pass streaming (2*Q*8 B per update, SURVEY.md 8d); "
-                                    "this kernel takes two steps per pass and moves about half of them (see `traffic`)") if 2 * launches == K else
+                                    "this kernel takes two steps per pass and moves about half of them (see `traffic`)") if paired else
                                    ("above 1: the contract's denominator is a plain device copy (MEASURED_PEAKS.json), not a hardware limit; "
                                     "see frac_of_nominal_8TBs")) if achieved > peak else None,
-                     "kernel": "stream_collide_" + args.scheme + ("2 (two steps per launch)" if 2 * launches == K else "_persistent" if launches < K else ""), "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch, "steps_per_launch": K / launches,
+                     "kernel": "stream_collide_" + args.scheme + ("2 (two steps per launch)" if paired else "_persistent" if launches < K else ""), "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch, "steps_per_launch": K / launches,
                      "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
         "checks": {"mass_drift_rel": abs(d_end[0] - d_init[0]) / d_init[0], "nonfinite_cells": d_end[7],
                    "kinetic_energy_ratio": d_end[4] / d_init[4] if d_init[4] else None, "e2e_mass": d_e2e[0]},
