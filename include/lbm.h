@@ -223,7 +223,7 @@ int lbm_set_persistent(lbm_handle h, int on);
  * (any z faces of those kinds) — lbm_step(h, n) takes the steps in pairs: one kernel runs step t on a tile extended by one cell, keeps the result in shared memory and
  * runs step t+1 from there, so that every population is read from HBM once and written once per TWO steps.  Same
  * arithmetic per cell, same results bit for bit as single steps; an odd n ends with one single step.  on = 1 (default):
- * where it pays — grids that give the kernel at least 1.4 waves of blocks (from about 96^3 up); on = 2: wherever the
+ * where it pays — grids that give the kernel at least 1.4 waves of blocks (from about 80^3 up); on = 2: wherever the
  * kernel exists (tests); on = 0: never (one pass per step, as for every other variant).  Grids small enough for the
  * persistent kernel (lbm_set_persistent) keep using that one. */
 int lbm_set_two_step(lbm_handle h, int on);

@@ -265,17 +265,27 @@ bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst, bool always) 
               ok = false;
               return;
             }
-            // z-chunks: enough blocks for ~16 waves (the tail of the last wave stays below a few percent), chunks of at
-            // least 16 planes (every chunk runs stage 1 on two planes more than it stores)
+            // z-chunks.  Every chunk runs stage 1 on two planes more than it stores (stage 1 is about 55 % of a plane's
+            // work: a chunk of zc planes costs zc + 1.1), and the last wave of blocks leaves SMs idle unless the block count
+            // is close to a multiple of what the device holds: take the chunk count that loses least to both.
             const long long tiles = (long long)((c.p.nx + TX - 1) / TX) * ((c.p.ny + TY - 1) / TY);
-            long long chunks = (16LL * resident + tiles - 1) / tiles;
-            if (chunks > c.p.nz / 16) chunks = c.p.nz / 16;
-            if (chunks < 1) chunks = 1;
-            const int zchunk = (int)((c.p.nz + chunks - 1) / chunks);
+            int zchunk = c.p.nz;
+            double best = 0.0;
+            for (int n = 1; n <= 64 && n * 8 <= c.p.nz; ++n) {
+              const int zc = (c.p.nz + n - 1) / n;
+              const long long blocks = tiles * ((c.p.nz + zc - 1) / zc);
+              const double waves = (double)blocks / resident;
+              // (+ 0.25 wave: blocks do not all take the same time, so a nearly full last wave still costs)
+              const double eff = waves / ((double)((blocks + resident - 1) / resident) + 0.25) * zc / (zc + 1.1);
+              if (eff > best * 1.002) {  // (ties go to fewer, longer chunks)
+                best = eff;
+                zchunk = zc;
+              }
+            }
             const dim3 grid((c.p.nx + TX - 1) / TX, (c.p.ny + TY - 1) / TY, (c.p.nz + zchunk - 1) / zchunk);
-            // Too few blocks: the last (or only) wave leaves SMs idle and ragged tiles waste lanes — measured with the
-            // one-step kernel at 18.8 / 19.6 / 20.5 GLUPS: 80^3 (150 blocks) 15.3, 88^3 (165) 18.9, 96^3 (216) 24.3, 128^3
-            // (512) 28.6.  Below 1.4 waves the one-step kernel takes the steps.
+            // Too few blocks: the only wave or two leave SMs idle and ragged tiles waste lanes.  Measured, one-step /
+            // two-step GLUPS: 72^3 (135 blocks) 18.1 / 19.2 at best, 80^3 (300 blocks of 8 planes) 18.8 / 22.7, 88^3 19.6 / 24.7,
+            // 96^3 20.5 / 28.6, 128^3 21.8 / 29.1.  Below 1.4 waves the one-step kernel takes the steps.
             if (!always && 10LL * grid.x * grid.y * grid.z < 14LL * resident) {
               ok = false;
               return;

@@ -695,8 +695,9 @@ def test_two_step_kernel_on_a_grid_that_fills_the_device(lbm, faces, Q):
 
 def test_two_step_default_leaves_small_grids_to_the_one_step_kernel(lbm):
     """lbm_set_two_step's default (1) takes steps in pairs only where the grid gives stream_collide_ab2 at least 1.4 waves of
-    blocks (measured: 80^3 = 150 blocks is slower in pairs, 96^3 = 216 faster); 2 forces it, 0 switches it off."""
-    for n, paired in ((80, False), (128, True)):
+    blocks (64^3 gives at most 128 blocks of 32 x 8 x 8 cells: one-step kernel; 128^3 gives 576); 2 forces it, 0 switches it
+    off."""
+    for n, paired in ((64, False), (128, True)):
         s = lbm.Solver(n, n, n, 19, 0.6, scheme=lbm.LBM_SCHEME_AB)
         s.set_persistent(0)
         s.init_equilibrium()
