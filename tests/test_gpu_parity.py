@@ -62,6 +62,13 @@ FACE_CASES = {
     "mixed": ([B, M, P, P, M, B], {1: (0.0, 0.03, -0.02), 4: (0.05, 0.01, 0.0)}),
     "all_moving": ([M] * 6, {k: (0.01 * (k + 1), -0.02, 0.005 * k) for k in range(6)}),
 }
+# open faces (D:R22: velocity inlet, pressure outlet at the default density 1) for the two-step kernel's tests
+PR = inputs.FACE_PRESSURE
+OPEN_CASES = {
+    "inlet_outlet_x": ([M, PR, B, B, P, P], {0: (0.04, 0.0, 0.0)}),
+    "inlet_outlet_z": ([P, P, P, P, M, PR], {4: (0.0, 0.01, 0.03)}),
+}
+FACE_CASES_TWO_STEP = dict(FACE_CASES, **OPEN_CASES)
 
 
 def face_u_of(spec):
@@ -607,7 +614,7 @@ def test_persistent_kernel_equals_one_launch_per_step(lbm, scheme):
 def _two_step_case(lbm, Q, dims, faces, eq, forced, pairs=True):
     nx, ny, nz = dims
     N = nx * ny * nz
-    kinds, uspec = FACE_CASES[faces]
+    kinds, uspec = FACE_CASES_TWO_STEP[faces]
     fu = face_u_of(uspec)
     force = (1e-5, -2e-6, 3e-6) if forced else None
     f0 = random_f(Q, N, seed=nx + ny + nz + Q)
@@ -637,7 +644,7 @@ def _two_step_case(lbm, Q, dims, faces, eq, forced, pairs=True):
 
 
 @pytest.mark.parametrize("dims", [(32, 8, 4), (64, 16, 21), (40, 27, 19), (33, 9, 35), (96, 40, 50), (65, 17, 9), (128, 25, 12)])
-@pytest.mark.parametrize("faces", list(FACE_CASES))
+@pytest.mark.parametrize("faces", list(FACE_CASES_TWO_STEP))
 @pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
 def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq, forced):
     """stream_collide_ab2 (two time steps per pass through HBM: stage 1 on a tile extended by one cell into shared memory,
@@ -649,7 +656,7 @@ def test_two_step_kernel_equals_single_steps_and_the_oracle(lbm, dims, faces, eq
 
 
 @pytest.mark.parametrize("dims", [(16, 8, 4), (48, 16, 21), (40, 27, 19), (17, 9, 35), (96, 40, 50)])
-@pytest.mark.parametrize("faces", ["periodic", "channel_z", "couette_z"])
+@pytest.mark.parametrize("faces", ["periodic", "channel_z", "couette_z", "inlet_outlet_z"])
 @pytest.mark.parametrize("eq,forced", [(EQ_STANDARD, False), (EQ_STANDARD, True), (EQ_INCOMP, False), (EQ_INCOMP, True)])
 def test_two_step_kernel_d3q27(lbm, dims, faces, eq, forced):
     """The same for D3Q27: 16 x 8 tiles, two barriers per plane (1 / 2 / 3 slots per e_z class), no prefetch, two blocks
