@@ -182,6 +182,36 @@ int lbm_moments(lbm_handle h, double* rho, double* u, double* diagnostics);
  * to the neighbours' next step); on a z-slab handle only the own planes of the host arrays are written. */
 int lbm_moments_host(lbm_handle h, double* rho_host, double* u_host, double* diagnostics);
 
+/* The 8 diagnostics of lbm_moments (P:295-304 PostProcessing, P:404-427 Monitor; Eq. 8-9) WITHOUT a handle
+ * and WITHOUT allocating anything — for callers that must not call cudaMalloc:
+ *   - a process whose device memory is owned outright by a pool of its own (torch's caching allocator, a solver that
+ *     sizes its arrays to the card): an allocation made behind the pool's back fails, or takes the room the next
+ *     time step needs;
+ *   - a monitor inside a running time loop: cudaMalloc / cudaFree synchronise the whole device and would stall the
+ *     other streams of the loop;
+ *   - code that only holds a pointer to populations somebody else owns (a checkpoint, another solver's arrays) and
+ *     has no handle — lbm_create allocates.
+ * lbm_moments keeps the per-block records of its two-pass reduction in memory lbm_create allocated; this entry point
+ * runs the same reduction (same per-cell arithmetic, same non-finite rule, same 8 outputs) with the records in a
+ * fixed 2 MiB `static __device__` array inside the library.  It calls no cudaMalloc, cudaFree or allocating routine.
+ *   f           DEVICE, Q*ncells doubles, canonical populations f[a*ncells + i] (what lbm_get_populations returns;
+ *               no solid mask: every cell counts), read only, caller-owned;
+ *   ncells      1 <= ncells <= LBM_STATIC_MAX_CELLS (2^27 = 512^3), else LBM_EINVAL — the array holds one record
+ *               per 4096 cells and cannot grow; larger grids go through lbm_moments on a handle;
+ *   lattice     LBM_D2Q9 / LBM_D3Q19 / LBM_D3Q27, optionally | LBM_EQ_INCOMP; any other bit: LBM_EINVAL;
+ *   force       HOST pointer to the 3 doubles of the body force F (u includes the F/2 shift, D:R7) or NULL = 0;
+ *   diagnostics DEVICE, 8 doubles, written by the call (same order and meaning as lbm_moments), caller-owned;
+ *   stream      cudaStream_t the two kernels are enqueued on (NULL = legacy default stream).  Asynchronous.
+ * The cost of the fixed array: its 2 MiB stay resident on every GPU that loads this library, until the process exits.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress; once per device, cached) — make
+ *   that first call at start-up, before any stream capture is begun.  After cudaDeviceReset the cached address is stale.
+ * Sharing: every call on a device uses the same array, and the array keeps the previous call's records.  That needs
+ *   no clearing (pass 1 overwrites every record pass 2 reads), but two calls that can overlap on the GPU — different
+ *   streams with no event between them — race and both results are wrong.  Keep the calls of one device on one stream
+ *   or order them.  Block records always cover the same 4096 cells, so the result does not depend on the SM count. */
+enum { LBM_STATIC_MAX_CELLS = 1 << 27 };
+int lbm_diagnostics_static(const double* f, int64_t ncells, int lattice, const double* force, double* diagnostics, void* stream);
+
 /* Canonical populations f[a*N+i] (Q*N doubles, device): export / import.  Not on the hot path
  * (tests, checkpointing).  lbm_set_populations does not change the step counter. */
 int lbm_get_populations(lbm_handle h, double* f);

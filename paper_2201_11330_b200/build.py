@@ -2,7 +2,7 @@
 
 `python -m paper_2201_11330_b200.build [--force] [--verbose] [--ptxas]`.  nvcc cross-compiles
 without a GPU.  The kernel instantiations (csrc/lbm_inst.cu) are compiled once per lattice and
-part into separate objects, in parallel, then linked with the C ABI (csrc/lbm_abi.cu).  The .so
+part into separate objects, in parallel, then linked with the C ABI (csrc/lbm_abi.cu, csrc/lbm_static.cu).  The .so
 is built in-tree (git-ignored) so that it travels to the GPU box with the repo.
 """
 from __future__ import annotations
@@ -18,7 +18,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbm_b200.so")
-DEPS = ["lbm_abi.cu", "lbm_inst.cu", "lbm_kernels.cuh", "lbm_launch.cuh", os.path.join(ROOT, "include", "lbm.h")]
+DEPS = ["lbm_abi.cu", "lbm_inst.cu", "lbm_static.cu", "lbm_kernels.cuh", "lbm_launch.cuh", os.path.join(ROOT, "include", "lbm.h")]
 LATTICES = (9, 19, 27)
 PARTS = (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10)  # A/B step, AA even, AA odd, export/import/init/geometry, moments/force, A/B slab step,
                                   # A/B step with SYMMETRY faces, A/B slab step with SYMMETRY faces, persistent A/B kernel, persistent AA kernel,
@@ -52,7 +52,8 @@ def needs_build() -> bool:
 
 def _units():
     """(object path, source, extra defines) of every translation unit."""
-    units = [(os.path.join(OBJ, "lbm_abi.o"), os.path.join(CSRC, "lbm_abi.cu"), [])]
+    units = [(os.path.join(OBJ, "lbm_abi.o"), os.path.join(CSRC, "lbm_abi.cu"), []),
+             (os.path.join(OBJ, "lbm_static.o"), os.path.join(CSRC, "lbm_static.cu"), [])]  # lbm_diagnostics_static
     for q in LATTICES:
         for part in PARTS:
             units.append((os.path.join(OBJ, f"lbm_inst_q{q}_p{part}.o"), os.path.join(CSRC, "lbm_inst.cu"),

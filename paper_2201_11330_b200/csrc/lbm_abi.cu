@@ -41,6 +41,11 @@ constexpr size_t kChunkBytes = 64u << 20;  // ... each at least this many bytes 
 
 }  // namespace
 
+namespace lbm {
+// for the library's other translation units (lbm_static.cu): leave a message for lbm_last_error() on this thread
+void set_last_error(const std::string& msg) { g_err = msg; }
+}  // namespace lbm
+
 struct lbm_handle_s {
   int nx, ny, nz, Q, eq, scheme, f32;
   int soa;            // LBM_LAYOUT_SOA: plain structure of arrays instead of the row-interleaved layout

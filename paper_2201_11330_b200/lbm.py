@@ -21,6 +21,7 @@ LBM_LAYOUT_ROWS, LBM_LAYOUT_SOA = 0, 1 << 20
 LBM_FACE_PERIODIC, LBM_FACE_BOUNCE, LBM_FACE_MOVING, LBM_FACE_PRESSURE, LBM_FACE_SYMMETRY = 0, 1, 2, 3, 4
 LBM_WALL_HALFWAY, LBM_WALL_NODAL = 0, 1
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_EUNSUPPORTED = 0, -1, -2, -3, -4
+LBM_STATIC_MAX_CELLS = 1 << 27  # largest grid lbm_diagnostics_static accepts (its scratch array is fixed)
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblbm_b200.so")
 
@@ -32,7 +33,7 @@ SYMBOLS = (
     "lbm_set_geometry", "lbm_set_geometry_host", "lbm_boundary_force",
     "lbm_set_face_velocity", "lbm_set_face_velocity_host", "lbm_set_face_density",
     "lbm_create_slab", "lbm_slab_export", "lbm_slab_connect", "lbm_slab_set_sync",
-    "lbm_debug_arm", "lbm_debug_check",
+    "lbm_debug_arm", "lbm_debug_check", "lbm_diagnostics_static",
 )
 
 
@@ -133,6 +134,8 @@ def load():
     lib.lbm_debug_arm.argtypes = [vp, i32]
     lib.lbm_debug_check.restype = i64
     lib.lbm_debug_check.argtypes = [vp]
+    lib.lbm_diagnostics_static.restype = i32
+    lib.lbm_diagnostics_static.argtypes = [dp, i64, i32, C.c_void_p, dp, vp]
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_last_error.argtypes = []
     _lib = lib
@@ -269,6 +272,24 @@ def lbm_moments_host(h, rho=None, u=None, diagnostics=False):
     diag = np.empty(8) if diagnostics else None
     _check(load().lbm_moments_host(h, _ptr(rho, device="cpu"), _ptr(u, device="cpu"), None if diag is None else diag.ctypes.data))
     return diag
+
+
+def lbm_diagnostics_static(f, lattice, out, force=None, stream=None):
+    """The 8 diagnostics of `lbm_moments` for callers that may not allocate device memory and have no handle (a
+    process whose GPU memory belongs to its own pool, a monitor inside a time loop that a cudaMalloc would stall,
+    code that only holds a pointer to someone else's populations).  The library allocates nothing: its scratch is a
+    fixed array inside the library, which is why grids beyond LBM_STATIC_MAX_CELLS cells are refused and why two
+    calls that overlap on one GPU (different streams, no ordering) race.  See include/lbm.h.
+
+    f: contiguous float64 CUDA tensor, Q*ncells canonical populations f[a*ncells + i]; lattice: Q, optionally
+    | LBM_EQ_INCOMP; out: float64 CUDA tensor of 8 elements that receives the result (the caller passes it: this
+    function creates no tensor); force: 3 floats or None; stream: raw cudaStream_t (int) or None = default stream.
+    Asynchronous: read `out` after synchronising the stream."""
+    Q = int(lattice) & 0xFF
+    assert Q > 0 and f.numel() % Q == 0, (f.numel(), Q)
+    fo = None if force is None else np.ascontiguousarray(force, dtype=np.float64).reshape(3)
+    _check(load().lbm_diagnostics_static(_ptr(f), f.numel() // Q, int(lattice), None if fo is None else fo.ctypes.data,
+                                         _ptr(out, 8), None if stream is None else int(stream)))
 
 
 def lbm_get_populations(h, f):
