@@ -159,9 +159,10 @@ int lbm_boundary_force(lbm_handle h, double* F);
  * Under LBM_WALL_NODAL the wall nodes then satisfy Eq. 10 (D:R17). */
 int lbm_init_equilibrium(lbm_handle h, const double* rho, const double* u);
 /* Same with HOST pointers (pinned memory recommended).  The fields are copied in z-chunks on an internal copy stream
- * and chunk k is initialised on the handle's stream while chunk k+1 is still on the bus; the handle's stream waits for
- * every copy, so synchronising it (or any later synchronising call) also means the host arrays have been read.  On a
- * z-slab handle only the own planes of the arrays are read. */
+ * and chunk k is initialised on the handle's stream while chunk k+1 is still on the bus.  The call returns when the
+ * host arrays have been read in full — they may be freed, reused or overwritten at once (the copy stream is not
+ * visible to the caller, so nothing else could tell) — while the initialisation kernels of the last chunks may still
+ * be running on the handle's stream.  On a z-slab handle only the own planes of the arrays are read. */
 int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double* u_host);
 
 /* Advance nsteps >= 0 time steps: per step and cell, pull-stream (Eq. 7) with wall links

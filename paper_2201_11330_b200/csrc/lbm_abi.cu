@@ -912,7 +912,12 @@ int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double
     launch_init_rows(h, c, mode, d_rho, d_u, h->ny * zc[k], h->ny * zc[k + 1]);
   }
   finish_init(h);
-  return check_launch("init_equilibrium_host");
+  rc = check_launch("init_equilibrium_host");
+  // The copies run on a stream the caller cannot see, so the caller cannot know when the host arrays may be reused:
+  // wait here until the last chunk has left the host (the copy stream is in order, so that covers every chunk).  Only
+  // the copies are waited for; the initialisation kernels of the last chunks may still be running on return.
+  CUDA_TRY(cudaEventSynchronize(h->chunk_ev[n - 1]));
+  return rc;
 }
 
 int lbm_step(lbm_handle h, int nsteps) {

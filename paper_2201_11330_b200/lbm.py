@@ -409,6 +409,9 @@ class Solver:
         self._after(rho, u)
 
     def init_equilibrium_host(self, rho=None, u=None):
+        # Contract (include/lbm.h): the library returns once rho / u have left the host, so temporaries such as
+        # `x.pin_memory()` passed inline may be dropped by the caller right away — torch's pinned-memory cache can
+        # recycle their blocks without racing the library's internal copy stream.  No reference is kept here.
         lbm_init_equilibrium_host(self.h, rho, u)
 
     def step(self, n=1):

@@ -201,6 +201,31 @@ def test_host_entry_points_equal_device_ones(lbm, scheme):
     b.close()
 
 
+def test_host_arrays_may_be_reused_as_soon_as_init_returns(lbm):
+    """include/lbm.h: lbm_init_equilibrium_host returns when rho / u have left the host (its copy stream is internal, so
+    the caller could not wait for it).  Overwrite the pinned arrays the moment the call returns — 0.5 GB at 256^3, tens of
+    milliseconds on the bus — and the initial state must still be the one made from the original values."""
+    n = 256
+    N = n ** 3
+    g = torch.Generator(device="cuda")
+    g.manual_seed(7)
+    rho_d = 1.0 + 1e-3 * (torch.rand(N, dtype=torch.float64, device="cuda", generator=g) - 0.5)
+    u_d = 0.05 * (torch.rand(3 * N, dtype=torch.float64, device="cuda", generator=g) - 0.5)
+    rho_h = rho_d.cpu().pin_memory()
+    u_h = u_d.cpu().pin_memory()
+    a = lbm.Solver(n, n, n, 19, 0.6, scheme=lbm.LBM_SCHEME_AA)  # (one buffer each: 2.5 GB)
+    b = lbm.Solver(n, n, n, 19, 0.6, scheme=lbm.LBM_SCHEME_AA)
+    a.init_equilibrium(rho_d, u_d)
+    b.init_equilibrium_host(rho_h, u_h)
+    rho_h.fill_(float("nan"))  # the caller reuses its buffers at once
+    u_h.fill_(float("nan"))
+    fa = a.get_populations()
+    a.close()
+    fb = b.get_populations()
+    b.close()
+    assert bool(torch.isfinite(fb).all()) and torch.equal(fa, fb)
+
+
 def test_nonfinite_cells_are_counted(lbm):
     dims = (8, 8, 8)
     s = lbm.Solver(*dims, 19, 0.8)
