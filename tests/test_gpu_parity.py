@@ -745,3 +745,41 @@ def test_two_step_default_leaves_small_grids_to_the_one_step_kernel(lbm):
             s.set_two_step(3)
         finally:
             s.close()
+
+
+# fp32 storage: the two-cells-per-thread kernel against the one-cell kernel ------------------------------------------
+# D2Q9 lives in the x-y plane: its own face mixes (z faces periodic)
+FACE_CASES_F32_2D = {
+    "periodic": ([P] * 6, None),
+    "cavity": ([B, B, B, M, P, P], {3: (0.1, 0.0, 0.0)}),
+    "mixed": ([B, M, P, P, P, P], {1: (0.0, 0.03, 0.0)}),
+    "inlet_outlet_x": ([M, PR, B, B, P, P], {0: (0.04, 0.0, 0.0)}),
+}
+
+
+@pytest.mark.parametrize("forced", [False, True], ids=["unforced", "forced"])
+@pytest.mark.parametrize("faces", ["periodic", "cavity", "mixed", "inlet_outlet_x"])
+@pytest.mark.parametrize("Q", [19, 9])
+def test_fp32_two_cell_kernel_equals_one_cell_kernel(lbm, Q, faces, forced):
+    """stream_collide_ab_f32x2 (the default fp32 A/B kernel of every even-nx D3Q19 / D2Q9 box without a mask: two cells
+    per thread) claims the bits of the one-cell kernel.  The one-cell kernel is reached through an all-fluid solid mask
+    (the BC_GEO path, which test_returning_to_the_analytic_box shows to be bit-identical to the analytic box in fp64).
+    Random non-equilibrium f, so that a wrong wall, wrap or pair link at x = 0 / x = nx-2 cannot hide below a tolerance.
+    Row widths: nx = 2*bx exactly (64 with bx = 32; 256 with bx = 128), and nx that is not a multiple of 2*bx (70, 300)."""
+    kinds, uspec = (FACE_CASES_TWO_STEP if Q == 19 else FACE_CASES_F32_2D)[faces]
+    fu = face_u_of(uspec)
+    force = ((1e-5, -2e-6, 3e-6) if Q == 19 else (1e-5, -2e-6, 0.0)) if forced else None
+    for dims in ((64, 6, 5), (70, 5, 4), (256, 3, 3), (300, 4, 3)):
+        N = dims[0] * dims[1] * dims[2]
+        f0 = dev(random_f(Q, N, seed=Q + dims[0]).reshape(-1))
+        out = []
+        for one_cell in (False, True):
+            s = lbm.Solver(*dims, Q, 0.57, scheme=lbm.LBM_SCHEME_AB, store=lbm.LBM_STORE_F32, face_kind=kinds, face_u=fu, force=force)
+            if one_cell:
+                s.set_geometry(torch.zeros(N, dtype=torch.uint8, device="cuda"), lbm.LBM_WALL_HALFWAY)
+            s.set_populations(f0)
+            s.step(7)
+            out.append(s.get_populations().clone())
+            s.close()
+        assert bool(torch.isfinite(out[0]).all())
+        assert torch.equal(out[0], out[1]), (Q, faces, forced, dims, float((out[0] - out[1]).abs().max()))
