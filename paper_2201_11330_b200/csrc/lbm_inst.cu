@@ -5,6 +5,8 @@
 //            7 A/B step of a z-slab with SYMMETRY faces   8 persistent A/B kernel (all steps of a call in one launch)
 //            9 persistent in-place AA kernel   10 A/B, two steps per pass (stream_collide_ab2)
 // Each unit defines the launch_* specialisations of lbm_launch.cuh for its lattice.
+#include <atomic>
+
 #include "lbm_launch.cuh"
 
 #ifndef LBM_Q
@@ -242,25 +244,27 @@ bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst, bool always) 
             using P = Ab2Pick<Q_, decltype(bc)::value>;
             using T = typename P::T;
             auto kernel = stream_collide_ab2<Q_, decltype(eq)::value, decltype(bc)::value, decltype(force)::value != 0, P::TX, P::TY, P::MINB, P::ONEBAR, P::PREFETCH>;
-            static int resident_on[64] = {0};  // per device: blocks of this instantiation resident at once (0 = not asked yet)
+            // per device: blocks of this instantiation resident at once (0 = not asked yet, or to be asked again).  Atomic:
+            // handles driven from several host threads share it (they would all store the same value).
+            static std::atomic<int> resident_on[64];
             int dev = 0;
             if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
               cudaGetLastError();
               ok = false;
               return;
             }
-            if (resident_on[dev] == 0) {
+            if (resident_on[dev].load(std::memory_order_relaxed) == 0) {
               int sms = 0, per_sm = 0;
               if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
                   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
                   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, T::THREADS, T::SMEM_BYTES) != cudaSuccess || per_sm < 1) {
                 cudaGetLastError();
-                resident_on[dev] = -1;
+                resident_on[dev].store(-1, std::memory_order_relaxed);
               } else {
-                resident_on[dev] = per_sm * sms;
+                resident_on[dev].store(per_sm * sms, std::memory_order_relaxed);
               }
             }
-            const int resident = resident_on[dev];
+            const int resident = resident_on[dev].load(std::memory_order_relaxed);
             if (resident < 0) {
               ok = false;
               return;
@@ -291,6 +295,15 @@ bool launch_step_ab2<Q_>(const Ctx& c, const void* src, void* dst, bool always) 
               return;
             }
             kernel<<<grid, T::THREADS, T::SMEM_BYTES, c.stream>>>((const double*)src, (double*)dst, zchunk, c.p);
+            // A launch that was refused (after cudaDeviceReset or in a new context the opt-in shared-memory size above is
+            // gone while the cache still says "ready") must not count as two steps taken: report "not launched" so that
+            // lbm_step leaves cur / time alone and takes the steps with the one-step kernel, and ask again next time.
+            if (cudaPeekAtLastError() != cudaSuccess) {
+              cudaGetLastError();
+              resident_on[dev].store(0, std::memory_order_relaxed);
+              ok = false;
+              return;
+            }
           }
         });
       });
