@@ -4,14 +4,20 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
                     [--config i] [--scheme ab|aa] [--store f64|f32] [--block bx,by]
 
-A "step" is one LBM time step = one launch of the fused kernel over the whole grid.  The N=1
+A "step" is one LBM time step over the whole grid.  How many launches that is depends on the grid (include/lbm.h,
+lbm_step): D3Q19 / D3Q27 fp64 boxes without a solid mask take TWO time steps per launch (stream_collide_ab2), grids
+small enough to be resident at once take all K steps in ONE launch of the persistent kernel, every other case is one
+launch per step; `gpu_launches` and `roofline.steps_per_launch` say which it was.  The N=1
 workload is BASELINE.json configs[3] (the headline roofline run: D3Q19 BGK fp64, 512^3 periodic
 Taylor-Green vortex, tau 0.52); --config picks another one.  Prints ONE JSON line on stdout.
   value     MLUPS with the populations resident in HBM (CUDA events on the launch stream): the median of
             `repeats.n` timed segments of exactly --steps steps each
   e2e       MLUPS of the whole job through the host-buffer C-ABI calls: pinned-host rho,u -> device,
             equilibrium init, K steps, moments + diagnostics, rho,u -> pinned host
-  roofline  algorithmic bytes (2*Q*8 B per cell update) / measured kernel time vs measured HBM peak
+  roofline  algorithmic bytes (2*Q*8 B per cell update) / measured kernel time vs measured HBM peak (`frac`, SURVEY.md 8d);
+            beside it `floor_frac` = the bytes one launch cannot avoid moving (each population read once and written once
+            per LAUNCH, whether the launch takes one step or two) / launch time / peak, and `dram_frac` = the DRAM bytes
+            ncu counted for that launch (`traffic`) / launch time / peak: neither can exceed 1 by much, whatever `frac` says
   cpu_baseline  the oracle, as it stands, on this box's host cores, on a bounded sample
 With --gpus N > 1 (torchrun) every rank runs an independent replica (the path does not shard in this
 build); value = total cell updates of all ranks / max-over-ranks device time.
@@ -339,6 +345,13 @@ def run_gpu(args, w):
     # steps in pairs (stream_collide_ab2; an odd K ends with one single step) vs all K in one launch of the persistent kernel
     paired = K > 2 and 2 * launches in (K, K + 1)
     traffic, traffic_src = ncu_traffic(w.name, args.scheme + ("2" if paired else "") + ("" if args.store == "f64" else "_f32"))
+    # What one launch cannot avoid moving through HBM: every stored population read once and written once per LAUNCH —
+    # the same bytes for a one-step and for a two-step launch.  The persistent kernel keeps a small grid in the L2 over
+    # all K steps, so it has no HBM floor.
+    persistent = launches < K and not paired
+    floor_bytes = None if persistent else float(bytes_per_cell * w.N)
+    floor_frac = None if persistent else floor_bytes / (ms_per_launch * 1e-3) / 1e9 / peak
+    dram_frac = None if (persistent or traffic is None) else traffic / (ms_per_launch * 1e-3) / 1e9 / peak
     out = {
         "metric": METRIC, "value": ups / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": secs_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -363,7 +376,12 @@ def run_gpu(args, w):
                                    ("above 1: the contract's denominator is a plain device copy (MEASURED_PEAKS.json), not a hardware limit; "
                                     "see frac_of_nominal_8TBs")) if achieved > peak else None,
                      "kernel": "stream_collide_" + args.scheme + ("2 (two steps per launch)" if paired else "_persistent" if launches < K else ""), "bytes_per_cell_update": bytes_per_cell, "ms_per_launch": ms_per_launch, "steps_per_launch": K / launches,
-                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
+                     "floor_bytes_per_launch": floor_bytes, "floor_frac": floor_frac, "dram_frac": dram_frac,
+                     "bound_note": ("two steps per pass: the kernel runs at floor_frac of its own HBM floor (one read + one write of "
+                                    "every population per launch); what holds it below 1 is latency / shared-memory staging, not DRAM "
+                                    "bandwidth (profiles/README.md)") if paired else
+                                   ("all steps in one launch on an L2-resident grid: no HBM floor, not a roofline statement" if persistent else None)},
         "checks": {"mass_drift_rel": abs(d_end[0] - d_init[0]) / d_init[0], "nonfinite_cells": d_end[7],
                    "kinetic_energy_ratio": d_end[4] / d_init[4] if d_init[4] else None, "e2e_mass": d_e2e[0]},
     }

@@ -40,6 +40,13 @@ def test_bench_line_has_the_contract_keys():
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["bytes_per_cell_update"] == 304
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert abs(r["achieved"] - d["value"] * 1e6 * 304 / 1e9) <= 1e-6 * r["achieved"]
+    # what the launch itself must move (one read + one write of every population per launch, one step or two) and what ncu
+    # saw it move can never be much above the measured peak — `frac` may be (two steps per pass), these two may not
+    for rr, spl in ((r, 2), (one["roofline"], 1)):
+        assert rr["floor_bytes_per_launch"] == 304 * 128**3
+        assert abs(rr["floor_frac"] - rr["frac"] / spl) <= 1e-9 * rr["floor_frac"]
+        assert 0 < rr["floor_frac"] <= 1.2
+        assert rr["dram_frac"] is None or 0 < rr["dram_frac"] <= 1.2
     e = d["e2e"]
     assert e["unit"] == "MLUPS" and 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     c = d["cpu_baseline"]
@@ -54,3 +61,7 @@ def test_bench_runs_the_papers_examples():
         assert d["config"]["workload"] == name and d["gpu_launches"] == (1 if cfg == 7 else 30) and d["checks"]["nonfinite_cells"] == 0
         assert d["roofline"]["steps_per_launch"] == 30 / d["gpu_launches"]
         assert d["roofline"]["bytes_per_cell_update"] == 2 * (9 if cfg == 7 else 27) * 8 + 4  # + the 4-byte link mask
+        if cfg == 7:  # persistent kernel on an L2-resident grid: no HBM floor is claimed
+            assert d["roofline"]["floor_frac"] is None and d["roofline"]["dram_frac"] is None
+        else:
+            assert 0 < d["roofline"]["floor_frac"] <= 1.2 and 0 < d["roofline"]["dram_frac"] <= 1.2
