@@ -286,9 +286,11 @@ int lbm_set_block(lbm_handle h, int bx, int by);
  * index 2 + (z_global - z0), periodic wrap included, ignored beyond a non-periodic z face — because under
  * LBM_WALL_NODAL the wall-node status of a halo node depends on the plane beyond it (D:R16).  lbm_boundary_force
  * returns the part of Eq. 13 carried by the fluid nodes of the own planes: sum it over the slabs.
- * Restrictions: LBM_SCHEME_AB only; every slab must be advanced by the same number of steps; connected slabs of one
- * process need a stream each (lbm_slab_connect returns LBM_EINVAL otherwise: on a shared stream the second step of one
- * slab would wait for a step of the other that is queued behind it); lbm_init_equilibrium(_host) /
+ * Restrictions: LBM_SCHEME_AB only; every slab must be advanced by the same number of steps; under device-side
+ * ordering connected slabs of one process need a stream each (lbm_slab_connect returns LBM_EINVAL otherwise: on a shared
+ * stream the second step of one slab would wait for a step of the other that is queued behind it) — host-ordered slabs
+ * (lbm_slab_set_sync(h, 0) BEFORE lbm_slab_connect) may share a stream, the NULL stream included, as long as the
+ * caller issues the steps one per slab in turn; lbm_init_equilibrium(_host) /
  * lbm_set_populations / lbm_set_geometry need all connected slabs idle (they rewrite halo planes the neighbours
  * store into); lbm_moments(_host) / lbm_get_populations may be called between unsynchronised steps (they wait for
  * the neighbours' last step on the device and touch no memory a neighbour writes).  SYMMETRY faces are supported. */
@@ -325,7 +327,10 @@ int lbm_slab_export(lbm_handle h, lbm_slab_peer_t* out);
 int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_peer_t* upper);
 
 /* 1 = (default) device-side ordering by step counters; 0 = none: the caller synchronises all slabs between
- * steps (lbm_step(h,1); stream sync; barrier) — for debugging and for several processes on ONE device. */
+ * steps (lbm_step(h,1); stream sync; barrier) — for debugging and for several processes on ONE device; slabs of one
+ * process that share one stream need no synchronisation at all, only one step per slab in turn.  May be called before
+ * or after lbm_slab_connect; switching back to 1 on a slab that is connected to a slab on its own stream is refused
+ * (LBM_EINVAL). */
 int lbm_slab_set_sync(lbm_handle h, int device_sync);
 
 /* Message of the calling thread's last failed call ("" if none).  Static storage. */

@@ -82,6 +82,7 @@ struct lbm_handle_s {
   uint32_t* flags;        // device, 2 counters: steps finished by the lower / by the upper neighbour (they write, we wait)
   uint32_t sync_count;    // steps this slab has finished since it was created (never reset)
   int device_sync;
+  bool shares_stream;  // a connected neighbour of this process runs on this handle's stream (legal only host-ordered)
   void* peer_lo[2];       // lower / upper neighbour's population buffers as seen from this process
   void* peer_hi[2];
   long long peer_lo_N, peer_hi_N;
@@ -703,6 +704,7 @@ void close_peers(lbm_handle_s* h) {
   h->n_ipc_opened = 0;
   h->peer_lo[0] = h->peer_lo[1] = h->peer_hi[0] = h->peer_hi[1] = nullptr;
   h->peer_lo_flag = h->peer_hi_flag = nullptr;
+  h->shares_stream = false;
   cudaGetLastError();
 }
 }  // namespace
@@ -713,6 +715,7 @@ int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   close_peers(h);
   const long long plane = (long long)h->nx * h->ny;
+  bool shares = false;
   for (int side = 0; side < 2; ++side) {
     const lbm_slab_peer_t* d = side ? upper : lower;
     if (!d) continue;
@@ -721,13 +724,20 @@ int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_
     // the halo stores write the neighbour's buffer in THIS slab's lattice, element type and layout
     if (d->Q != h->Q || d->elem_bytes != (int32_t)h->elem() || d->layout_soa != h->soa)
       { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: neighbour has another lattice, storage type or layout"); }
-    // two different slabs of one process on ONE stream: the second step of one waits (in the stream) for the first step
-    // of the other, which is queued behind that wait
+    // two different slabs of one process on ONE stream.  With device-side ordering the second step of one waits (in the
+    // stream) for the first step of the other, which is queued behind that wait: refused.  Host-ordered
+    // (lbm_slab_set_sync(h, 0) before this call) the stream itself orders the steps issued slab by slab: allowed.
     if (d->pid == (int64_t)getpid() && d->buf[0] != (uint64_t)h->buf[0] && d->stream == (uint64_t)h->stream) {
       int dev = 0;
       cudaGetDevice(&dev);
-      if (d->device == dev)
-        { close_peers(h); return fail(LBM_EINVAL, "lbm_slab_connect: connected slabs of one process need a stream each (lbm_bc_t.stream)"); }
+      if (d->device == dev) {
+        if (h->device_sync) {
+          close_peers(h);
+          return fail(LBM_EINVAL, "lbm_slab_connect: connected slabs of one process need a stream each (lbm_bc_t.stream) under device-side "
+                                  "ordering; for host-ordered stepping on a shared stream call lbm_slab_set_sync(h, 0) before lbm_slab_connect");
+        }
+        shares = true;
+      }
     }
     void* b[2] = {nullptr, nullptr};
     void* fl = nullptr;
@@ -750,11 +760,14 @@ int lbm_slab_connect(lbm_handle h, const lbm_slab_peer_t* lower, const lbm_slab_
   }
   h->p.push_lo_N = h->peer_lo_N; h->p.push_lo_off = h->peer_lo_off;
   h->p.push_hi_N = h->peer_hi_N; h->p.push_hi_off = h->peer_hi_off;
+  h->shares_stream = shares;
   return LBM_OK;
 }
 
 int lbm_slab_set_sync(lbm_handle h, int device_sync) {
   if (!h || !h->slab) return fail(LBM_EINVAL, "lbm_slab_set_sync: not a slab handle");
+  if (device_sync && h->shares_stream)
+    return fail(LBM_EINVAL, "lbm_slab_set_sync: this slab is connected to a slab on the same stream; device-side ordering would deadlock there");
   h->device_sync = device_sync ? 1 : 0;
   return LBM_OK;
 }

@@ -234,9 +234,11 @@ class SlabSolver(Slab):
 
 class SlabGroup:
     """All slabs of a box in one process: slab r on devices[r % len(devices)], each on its own stream.
-    Used to test the slab path on one GPU and to drive several GPUs from one process."""
+    Used to test the slab path on one GPU and to drive several GPUs from one process.
+    shared_stream=True: every slab on the default stream instead, host-ordered (lbm_slab_set_sync(h, 0) before the
+    connect, include/lbm.h): step() issues one step per slab in turn and the one stream keeps them in order."""
 
-    def __init__(self, w, nslabs, devices=None, **kw):
+    def __init__(self, w, nslabs, devices=None, shared_stream=False, **kw):
         import torch
         self.w = w
         self.devices = list(devices) if devices else [torch.cuda.current_device()]
@@ -244,7 +246,9 @@ class SlabGroup:
         self.parts = partition(w.nz, nslabs)
         for r, (z0, nzl) in enumerate(self.parts):
             with torch.cuda.device(self._dev(r)):
-                self.slabs.append(Slab(w, z0, nzl, stream=torch.cuda.Stream(), **kw))
+                self.slabs.append(Slab(w, z0, nzl, stream=None if shared_stream else torch.cuda.Stream(), **kw))
+                if shared_stream:
+                    lbm.lbm_slab_set_sync(self.slabs[-1].h, False)
         descs = [s.descriptor() for s in self.slabs]
         for r, s in enumerate(self.slabs):
             lo, up = neighbours(r, nslabs, w.face_kind[4] == 0)
@@ -263,8 +267,12 @@ class SlabGroup:
         return out
 
     def synchronize(self):
-        for s in self.slabs:
-            s.torch_stream.synchronize()
+        import torch
+        for r, s in enumerate(self.slabs):
+            if s.torch_stream is not None:
+                s.torch_stream.synchronize()
+            else:
+                torch.cuda.default_stream(self._dev(r)).synchronize()
 
     def init_equilibrium(self):
         self.synchronize()

@@ -158,6 +158,29 @@ def test_host_synchronised_mode(mods):
     assert torch.equal(f, one)
 
 
+def test_host_ordered_slabs_may_share_a_stream(mods):
+    """Device-side ordering needs a stream per slab (a step would wait for one queued behind it) and lbm_slab_connect
+    refuses a shared one; host-ordered slabs (lbm_slab_set_sync(h, 0) BEFORE the connect) may all sit on the default
+    stream, which then orders the steps issued slab by slab — no synchronisation between steps at all."""
+    lbm, slabs = mods
+    w = workload((16, 8, 10), 19, 0.7, steps=6)
+    one, _ = single_run(lbm, w, w.steps)
+    a, b = slabs.Slab(w, 0, 5), slabs.Slab(w, 5, 5)  # both on the default stream, device-side ordering still on
+    with pytest.raises(lbm.LBMError) as ei:
+        a.connect(b.descriptor(), b.descriptor())
+    assert ei.value.code == lbm.LBM_EINVAL and "lbm_slab_set_sync" in str(ei.value)
+    a.close()
+    b.close()
+    g = slabs.SlabGroup(w, 3, shared_stream=True)
+    with pytest.raises(lbm.LBMError):
+        lbm.lbm_slab_set_sync(g.slabs[0].h, True)  # would deadlock on the shared stream
+    g.init_equilibrium()
+    g.step(w.steps)
+    f = g.get_populations()
+    g.close()
+    assert torch.equal(f, one)
+
+
 def test_moments_fields_of_the_slabs(mods):
     lbm, slabs = mods
     w = workload((12, 10, 8), 19, 0.9, faces=[P, P, P, P, B, B], force=(2e-5, 0.0, 0.0), kind="rest", steps=7)
