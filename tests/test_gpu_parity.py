@@ -2,6 +2,8 @@
 on the same seeded inputs.  Tolerances (BASELINE.json north_star): max |df| <= 1e-12 for fp64
 storage, <= 2e-5 relative for the fp32-storage variant.  Run with `pytest -m gpu` on a B200.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -318,18 +320,52 @@ def test_config2_cavity_analogue_full_length(lbm, scheme):
 
 
 def test_config2_cavity256_first_steps(lbm):
-    """configs[2] at its full 256^3 size, first 10 steps, element-wise."""
+    """configs[2] at its full 256^3 size, the first 200 steps ("else first 200 steps"), every
+    cell against the oracle, through the kernel bench.py times for this config (stream_collide_ab2 with walls).  The
+    cavity starts at rest, so the test also says how much of the box has left the rest state t_a by then (the lid's
+    shear layer, and the sound waves from the two edges where the lid runs into a side wall, which travel
+    c_s * 200 = 115 cells)."""
     w = inputs.config(2)
+    nsteps = 200
     o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u)
     s = lbm.Solver.from_workload(w)
     o.init_equilibrium(None, None)
     s.init_equilibrium(None, None)
-    o.step(10)
-    s.step(10)
+    rest = s.get_populations().cpu().numpy().copy()  # t_a everywhere
+    l0 = s.launches
+    o.step(nsteps)
+    s.step(nsteps)
+    assert s.launches - l0 == nsteps // 2  # two steps per launch: the walled two-step kernel took them
     got = s.get_populations().cpu().numpy()
-    err = float(np.abs(got - o.get_f()).max())
-    print(f"\ntest_config2_cavity256_first_steps: max|df| vs oracle = {err:.2e}")
+    ref = o.get_f()
+    err = float(np.abs(got - ref).max())
+    moved = float((np.abs(ref - rest).max(axis=0) > 1e-12).mean())
+    print(f"\ntest_config2_cavity256_first_steps: {nsteps} steps, max|df| vs oracle = {err:.2e}; "
+          f"{100 * moved:.1f} % of the cells differ from the rest state by more than 1e-12")
     assert err <= TOL
+    assert moved > 0.10  # the comparison is not one of fixed points
+    s.close()
+
+
+def test_config2_cavity_analogue_full_length_two_step_kernel(lbm):
+    """configs[2]'s full 2000 steps against the oracle, every cell, through stream_collide_ab2 with walls and lid — the
+    32^3 analogue above runs in the persistent kernel instead.  64 x 32 x 32 (two 32 x 8 tile columns in x, four in y)."""
+    w = dataclasses.replace(inputs.config(2).scaled(32), nx=64)
+    o = Oracle(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u)
+    s = lbm.Solver(w.nx, w.ny, w.nz, w.Q, w.tau, face_kind=w.face_kind, face_u=w.face_u)
+    s.set_persistent(0)
+    s.set_two_step(2)
+    o.init_equilibrium(None, None)
+    s.init_equilibrium(None, None)
+    l0 = s.launches
+    o.step(w.steps)
+    s.step(w.steps)
+    assert w.steps == 2000 and s.launches - l0 == w.steps // 2
+    err = float(np.abs(s.get_populations().cpu().numpy() - o.get_f()).max())
+    print(f"\ntest_config2_cavity_analogue_full_length_two_step_kernel: max|df| vs oracle = {err:.2e}")
+    assert err <= TOL
+    d = s.diagnostics()
+    assert abs(d[0] - w.nx * w.ny * w.nz) / (w.nx * w.ny * w.nz) < 1e-12  # mass: the lid's +- links cancel (R6)
     s.close()
 
 
