@@ -12,7 +12,8 @@ chosen from the literature.  Pinned by what the mathematics fixes, not by the or
 import numpy as np
 import pytest
 
-from oracle import Oracle, lattice
+from oracle import Oracle
+from typed_lattice import typed_lattice
 from oracle.binding import EQ_INCOMP, EQ_STANDARD
 
 P, B, M, PR = 0, 1, 2, 3
@@ -103,7 +104,7 @@ def test_brute_force_open_faces(name, fk, Q, eq):
     N = nx * ny * nz
     if Q == 9 and (fk[4] != P or fk[5] != P):
         fk = fk[:4] + [P, P]  # D2Q9 has no z links; keep z periodic
-    E, T = lattice(Q)
+    E, T = typed_lattice(Q)  # typed by hand (tests/typed_lattice.py), not the oracle's own table
     E = [tuple(int(v) for v in row) for row in E]
     rng = np.random.default_rng(11 + Q)
     f0 = (1.0 / Q) * (1.0 + 0.2 * rng.uniform(-1, 1, (Q, N)))

@@ -15,7 +15,8 @@ P:n = /root/reference/PAPER.md line n.
 import numpy as np
 import pytest
 
-from oracle import Oracle, lattice
+from oracle import Oracle
+from typed_lattice import typed_lattice
 from oracle.binding import EQ_INCOMP, EQ_STANDARD, WALL_HALFWAY, WALL_NODAL
 
 P, B, M, PR, S = 0, 1, 2, 3, 4
@@ -38,7 +39,7 @@ def _run_pair(dims, Q, eq, model, fk, doubled_axes, steps, geo=None, tau=0.63, s
     """Half box with SYMMETRY on the lower face of every axis in doubled_axes (and on the upper one too if the
     face list says so) against the mirror-extended box.  Returns max |f_half - f_doubled restricted|."""
     nx, ny, nz = dims
-    E, T = lattice(Q)
+    E, T = typed_lattice(Q)  # typed by hand (tests/typed_lattice.py), not the oracle's own table
     rng = np.random.default_rng(seed)
     f0 = T[:, None, None, None] * (1.0 + 0.2 * rng.uniform(-1, 1, (Q, nz, ny, nx)))
     g0 = np.zeros((nz, ny, nx), dtype=np.uint8) if geo is None else geo.reshape(nz, ny, nx)
@@ -244,7 +245,7 @@ def test_brute_force_all_face_kinds_with_mask(name, fk, Q, eq, nodal):
     fk = list(fk)
     if Q == 9:
         fk[4] = fk[5] = P
-    E, T = lattice(Q)
+    E, T = typed_lattice(Q)  # typed by hand (tests/typed_lattice.py), not the oracle's own table
     E = [tuple(int(v) for v in row) for row in E]
     rng = np.random.default_rng(17 + Q)
     f0 = T[:, None] * (1.0 + 0.2 * rng.uniform(-1, 1, (Q, N)))
