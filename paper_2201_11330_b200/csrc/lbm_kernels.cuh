@@ -1,10 +1,12 @@
 // lbm_kernels.cuh — hand-written sm_100a kernels of the fused stream-collide hot path.
 //
 // P:n = PAPER.md line n; D:Rk = DESIGN.md §2 reading k; S:§8 = SURVEY.md hot-path table.
-// Everything here is HBM-bound (S:§8d: 2*Q*8 B per lattice update, ~1 flop/B): no tensor
-// cores, no shared-memory staging; one thread owns one cell, the Q populations live in
-// registers, every per-direction stream is unit-stride in x (rows f[z][y][a][x]: the Q rows of one grid row are
-// adjacent).
+// Everything here is HBM-bound (S:§8d: 2*Q*8 B per lattice update, ~1 flop/B): no tensor cores.
+// The one-step-per-pass kernels (stream_collide_ab, _ab_f32x2, _aa_*, the persistent kernels) use no shared-memory
+// staging: one thread owns one cell (two in _ab_f32x2), the Q populations live in registers, every per-direction stream is
+// unit-stride in x (rows f[z][y][a][x]: the Q rows of one grid row are adjacent).
+// stream_collide_ab2 — the default for D3Q19 / D3Q27 fp64 boxes without a mask — takes TWO steps per pass: step t runs on
+// a tile extended by one cell and stays in shared memory, step t+1 runs from there.
 #pragma once
 #include <type_traits>
 #include <cstdint>
