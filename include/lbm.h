@@ -167,7 +167,16 @@ int lbm_init_equilibrium_host(lbm_handle h, const double* rho_host, const double
 
 /* Advance nsteps >= 0 time steps: per step and cell, pull-stream (Eq. 7) with wall links
  * (Eq. 10, D:R6), moments (Eq. 8-9), equilibrium (Eq. 2 / 5), BGK relaxation (Eq. 6), forcing
- * (D:R7) and store, in ONE kernel launch per step.  Asynchronous. */
+ * (D:R7) and store, all fused: nothing but the populations (and the 4-byte link mask of a geometry) touches HBM.
+ * How many kernel launches that takes depends on the handle, and the results are the same bit for bit in every regime:
+ *   - persistent: a grid small enough to be resident on the device at once, with its buffers in the L2, takes all
+ *     nsteps in ONE cooperative launch (lbm_set_persistent);
+ *   - pairs: D3Q19 / D3Q27 fp64 boxes under LBM_SCHEME_AB without a solid mask take TWO steps per launch, each
+ *     population read from HBM once and written once per two steps; an odd nsteps ends with one single step
+ *     (lbm_set_two_step lists the exact conditions);
+ *   - singles: everything else — fp32 storage, LBM_SCHEME_AA, solid masks, SYMMETRY faces, z-slabs, D2Q9 on large
+ *     grids — takes one launch per step.
+ * lbm_launch_count tells which regime ran.  Asynchronous. */
 int lbm_step(lbm_handle h, int nsteps);
 
 /* P:295-304 (PostProcessing, Monitor): moments of the current canonical state.
@@ -245,7 +254,8 @@ int64_t lbm_debug_check(lbm_handle h);
 /* Small grids (every block of the step kernel resident on the device at once, e.g. 32^3 or the paper's 512 x 128
  * channel) are bound by the launch rate of one kernel per step; for them lbm_step(h, n) takes all n steps in ONE
  * cooperative launch of a persistent kernel (a grid-wide barrier separates the steps; same arithmetic per cell, same
- * results bit for bit).  on = 0 switches that off (one launch per step, as for every larger grid); default on. */
+ * results bit for bit).  on = 0 switches that off (the grid is then stepped like a larger one: in pairs where
+ * lbm_set_two_step applies, else one launch per step); default on. */
 int lbm_set_persistent(lbm_handle h, int on);
 
 /* Two time steps per pass through HBM (Eq. 7 applied twice; the same collision, Eq. 6, in between).  For a

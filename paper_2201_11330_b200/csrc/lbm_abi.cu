@@ -939,7 +939,7 @@ int lbm_step(lbm_handle h, int nsteps) {
   if (nsteps == 0) return LBM_OK;
   Ctx c = make_ctx(h);
   // Small grids (both buffers fit the L2): all steps of this call in ONE cooperative launch of the persistent kernel;
-  // otherwise, and for slabs / in-place AA, one launch per step.
+  // otherwise pairs of steps where stream_collide_ab2 applies (below), and one launch per step for everything else.
   if (h->persistent && h->scheme == LBM_SCHEME_AB && !h->slab && nsteps >= 2 && h->l2_bytes > 0 &&
       2.0 * (double)h->buf_bytes() <= 0.8 * h->l2_bytes) {
     bool ok = false;
